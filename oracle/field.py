@@ -1,0 +1,154 @@
+"""Effective-field terms, torque and energies, fp64, written out from the paper's definitions.
+Test infrastructure.  Arrays are [component][z][y][x]; `Lnnn` = PAPER.md line.
+"""
+import numpy as np
+
+MU0 = 4e-7 * np.pi
+COMPS = (("xx", "xy", "xz"), ("xy", "yy", "yz"), ("xz", "yz", "zz"))
+
+
+# ---------------------------------------------------------------- demag (Eq. 3)
+def b_demag_direct(M, K, origin, pbc):
+    """B_i(r) = sum_r' sum_j K_ij(r - r') M_j(r'), the double sum written out (O(N^2)).
+
+    M = mu0 Msat m in tesla, [3][z][y][x]. K, origin from demag_tensor.kernel_displacements.
+    """
+    _, nz, ny, nx = M.shape
+    oz, oy, ox = origin
+    B = np.zeros_like(M)
+    zs = np.arange(nz)[:, None, None]; ys = np.arange(ny)[None, :, None]; xs = np.arange(nx)[None, None, :]
+    for z in range(nz):
+        iz = np.mod(z - zs, nz) if pbc[2] else (z - zs + oz)
+        for y in range(ny):
+            iy = np.mod(y - ys, ny) if pbc[1] else (y - ys + oy)
+            for x in range(nx):
+                ix = np.mod(x - xs, nx) if pbc[0] else (x - xs + ox)
+                for i in range(3):
+                    acc = 0.0
+                    for j in range(3):
+                        acc += (K[COMPS[i][j]][iz, iy, ix] * M[j]).sum()
+                    B[i, z, y, x] = acc
+    return B
+
+
+def b_demag_fft(M, K, origin, pbc):
+    """The same sum through the convolution theorem (L123) with numpy's fp64 FFT.
+
+    Open axes are zero-padded to 2N (any length >= 2N-1 gives the identical linear
+    convolution); periodic axes are not padded (L509).
+    """
+    _, nz, ny, nx = M.shape
+    n = (nz, ny, nx)
+    P = tuple(n[a] if pbc[2 - a] else (2 * n[a] if n[a] > 1 else 1) for a in range(3))
+    Kp = {}
+    for k, arr in K.items():
+        buf = np.zeros(P)
+        idx = []
+        for a in range(3):
+            L = arr.shape[a]
+            d = np.arange(L) - origin[a]          # displacement of every stored entry
+            idx.append(np.mod(d, P[a]))
+        buf[np.ix_(*idx)] = arr
+        Kp[k] = np.fft.rfftn(buf)
+    Mf = [np.fft.rfftn(M[j], s=P, axes=(0, 1, 2)) for j in range(3)]
+    B = np.empty_like(M)
+    for i in range(3):
+        acc = sum(Kp[COMPS[i][j]] * Mf[j] for j in range(3))
+        B[i] = np.fft.irfftn(acc, s=P, axes=(0, 1, 2))[:nz, :ny, :nx]
+    return B
+
+
+# ---------------------------------------------------------------- exchange (Eq. 6, 9)
+def exchange_table(Aex, Msat, scale):
+    """L[a, b] = S_ab * 2 (A_a/M_a)(A_b/M_b) / (A_a/M_a + A_b/M_b)  (Eq. 9), in T m^2.
+
+    `scale` is None (S = 1) or lower-triangular S[i(i+1)/2 + j], i >= j.  Msat = 0 -> A/M := 0.
+    """
+    n = len(Msat)
+    q = np.where(Msat > 0, Aex / np.where(Msat > 0, Msat, 1.0), 0.0)
+    L = np.zeros((n, n))
+    for a in range(n):
+        for b in range(n):
+            s = q[a] + q[b]
+            h = 2.0 * q[a] * q[b] / s if s > 0 else 0.0
+            i, j = max(a, b), min(a, b)
+            S = 1.0 if scale is None else scale[i * (i + 1) // 2 + j]
+            L[a, b] = S * h
+    return L
+
+
+def b_exchange(m, regions, L, cell, pbc):
+    """B_exch = sum over the 6 nearest neighbours of (2 / D_i^2) L[r, r_i] (m_i - m)  (Eq. 6).
+
+    A missing neighbour at an open boundary contributes 0 (own value used, L196);
+    periodic axes wrap (L173).
+    """
+    B = np.zeros_like(m)
+    for axis, d in ((3, cell[0]), (2, cell[1]), (1, cell[2])):       # array axes x, y, z
+        n = m.shape[axis]
+        periodic = pbc[3 - axis] > 0
+        if n == 1 and not periodic:
+            continue
+        for shift in (+1, -1):
+            mi = np.roll(m, -shift, axis=axis)                        # neighbour at +shift
+            ri = np.roll(regions, -shift, axis=axis - 1)
+            w = (2.0 / (d * d)) * L[regions, ri]
+            if not periodic:                                          # cut the wrap-around link
+                sl = [slice(None)] * 3
+                sl[axis - 1] = (n - 1) if shift == +1 else 0
+                w[tuple(sl)] = 0.0
+            B += w[None] * (mi - m)
+    return B
+
+
+# ---------------------------------------------------------------- anisotropy (Eq. 18, 21)
+def _unit(v):
+    nrm = np.sqrt((v * v).sum(axis=-1, keepdims=True))
+    return np.where(nrm > 0, v / np.where(nrm > 0, nrm, 1.0), 0.0)
+
+
+def _inv_msat(Msat):
+    return np.where(Msat > 0, 1.0 / np.where(Msat > 0, Msat, 1.0), 0.0)
+
+
+def b_anis_uniaxial(m, regions, p, only=None):
+    """Eq. 18 (L269) with B_sat read as Msat [A/m]."""
+    u = _unit(p.anisU)[regions]                                       # [z][y][x][3]
+    um = sum(u[..., c] * m[c] for c in range(3))
+    im = _inv_msat(p.Msat)[regions]
+    k1 = p.Ku1[regions] if only in (None, 1) else 0.0
+    k2 = p.Ku2[regions] if only in (None, 2) else 0.0
+    mag = 2.0 * k1 * im * um + 4.0 * k2 * im * um ** 3
+    return np.stack([mag * u[..., c] for c in range(3)])
+
+
+def b_anis_cubic(m, regions, p, only=None):
+    """Eq. 21 (L284-L286), c3 = c1 x c2."""
+    c1 = _unit(p.anisC1); c2 = _unit(p.anisC2); c3 = np.cross(c1, c2)
+    c = [c1[regions], c2[regions], c3[regions]]
+    a = [sum(ci[..., k] * m[k] for k in range(3)) for ci in c]
+    im = _inv_msat(p.Msat)[regions]
+    K1 = p.Kc1[regions] if only in (None, 1) else 0.0
+    K2 = p.Kc2[regions] if only in (None, 2) else 0.0
+    K3 = p.Kc3[regions] if only in (None, 3) else 0.0
+    B = np.zeros_like(m)
+    for i in range(3):
+        j, k = (i + 1) % 3, (i + 2) % 3
+        coef = (-2.0 * K1 * im * (a[j] ** 2 + a[k] ** 2) * a[i]
+                - 2.0 * K2 * im * (a[j] ** 2 * a[k] ** 2) * a[i]
+                - 4.0 * K3 * im * (a[j] ** 4 + a[k] ** 4) * a[i] ** 3)
+        for comp in range(3):
+            B[comp] += coef * c[i][..., comp]
+    return B
+
+
+# ---------------------------------------------------------------- torque (Eq. 2)
+def cross(a, b):
+    return np.stack([a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]])
+
+
+def ll_torque_over_gamma(m, B, alpha_cell):
+    """tau / gamma_LL = -1/(1+alpha^2) [ m x B + alpha m x (m x B) ]  (Eq. 2 with the sign of
+    SURVEY.md 8(c) #5: damping must move m towards B)."""
+    mxB = cross(m, B)
+    return -(mxB + alpha_cell[None] * cross(m, mxB)) / (1.0 + alpha_cell[None] ** 2)

@@ -1,0 +1,167 @@
+"""RefSim: the oracle's call sequence (mirrors mm_create / mm_set_* / mm_b_eff / mm_step_rk45 /
+mm_run of include/mm.h, but shares no code with it).  fp64, numpy.  Test infrastructure.
+
+Time stepping: Dormand-Prince 5(4), 7 stages with FSAL ("RK45, the Dormand-Prince method",
+PAPER.md L365), error eps = dt * max_cells ||tau_high - tau_low||_2 (L372), MaxErr 1e-5 and
+headroom 0.8 (L372-L374); the controller details are the readings of SURVEY.md 8(c) #7-#10.
+"""
+import numpy as np
+from . import demag_tensor as dt
+from . import field as fld
+
+MM_DEMAG, MM_EXCH, MM_ANIS, MM_ZEEMAN, MM_ALL = 1, 2, 4, 8, 15
+
+# Dormand-Prince tableau (textbook); tests pin row sums, order and convergence
+DP_C = (0.0, 1 / 5, 3 / 10, 4 / 5, 8 / 9, 1.0, 1.0)
+DP_A = (
+    (),
+    (1 / 5,),
+    (3 / 40, 9 / 40),
+    (44 / 45, -56 / 15, 32 / 9),
+    (19372 / 6561, -25360 / 2187, 64448 / 6561, -212 / 729),
+    (9017 / 3168, -355 / 33, 46732 / 5247, 49 / 176, -5103 / 18656),
+    (35 / 384, 0.0, 500 / 1113, 125 / 192, -2187 / 6784, 11 / 84),
+)
+DP_B5 = (35 / 384, 0.0, 500 / 1113, 125 / 192, -2187 / 6784, 11 / 84, 0.0)
+DP_B4 = (5179 / 57600, 0.0, 7571 / 16695, 393 / 640, -92097 / 339200, 187 / 2100, 1 / 40)
+DP_E = tuple(b5 - b4 for b5, b4 in zip(DP_B5, DP_B4))
+
+DIRECT_SUM_MAX_CELLS = 2048
+
+
+def _normalise(v):
+    n = np.sqrt((v * v).sum(axis=0, keepdims=True))
+    return np.where(n > 0, v / np.where(n > 0, n, 1.0), 0.0)
+
+
+class RefSim:
+    def __init__(self, grid, cell, pbc=(0, 0, 0), demag_method=None):
+        self.grid = tuple(int(g) for g in grid)
+        self.cell = tuple(float(c) for c in cell)
+        self.pbc = tuple(int(p) for p in pbc)
+        nx, ny, nz = self.grid
+        self.shape = (nz, ny, nx)
+        self.ncells = nx * ny * nz
+        self.regions = np.zeros(self.shape, dtype=np.int64)
+        self.p = None
+        self.m = None
+        self.t = 0.0
+        self.max_err, self.headroom, self.fix_dt = 1e-5, 0.8, 0.0
+        self.dt, self.dt_min, self.dt_max = 1e-14, 1e-18, 1e-9
+        self.k1 = None
+        self.n_eval = self.n_steps = self.n_rejected = 0
+        self.demag_method = demag_method or ("direct" if self.ncells <= DIRECT_SUM_MAX_CELLS else "fft")
+        self._K = None
+        self.terms = MM_ALL
+
+    # ---- setup
+    def set_terms(self, mask):
+        """Which B_eff terms drive the dynamics (the paper's EnableDemag = false, L611)."""
+        self.terms = int(mask)
+        self.k1 = None
+
+    def set_regions(self, regions):
+        self.regions = np.asarray(regions).reshape(self.shape).astype(np.int64)
+        self.k1 = None
+
+    def set_params(self, p):
+        self.p = p
+        self.L = fld.exchange_table(p.Aex, p.Msat, p.exch_scale)
+        self.k1 = None
+
+    def set_solver(self, max_err=1e-5, headroom=0.8, fix_dt=0.0, dt_init=1e-14, dt_min=1e-18, dt_max=1e-9):
+        self.max_err, self.headroom, self.fix_dt = max_err, headroom, fix_dt
+        self.dt, self.dt_min, self.dt_max = (fix_dt if fix_dt > 0 else dt_init), dt_min, dt_max
+
+    def set_m(self, m):
+        self.m = _normalise(np.asarray(m, dtype=np.float64).reshape((3,) + self.shape))
+        self.k1 = None
+
+    def kernel(self):
+        if self._K is None:
+            self._K = dt.kernel_displacements(self.grid, self.cell, self.pbc)
+        return self._K
+
+    # ---- field (L108-L113)
+    def b_demag(self, m):
+        K, origin = self.kernel()
+        M = (fld.MU0 * self.p.Msat)[self.regions][None] * m
+        fn = fld.b_demag_direct if self.demag_method == "direct" else fld.b_demag_fft
+        return fn(M, K, origin, self.pbc)
+
+    def b_eff(self, term_mask=MM_ALL, m=None):
+        m = self.m if m is None else m
+        B = np.zeros_like(m)
+        if term_mask & MM_DEMAG:
+            B += self.b_demag(m)
+        if term_mask & MM_EXCH:
+            B += fld.b_exchange(m, self.regions, self.L, self.cell, self.pbc)
+        if term_mask & MM_ANIS:
+            B += fld.b_anis_uniaxial(m, self.regions, self.p) + fld.b_anis_cubic(m, self.regions, self.p)
+        if term_mask & MM_ZEEMAN:
+            B += np.asarray(self.p.B_ext, dtype=np.float64)[:, None, None, None]
+        return B
+
+    def torque(self, m):
+        """dm/dt [1/s] (Eq. 1-2)."""
+        self.n_eval += 1
+        alpha = self.p.alpha[self.regions]
+        return self.p.gamma_LL * fld.ll_torque_over_gamma(m, self.b_eff(self.terms, m), alpha)
+
+    # ---- energies (Eq. 4, 8, 20, 23; Zeeman -M.B_ext), joules
+    def energy(self, m=None):
+        m = self.m if m is None else m
+        Ms = self.p.Msat[self.regions][None]
+        M = Ms * m
+        e = -0.5 * (M * self.b_demag(m)).sum()
+        e += -0.5 * (M * fld.b_exchange(m, self.regions, self.L, self.cell, self.pbc)).sum()
+        e += -0.5 * (M * fld.b_anis_uniaxial(m, self.regions, self.p, only=1)).sum()
+        e += -0.25 * (M * fld.b_anis_uniaxial(m, self.regions, self.p, only=2)).sum()
+        e += -(1 / 4) * (M * fld.b_anis_cubic(m, self.regions, self.p, only=1)).sum()
+        e += -(1 / 6) * (M * fld.b_anis_cubic(m, self.regions, self.p, only=2)).sum()
+        e += -(1 / 8) * (M * fld.b_anis_cubic(m, self.regions, self.p, only=3)).sum()
+        e += -(M * np.asarray(self.p.B_ext)[:, None, None, None]).sum()
+        return e * self.cell[0] * self.cell[1] * self.cell[2]
+
+    # ---- one attempted Dormand-Prince step
+    def step(self, dt_force=None):
+        if self.k1 is None:
+            self.k1 = self.torque(self.m)
+        h = self.dt if dt_force is None else dt_force
+        m0 = self.m
+        k = [self.k1]
+        y = None
+        for i in range(1, 7):
+            y = _normalise(m0 + h * sum(a * kj for a, kj in zip(DP_A[i], k)))   # every stage input
+            k.append(self.torque(y))                                              # is renormalised (#9)
+        err_vec = sum(e * kj for e, kj in zip(DP_E, k))
+        err = h * np.sqrt((err_vec * err_vec).sum(axis=0)).max()
+        fixed = self.fix_dt > 0
+        accepted = fixed or (err <= self.max_err)
+        if accepted:
+            self.m, self.k1 = y, k[6]            # y_7 is the 5th-order result; FSAL: k7 -> k1
+            self.t += h
+            self.n_steps += 1
+        else:
+            self.n_rejected += 1
+        if not fixed:
+            fac = 2.0 if err == 0 else min(2.0, max(0.5, (self.max_err / err) ** 0.2))
+            self.dt = min(self.dt_max, max(self.dt_min, h * self.headroom * fac))
+        return dict(t=self.t, dt_taken=h, dt_next=self.dt, err=err, accepted=accepted)
+
+    def run(self, duration):
+        """Advance t by exactly `duration` (last step clipped; controller's dt restored, #10)."""
+        t_end = self.t + duration
+        while t_end - self.t > 1e-12 * max(duration, 1e-30):
+            remaining = t_end - self.t
+            if self.dt >= remaining:
+                keep = self.dt
+                info = self.step(dt_force=remaining)
+                if info["accepted"]:
+                    self.dt = keep
+                    self.t = t_end
+            else:
+                self.step()
+
+    def avg_m(self):
+        return self.m.reshape(3, -1).mean(axis=1)

@@ -1,0 +1,257 @@
+"""Pins for the oracle's local field terms, torque and Dormand-Prince stepper (CPU only)."""
+import numpy as np
+import pytest
+
+from oracle import field as fld
+from oracle import sim as osim
+from oracle import RefSim, MM_DEMAG, MM_EXCH, MM_ANIS, MM_ZEEMAN, MM_ALL
+from synth import Params, random_unit_vectors
+
+GAMMA = 1.7595e11
+
+
+def _rand_m(seed, shape):
+    return random_unit_vectors(seed, int(np.prod(shape))).astype(np.float64).reshape((3,) + tuple(shape))
+
+
+# ------------------------------------------------------------------ exchange
+def test_exchange_field_vanishes_for_uniform_m():
+    rng = np.random.default_rng(0)
+    regions = rng.integers(0, 5, size=(3, 6, 7))
+    S = rng.uniform(0.5, 1.0, size=15)
+    p = Params.uniform(5, Msat=rng.uniform(5e5, 1e6, 5), Aex=rng.uniform(1e-11, 2e-11, 5), exch_scale=S)
+    L = fld.exchange_table(p.Aex, p.Msat, p.exch_scale)
+    m = np.zeros((3, 3, 6, 7)); m[0], m[1], m[2] = 0.6, 0.0, 0.8
+    for pbc in ((0, 0, 0), (1, 1, 1)):
+        assert np.abs(fld.b_exchange(m, regions, L, (1e-9, 2e-9, 3e-9), pbc)).max() == 0.0
+
+
+def test_exchange_spiral_energy_matches_the_papers_closed_form():
+    # N = 1024 cells of 1 nm with PBC, m rotating k times in the yz-plane;
+    # exact energy (Eq. 7) = vol * A * (2 pi k / (N c))^2.  Eq. 6 + Eq. 8 give instead
+    # (2A/c^2)(1 - cos theta) per unit volume, theta = 2 pi k / N.
+    N, c, A, Ms = 1024, 1e-9, 10e-12, 1e6
+    sim = RefSim((N, 1, 1), (c, c, c), (1, 0, 0))
+    sim.set_params(Params.uniform(1, Msat=Ms, Aex=A))
+    vol = N * c ** 3
+    i = np.arange(N)
+    for k in (1, 8, 32, 100):
+        phase = i * k * 2 * np.pi / N
+        m = np.zeros((3, 1, 1, N)); m[1, 0, 0] = np.sin(phase); m[2, 0, 0] = np.cos(phase)
+        B = fld.b_exchange(m, sim.regions, sim.L, sim.cell, sim.pbc)
+        E = (-0.5 * Ms * (m * B).sum()) * c ** 3                       # Eq. 8
+        theta = 2 * np.pi * k / N
+        exact = vol * A * (2 * np.pi * k / (N * c)) ** 2               # L723
+        assert np.isclose(E / exact, 2 * (1 - np.cos(theta)) / theta ** 2, rtol=1e-10)
+        if k <= 8:
+            assert np.isclose(E, exact, rtol=theta ** 2 / 10)           # small-angle limit (Fig. 5)
+
+
+def test_exchange_neumann_boundary_and_axis_spacing():
+    # 3 cells along y with a linear tilt: the middle cell sees +d and -d (field 0), the edge cells see
+    # one neighbour only; prefactor 2A/(Ms dy^2)
+    A, Ms, dy = 1.3e-11, 8e5, 2e-9
+    sim = RefSim((1, 3, 1), (5e-9, dy, 7e-9))
+    sim.set_params(Params.uniform(1, Msat=Ms, Aex=A))
+    m = np.zeros((3, 1, 3, 1)); m[0] = 1.0; m[1, 0, :, 0] = (-0.01, 0.0, 0.01)
+    B = fld.b_exchange(m, sim.regions, sim.L, sim.cell, sim.pbc)
+    assert np.isclose(B[1, 0, 0, 0], 2 * A / Ms * 0.01 / dy ** 2, rtol=1e-12)
+    assert abs(B[1, 0, 1, 0]) < 1e-12 and np.isclose(B[1, 0, 2, 0], -B[1, 0, 0, 0], rtol=1e-12)
+
+
+def test_interregion_exchange_is_the_harmonic_mean_with_scale():
+    # Eq. 9 (L208): 2 S (2 q1 q2)/(q1+q2), q = Aex/Msat; equal materials reduce to Eq. 6
+    A = np.array([1.0e-11, 2.0e-11]); M = np.array([5e5, 8e5])
+    L = fld.exchange_table(A, M, np.array([1.0, 0.25, 1.0]))
+    q = A / M
+    assert np.isclose(L[0, 0], q[0]) and np.isclose(L[1, 1], q[1])
+    assert np.isclose(L[0, 1], 0.25 * 2 * q[0] * q[1] / (q[0] + q[1])) and L[0, 1] == L[1, 0]
+    assert np.isclose(fld.exchange_table(A[[0, 0]], M[[0, 0]], None)[0, 1], q[0])
+    assert fld.exchange_table(np.array([1e-11, 0.0]), np.array([8e5, 0.0]), None)[0, 1] == 0.0   # vacuum
+
+
+# ------------------------------------------------------------------ anisotropy
+def _params_anis(rng, n):
+    p = Params.uniform(n, Msat=rng.uniform(5e5, 1e6, n), Ku1=rng.uniform(-5e5, 5e5, n), Ku2=rng.uniform(-2e5, 2e5, n),
+                       Kc1=rng.uniform(-5e4, 5e4, n), Kc2=rng.uniform(-5e4, 5e4, n), Kc3=rng.uniform(-5e4, 5e4, n))
+    p.anisU = rng.normal(size=(n, 3))
+    c1 = rng.normal(size=(n, 3)); c1 /= np.linalg.norm(c1, axis=1, keepdims=True)
+    t = rng.normal(size=(n, 3)); c2 = t - (t * c1).sum(1, keepdims=True) * c1
+    p.anisC1, p.anisC2 = c1 * 3.0, c2           # not normalised on purpose
+    return p
+
+
+def _energy_density_eq19_eq22(m, regions, p):
+    """Eq. 19 (L274) and Eq. 22 (L288, garbled; reading SURVEY.md 8(c) #6) written independently."""
+    u = p.anisU / np.linalg.norm(p.anisU, axis=1, keepdims=True)
+    c1 = p.anisC1 / np.linalg.norm(p.anisC1, axis=1, keepdims=True)
+    c2 = p.anisC2 / np.linalg.norm(p.anisC2, axis=1, keepdims=True)
+    c3 = np.cross(c1, c2)
+    dot = lambda v: np.einsum("zyxc,czyx->zyx", v[regions], m)
+    um, a1, a2, a3 = dot(u), dot(c1), dot(c2), dot(c3)
+    e = -p.Ku1[regions] * um ** 2 - p.Ku2[regions] * um ** 4
+    e += p.Kc1[regions] * (a1 ** 2 * a2 ** 2 + a1 ** 2 * a3 ** 2 + a2 ** 2 * a3 ** 2)
+    e += p.Kc2[regions] * (a1 ** 2 * a2 ** 2 * a3 ** 2)
+    e += p.Kc3[regions] * (a1 ** 4 * a2 ** 4 + a1 ** 4 * a3 ** 4 + a2 ** 4 * a3 ** 4)
+    return e
+
+
+def test_anisotropy_energy_identities_eq20_eq23():
+    rng = np.random.default_rng(5)
+    shape = (2, 3, 4)
+    regions = rng.integers(0, 3, size=shape)
+    p = _params_anis(rng, 3)
+    m = _rand_m(9, shape)
+    M = p.Msat[regions][None] * m
+    e = (-0.5 * (M * fld.b_anis_uniaxial(m, regions, p, only=1)).sum(0)
+         - 0.25 * (M * fld.b_anis_uniaxial(m, regions, p, only=2)).sum(0)
+         - (1 / 4) * (M * fld.b_anis_cubic(m, regions, p, only=1)).sum(0)
+         - (1 / 6) * (M * fld.b_anis_cubic(m, regions, p, only=2)).sum(0)
+         - (1 / 8) * (M * fld.b_anis_cubic(m, regions, p, only=3)).sum(0))
+    assert np.allclose(e, _energy_density_eq19_eq22(m, regions, p), rtol=1e-11, atol=1e-6)
+
+
+def test_anisotropy_field_is_minus_dE_dM():
+    rng = np.random.default_rng(6)
+    shape = (1, 2, 3)
+    regions = rng.integers(0, 2, size=shape)
+    p = _params_anis(rng, 2)
+    m = _rand_m(10, shape) * 0.9            # off the unit sphere on purpose: B = -dE/dM holds for any m
+    B = fld.b_anis_uniaxial(m, regions, p) + fld.b_anis_cubic(m, regions, p)
+    h = 1e-6
+    for c in range(3):
+        mp = m.copy(); mp[c] += h
+        mm = m.copy(); mm[c] -= h
+        dE = (_energy_density_eq19_eq22(mp, regions, p) - _energy_density_eq19_eq22(mm, regions, p)) / (2 * h)
+        assert np.allclose(B[c], -dE / p.Msat[regions], rtol=1e-6, atol=1e-9)
+
+
+def test_fig7_uniaxial_energy_versus_angle():
+    # L746-L763: Msat 1e6, u = x, m in the xy-plane: E = -Ku1 cos^2(theta) - Ku2 cos^4(theta)
+    p = Params.uniform(1, Msat=1000e3, Ku1=1e6, Ku2=-3e5, anisU=(1, 0, 0))
+    regions = np.zeros((1, 1, 1), dtype=int)
+    for deg in (0, 30, 77, 135, 260):
+        th = np.deg2rad(deg)
+        m = np.array([np.cos(th), np.sin(th), 0.0]).reshape(3, 1, 1, 1)
+        M = 1000e3 * m
+        e = -0.5 * (M * fld.b_anis_uniaxial(m, regions, p, only=1)).sum() - 0.25 * (M * fld.b_anis_uniaxial(m, regions, p, only=2)).sum()
+        assert np.isclose(e, -1e6 * np.cos(th) ** 2 + 3e5 * np.cos(th) ** 4, rtol=1e-12, atol=1e-6)
+
+
+# ------------------------------------------------------------------ torque and time stepping
+def _macrospin(alpha=0.0, B=(0, 0, 0.1), m0=(1, 0, 0)):
+    sim = RefSim((1, 1, 1), (1e-9, 1e-9, 1e-9))
+    sim.set_params(Params.uniform(1, Msat=1 / fld.MU0, Aex=10e-12, alpha=alpha, B_ext=B))
+    sim.set_terms(MM_EXCH | MM_ANIS | MM_ZEEMAN)         # EnableDemag = false (L611)
+    sim.set_m(np.array(m0, dtype=float).reshape(3, 1, 1, 1))
+    return sim
+
+
+def test_fig3_larmor_precession():
+    # Fig. 3 (L97): m_x = cos(gamma_LL * 0.1 T * t); frequency gamma B / 2 pi = 2.8003 GHz
+    sim = _macrospin()
+    sim.set_solver(max_err=1e-7)
+    for t in (0.1e-9, 0.35e-9, 1.0e-9):
+        sim.run(t - sim.t)
+        mx, my, mz = sim.m[:, 0, 0, 0]
+        assert abs(mx - np.cos(GAMMA * 0.1 * t)) < 2e-6 and abs(mz) < 1e-12
+        assert abs(my - np.sin(GAMMA * 0.1 * t)) < 2e-6          # sense fixed by the sign reading #5
+    assert np.isclose(GAMMA * 0.1 / (2 * np.pi), 2.8003e9, rtol=1e-4)
+
+
+def test_damping_moves_m_towards_the_field_and_lowers_the_energy():
+    sim = _macrospin(alpha=0.3, m0=(1, 0, 0.2))
+    sim.set_solver(max_err=1e-6)
+    e0, mz0 = sim.energy(), sim.m[2, 0, 0, 0]
+    sim.run(0.2e-9)
+    assert sim.m[2, 0, 0, 0] > mz0 and sim.energy() < e0
+
+
+def test_fig10_fifth_order_convergence_over_one_period():
+    # L840-L865: m = (1,0,1)/sqrt2, B = 0.1 T z, one period 2 pi/(B gamma); error ~ dt^5
+    period = 2 * np.pi / (0.1 * GAMMA)
+    errs = []
+    for n in (20, 40, 80):
+        sim = _macrospin(m0=(1, 0, 1))
+        sim.set_solver(fix_dt=period / n)
+        for _ in range(n):
+            sim.step()
+        errs.append(np.linalg.norm(sim.m[:, 0, 0, 0] - np.array([1, 0, 1]) / np.sqrt(2)))
+    assert 26 < errs[0] / errs[1] < 60 and 26 < errs[1] / errs[2] < 42    # 2^5 = 32 asymptotically
+    assert errs[2] < 1e-7
+
+
+def test_fig11_end_error_scales_with_maxerr():
+    period = 2 * np.pi / (0.1 * GAMMA)
+    errs = []
+    for tol in (1e-4, 1e-5, 1e-6):
+        sim = _macrospin(m0=(1, 0, 1))
+        sim.set_solver(max_err=tol, dt_init=1e-13)
+        sim.run(period)
+        assert abs(sim.t - period) < 1e-24
+        errs.append(np.linalg.norm(sim.m[:, 0, 0, 0] - np.array([1, 0, 1]) / np.sqrt(2)))
+    assert 3 < errs[0] / errs[1] < 30 and 3 < errs[1] / errs[2] < 30
+
+
+def test_dormand_prince_tableau_conditions():
+    A, c, b5, b4 = osim.DP_A, np.array(osim.DP_C), np.array(osim.DP_B5), np.array(osim.DP_B4)
+    for i in range(7):
+        assert abs(sum(A[i]) - c[i]) < 1e-15
+    assert tuple(A[6]) == tuple(b5[:6])                      # FSAL: stage 7 is evaluated at y_{n+1}
+    for q in range(5):                                        # quadrature conditions up to order 5 / 4
+        assert abs((b5 * c ** q).sum() - 1 / (q + 1)) < 1e-15
+    for q in range(4):
+        assert abs((b4 * c ** q).sum() - 1 / (q + 1)) < 1e-15
+    Am = np.zeros((7, 7))
+    for i in range(7):
+        Am[i, :len(A[i])] = A[i]
+    assert abs(b5 @ Am @ c - 1 / 6) < 1e-15 and abs(b4 @ Am @ c - 1 / 6) < 1e-15
+    assert abs(b5 @ Am @ Am @ c - 1 / 24) < 1e-15 and abs(b5 @ Am @ Am @ Am @ c - 1 / 120) < 1e-15
+    assert abs(sum(osim.DP_E)) < 1e-15
+
+
+def _small_film(alpha, seed=21, grid=(12, 6, 1), fix_dt=0.0):
+    sim = RefSim(grid, (4e-9, 4e-9, 3e-9))
+    sim.set_params(Params.uniform(1, Msat=8e5, Aex=1.3e-11, alpha=alpha))
+    sim.set_m(_rand_m(seed, sim.shape))
+    sim.set_solver(fix_dt=fix_dt)
+    return sim
+
+
+def test_norm_conserved_and_energy_monotone_with_damping():
+    sim = _small_film(alpha=0.5)
+    e = [sim.energy()]
+    for _ in range(40):
+        info = sim.step()
+        if info["accepted"]:
+            e.append(sim.energy())
+        assert np.abs(np.sqrt((sim.m ** 2).sum(0)) - 1).max() < 1e-14
+    e = np.array(e)
+    assert len(e) > 10 and np.all(np.diff(e) < 0)
+
+
+def test_energy_conserved_without_damping():
+    sim = _small_film(alpha=0.0)
+    sim.set_solver(max_err=1e-7)
+    e0 = sim.energy()
+    sim.run(5e-12)
+    assert abs(sim.energy() - e0) < 1e-6 * abs(e0)
+
+
+def test_run_lands_on_time_and_fsal_slope_is_consistent():
+    sim = _small_film(alpha=0.1)
+    sim.run(1e-12); sim.run(0.5e-12)
+    assert abs(sim.t - 1.5e-12) < 1e-27
+    k1 = sim.k1.copy()
+    assert np.allclose(k1, sim.torque(sim.m), rtol=0, atol=1e-3 * np.abs(k1).max() * 1e-9)
+    # fixed step: exact count, always accepted
+    sim = _small_film(alpha=0.1, fix_dt=1e-13)
+    sim.run(1e-12)
+    assert sim.n_steps == 10 and sim.n_rejected == 0 and abs(sim.t - 1e-12) < 1e-27
+
+
+def test_term_mask_sums():
+    sim = _small_film(alpha=0.1, grid=(6, 5, 2))
+    sim.p.Ku1[:] = 1e5; sim.p.B_ext = np.array([0.01, -0.02, 0.03])
+    parts = sum(sim.b_eff(t) for t in (MM_DEMAG, MM_EXCH, MM_ANIS, MM_ZEEMAN))
+    assert np.allclose(parts, sim.b_eff(MM_ALL), rtol=1e-13, atol=1e-15)
