@@ -1,0 +1,158 @@
+/* mm.h - C ABI of the B200-native micromagnetic hot path (libmm_b200.so).
+ *
+ * What it computes (citations: Lnnn = line of PAPER.md, arXiv 1406.7635, "The design and
+ * verification of MuMax3"; readings of silent/garbled passages are listed in DESIGN.md):
+ *   B_eff = B_ext + B_demag + B_exch + B_anis                         (L108-L113)
+ *   B_demag,i = K_ij * (mu0 Msat m_j), FFT-accelerated convolution     (Eq. 3)
+ *   B_exch: 6-neighbour stencil with region look-up tables             (Eq. 6, Eq. 9)
+ *   B_anis: uniaxial (Eq. 18) and cubic (Eq. 21)
+ *   torque = -gamma/(1+alpha^2) [m x B + alpha m x (m x B)]            (Eq. 2)
+ *   time stepping: Dormand-Prince RK45, FSAL, error eps = dt max|tau_hi - tau_lo|, adaptive dt
+ *   with MaxErr and headroom 0.8                                       (L365, L372-L374)
+ * All field arithmetic is fp32 on the GPU (L19, L143: "single precision"); the demag kernel is
+ * built in fp64 and truncated to fp32 (L143); time and dt are fp64.
+ *
+ * Conventions
+ *   - SI units: metres, A/m, J/m, J/m^3, tesla, seconds (as in the paper's scripts, L60-L66).
+ *   - Arrays are structure-of-arrays [component][z][y][x], x fastest; N = Nx*Ny*Nz cells, so a
+ *     vector field is 3N floats and the region map N bytes.
+ *   - Every array argument may be a HOST pointer or a DEVICE pointer (told apart with
+ *     cudaPointerGetAttributes). The caller owns every buffer it passes; the library copies
+ *     during the call and keeps no reference. The handle owns its device memory.
+ *   - All work is enqueued on the handle's CUDA stream. Calls that return data to the caller
+ *     (mm_get_*, mm_b_eff, mm_step_rk45 with info != NULL, mm_run) synchronise that stream.
+ *   - Every call returns MM_OK (0) or a negative error code; nothing throws or aborts across the
+ *     ABI. mm_last_error() gives a text for the last failure on a handle.
+ *   - A handle is not thread-safe; distinct handles are independent.
+ *   - There is no CPU fallback: without a CUDA device mm_create fails with MM_ECUDA.
+ */
+#ifndef MM_B200_H
+#define MM_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mm_sim mm_sim; /* opaque handle */
+
+enum { MM_OK = 0, MM_EINVAL = -1, MM_ENOMEM = -2, MM_ECUDA = -3, MM_ESTATE = -4, MM_ENAN = -5, MM_EDT = -6 };
+
+/* terms of B_eff (L108-L113); a mask replaces the paper's EnableDemag switch (L611) */
+enum { MM_DEMAG = 1, MM_EXCH = 2, MM_ANIS = 4, MM_ZEEMAN = 8, MM_ALL = 15 };
+
+#define MM_MAX_REGIONS 256 /* "region index between 0 and 256", L43 */
+
+/* Per-region material look-up tables (L43, Fig. 1) and the uniform applied field.
+ * All doubles, SI; the library converts to fp32 tables on the device. Host memory only. */
+typedef struct {
+  int nregions;                     /* 1..256; region ids >= nregions in the map -> MM_EINVAL */
+  double Msat[MM_MAX_REGIONS];      /* A/m, >= 0 (0 = vacuum: no torque, no exchange) */
+  double Aex[MM_MAX_REGIONS];       /* J/m, >= 0 */
+  double alpha[MM_MAX_REGIONS];     /* damping */
+  double Ku1[MM_MAX_REGIONS];       /* J/m^3, Eq. 18 */
+  double Ku2[MM_MAX_REGIONS];
+  double anisU[MM_MAX_REGIONS][3];  /* uniaxial axis; normalised by the library */
+  double Kc1[MM_MAX_REGIONS];       /* J/m^3, Eq. 21 */
+  double Kc2[MM_MAX_REGIONS];
+  double Kc3[MM_MAX_REGIONS];
+  double anisC1[MM_MAX_REGIONS][3]; /* cubic axes c1, c2 (normalised); c3 = c1 x c2 (L286) */
+  double anisC2[MM_MAX_REGIONS][3];
+  double B_ext[3];                  /* uniform applied field, tesla */
+  const double* exch_scale;         /* NULL => S = 1; else lower-triangular S[i(i+1)/2 + j], i >= j,
+                                       nregions(nregions+1)/2 entries (Eq. 9) */
+  double gamma_LL;                  /* rad/(T s); 0 => 1.7595e11 (L859) */
+} mm_params;
+
+typedef struct {
+  double t;        /* simulation time after the attempt, s */
+  double dt_taken; /* step size that was attempted */
+  double dt_next;  /* controller's suggestion for the next attempt */
+  double err;      /* eps = dt * max_cells || sum_j e_j tau_j ||_2   (L372) */
+  int accepted;    /* 1 if the step was taken (always 1 with a fixed step) */
+  long n_eval;     /* torque evaluations so far (the paper's Neval counter, L1071) */
+} mm_step_info;
+
+/* Create a simulation box (the paper's setgridsize / setcellsize / SetPBC, L60-L61, L175).
+ * Nx,Ny,Nz >= 1 cells of dx,dy,dz metres. pbc_a = number of repeats P_a of SetPBC on each side
+ * (0 = open boundary). Builds the demagnetising kernel (fp64 on the device, L143) and its
+ * real, mirror-symmetric spectrum (L145); cost grows with N and with the PBC repeats.
+ * Padded FFT length per open axis: the smallest 2^a 3^b 5^c >= 2N-1 (1 if N == 1), per periodic
+ * axis N itself (L509), each <= 8192 (MM_EINVAL beyond, or if a periodic N is not 5-smooth).
+ * On success *out owns device memory obtained with cudaMalloc on the current device. */
+int mm_create(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, double dz, int pbc_x, int pbc_y,
+              int pbc_z);
+
+/* As mm_create, with a caller-supplied device allocator (e.g. PyTorch's caching allocator) and
+ * CUDA stream (a cudaStream_t; NULL = legacy default stream). dev_alloc returns NULL on failure. */
+int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, double dz, int pbc_x, int pbc_y,
+                 int pbc_z, void* (*dev_alloc)(size_t bytes, void* ctx), void (*dev_free)(void* ptr, void* ctx),
+                 void* alloc_ctx, void* cuda_stream);
+
+/* Frees the handle and all device memory it owns. NULL is allowed. */
+int mm_destroy(mm_sim* sim);
+
+/* Region index of every cell (L43): N bytes [z][y][x]. Default: all 0. */
+int mm_set_regions(mm_sim* sim, const uint8_t* regions);
+
+/* Material tables and applied field. Rebuilds the device look-up tables (1-D tables per region and
+ * the lower-triangular inter-region exchange table, Fig. 1 L31) and invalidates the FSAL slope. */
+int mm_set_params(mm_sim* sim, const mm_params* params);
+
+/* Which B_eff terms drive the dynamics (default MM_ALL). */
+int mm_set_terms(mm_sim* sim, unsigned term_mask);
+
+/* Solver settings (L372-L374). max_err: MaxErr eps0 (default 1e-5); headroom (default 0.8);
+ * fix_dt > 0 selects a fixed step (every step accepted), 0 = adaptive; dt_init: first trial step
+ * (default 1e-14 s); dt_min/dt_max clip the controller (defaults 1e-18, 1e-9).
+ * Pass 0 for any argument to keep its default. */
+int mm_set_solver(mm_sim* sim, double max_err, double headroom, double fix_dt, double dt_init, double dt_min,
+                  double dt_max);
+
+/* Reduced magnetisation: 3N floats; normalised to unit length on entry (L85). Cells with
+ * Msat = 0 keep m = 0. Invalidates the FSAL slope. mm_get_m copies the current m out. */
+int mm_set_m(mm_sim* sim, const float* m);
+int mm_get_m(mm_sim* sim, float* m_out);
+
+/* Effective field of the current m for the selected terms, tesla, 3N floats (L108-L113). */
+int mm_b_eff(mm_sim* sim, unsigned term_mask, float* B_out);
+
+/* Torque dm/dt of the current m divided by gamma_LL (tesla), all enabled terms (Eq. 2). */
+int mm_torque(mm_sim* sim, float* tau_over_gamma_out);
+
+/* One attempted Dormand-Prince step (L365). With info == NULL the step is only enqueued (no
+ * synchronisation); otherwise the stream is synchronised and *info filled.
+ * MM_ESTATE before mm_set_params + mm_set_m; MM_ENAN if the error estimate is not finite. */
+int mm_step_rk45(mm_sim* sim, mm_step_info* info_or_null);
+
+/* n attempted steps, enqueued back to back without host synchronisation (the paper's steps(n),
+ * L1072, counting rejected attempts too). Synchronises once at the end. */
+int mm_steps(mm_sim* sim, int n);
+
+/* Advance time by exactly `duration` seconds (the paper's run(t), L74): the last step is clipped
+ * to land on the end time and the controller's suggestion is restored afterwards. The accept /
+ * reject decision and the step-size update happen on the device; the host only polls the time.
+ * MM_EDT if the step size falls below dt_min; MM_ENAN on a non-finite error estimate. */
+int mm_run(mm_sim* sim, double duration);
+
+int mm_get_time(mm_sim* sim, double* t);
+int mm_set_time(mm_sim* sim, double t);
+/* Plain mean of m over all cells (fp64 accumulation), the paper's m.average() (L861). */
+int mm_get_avg_m(mm_sim* sim, double avg[3]);
+/* Counters: accepted steps, rejected attempts, torque evaluations, peak device bytes owned. */
+int mm_get_stats(mm_sim* sim, long* steps, long* rejected, long* evals, size_t* peak_device_bytes);
+/* Padded FFT sizes chosen for this box (Px, Py, Pz). */
+int mm_get_fft_size(mm_sim* sim, int P[3]);
+/* Number of kernel launches the library has issued on this handle (for bench.py). */
+int mm_get_launch_count(mm_sim* sim, long* launches);
+
+const char* mm_last_error(const mm_sim* sim);
+const char* mm_strerror(int code);
+const char* mm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MM_B200_H */

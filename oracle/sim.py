@@ -75,6 +75,8 @@ class RefSim:
 
     def set_m(self, m):
         self.m = _normalise(np.asarray(m, dtype=np.float64).reshape((3,) + self.shape))
+        if self.p is not None:                      # vacuum cells (Msat = 0) carry no magnetisation (#12)
+            self.m = self.m * (self.p.Msat[self.regions] > 0)[None]
         self.k1 = None
 
     def kernel(self):

@@ -1,0 +1,214 @@
+// local_rk.cuh - local field terms, Landau-Lifshitz torque and the Dormand-Prince stage kernels.
+#pragma once
+#include "common.cuh"
+
+__device__ __forceinline__ int tri_index(int a, int b) {  // lower-triangular table index (Fig. 1, L31)
+  int i = max(a, b), j = min(a, b);
+  return i * (i + 1) / 2 + j;
+}
+
+// B_eff = [B_demag] + B_exch (Eq. 6 / Eq. 9) + B_anis (Eq. 18, 21) + B_ext, then either stored as the
+// field (out_torque = 0) or turned into the torque over gamma (Eq. 2, sign reading DESIGN.md #5).
+// One thread per cell; x fastest so every global access of a warp is one contiguous segment.
+__global__ void k_local(Geometry g, const uint8_t* __restrict__ regions, const Luts* __restrict__ lut, DevState* st,
+                        int m_role, int bd_role, int dst_role, unsigned mask, int out_torque) {
+  if (st->skip) return;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= g.N) return;
+  const float* __restrict__ m = st->ptr[m_role];
+  const float* __restrict__ bd = st->ptr[bd_role];
+  float* __restrict__ dst = st->ptr[dst_role];
+  const long long N = g.N;
+  const int x = (int)(i % g.Nx);
+  const long long t = i / g.Nx;
+  const int y = (int)(t % g.Ny), z = (int)(t / g.Ny);
+  const int r = regions[i];
+  const float mx = m[i], my = m[N + i], mz = m[2 * N + i];
+  float bx = 0.f, by = 0.f, bz = 0.f;
+  if (mask & MM_DEMAG) { bx = bd[i]; by = bd[N + i]; bz = bd[2 * N + i]; }
+  if (mask & MM_EXCH) {
+    float ex = 0.f, ey = 0.f, ez = 0.f;
+    auto nb = [&](long long j, float w) {
+      float a = w * __ldg(&lut->exch[tri_index(r, regions[j])]);
+      ex += a * (m[j] - mx); ey += a * (m[N + j] - my); ez += a * (m[2 * N + j] - mz);
+    };
+    if (g.Nx > 1) {
+      if (x + 1 < g.Nx) nb(i + 1, g.inv_dx2); else if (g.pbc[0]) nb(i + 1 - g.Nx, g.inv_dx2);
+      if (x > 0) nb(i - 1, g.inv_dx2); else if (g.pbc[0]) nb(i - 1 + g.Nx, g.inv_dx2);
+    }
+    if (g.Ny > 1) {
+      const long long s = g.Nx;
+      if (y + 1 < g.Ny) nb(i + s, g.inv_dy2); else if (g.pbc[1]) nb(i + s - s * g.Ny, g.inv_dy2);
+      if (y > 0) nb(i - s, g.inv_dy2); else if (g.pbc[1]) nb(i - s + s * g.Ny, g.inv_dy2);
+    }
+    if (g.Nz > 1) {
+      const long long s = (long long)g.Nx * g.Ny;
+      if (z + 1 < g.Nz) nb(i + s, g.inv_dz2); else if (g.pbc[2]) nb(i + s - s * g.Nz, g.inv_dz2);
+      if (z > 0) nb(i - s, g.inv_dz2); else if (g.pbc[2]) nb(i - s + s * g.Nz, g.inv_dz2);
+    }
+    bx += ex; by += ey; bz += ez;
+  }
+  if (mask & MM_ANIS) {
+    if (lut->has_uniaxial) {
+      float ux = lut->u[0][r], uy = lut->u[1][r], uz = lut->u[2][r];
+      float um = ux * mx + uy * my + uz * mz;
+      float s = lut->ku1[r] * um + lut->ku2[r] * um * um * um;
+      bx += s * ux; by += s * uy; bz += s * uz;
+    }
+    if (lut->has_cubic) {
+      float c1x = lut->c1[0][r], c1y = lut->c1[1][r], c1z = lut->c1[2][r];
+      float c2x = lut->c2[0][r], c2y = lut->c2[1][r], c2z = lut->c2[2][r];
+      float c3x = lut->c3[0][r], c3y = lut->c3[1][r], c3z = lut->c3[2][r];
+      float a1 = c1x * mx + c1y * my + c1z * mz, a2 = c2x * mx + c2y * my + c2z * mz, a3 = c3x * mx + c3y * my + c3z * mz;
+      float q1 = a1 * a1, q2 = a2 * a2, q3 = a3 * a3;
+      float k1 = lut->kc1[r], k2 = lut->kc2[r], k3 = lut->kc3[r];
+      float f1 = (k1 * (q2 + q3) + k2 * (q2 * q3) + k3 * (q2 * q2 + q3 * q3) * q1) * a1;
+      float f2 = (k1 * (q1 + q3) + k2 * (q1 * q3) + k3 * (q1 * q1 + q3 * q3) * q2) * a2;
+      float f3 = (k1 * (q1 + q2) + k2 * (q1 * q2) + k3 * (q1 * q1 + q2 * q2) * q3) * a3;
+      bx += f1 * c1x + f2 * c2x + f3 * c3x;
+      by += f1 * c1y + f2 * c2y + f3 * c3y;
+      bz += f1 * c1z + f2 * c2z + f3 * c3z;
+    }
+  }
+  if (mask & MM_ZEEMAN) { bx += lut->bext[0]; by += lut->bext[1]; bz += lut->bext[2]; }
+  if (out_torque) {
+    const float al = lut->alpha[r];
+    const float pre = -lut->live[r] / (1.f + al * al);
+    float tx = my * bz - mz * by, ty = mz * bx - mx * bz, tz = mx * by - my * bx;   // m x B
+    float dx = my * tz - mz * ty, dy = mz * tx - mx * tz, dz = mx * ty - my * tx;   // m x (m x B)
+    bx = pre * (tx + al * dx); by = pre * (ty + al * dy); bz = pre * (tz + al * dz);
+  }
+  dst[i] = bx; dst[N + i] = by; dst[2 * N + i] = bz;
+}
+
+// Dormand-Prince stage input y_i = normalise(m0 + h sum_j a_ij k_j) (L365; every stage input is
+// renormalised, reading #9). k_j are torques over gamma [T], hg = gamma * h.
+struct StageCoef { float a[6]; int n; };
+
+__global__ void k_stage(long long N, DevState* st, StageCoef sc, int dst_role) {
+  if (st->skip) return;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const float* __restrict__ m = st->ptr[R_M];
+  const float hg = st->hg;
+  float sx = 0.f, sy = 0.f, sz = 0.f;
+#pragma unroll
+  for (int j = 0; j < 6; ++j) {
+    if (j < sc.n && sc.a[j] != 0.f) {
+      const float* __restrict__ k = st->ptr[R_K0 + j];
+      sx += sc.a[j] * k[i]; sy += sc.a[j] * k[N + i]; sz += sc.a[j] * k[2 * N + i];
+    }
+  }
+  float yx = m[i] + hg * sx, yy = m[N + i] + hg * sy, yz = m[2 * N + i] + hg * sz;
+  float n2 = yx * yx + yy * yy + yz * yz;
+  float inv = n2 > 0.f ? rsqrtf(n2) : 0.f;
+  float* __restrict__ dst = st->ptr[dst_role];
+  dst[i] = yx * inv; dst[N + i] = yy * inv; dst[2 * N + i] = yz * inv;
+}
+
+// eps / h = max_cells || sum_j e_j k_j ||_2   (L372; Euclidean norm, reading #8)
+struct ErrCoef { float e[7]; };
+
+__global__ void k_error(long long N, DevState* st, ErrCoef ec) {
+  if (st->skip) return;
+  float best = 0.f;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+    float sx = 0.f, sy = 0.f, sz = 0.f;
+#pragma unroll
+    for (int j = 0; j < 7; ++j) {
+      if (ec.e[j] != 0.f) {
+        const float* __restrict__ k = st->ptr[R_K0 + j];
+        sx += ec.e[j] * k[i]; sy += ec.e[j] * k[N + i]; sz += ec.e[j] * k[2 * N + i];
+      }
+    }
+    float n = sqrtf(sx * sx + sy * sy + sz * sz);
+    best = (n > best || n != n) ? n : best;          // NaN propagates
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    float other = __shfl_xor_sync(0xffffffffu, best, o);
+    best = (other > best || other != other) ? other : best;
+  }
+  if ((threadIdx.x & 31) == 0) {
+    unsigned bits = (best != best) ? 0x7fc00000u : __float_as_uint(best);   // NaN sorts above +inf
+    atomicMax(&st->err_bits, bits);
+  }
+}
+
+// Step-size control on the device (single thread each).
+// begin: choose the step h of this attempt; in run mode clip it to land exactly on t_end
+// (reading #10) or mark the run as finished (skip = 1: the rest of the step is a no-op).
+__global__ void k_ctrl_begin(DevState* st) {
+  if (st->status != MM_OK) { st->skip = 1; return; }
+  double h = st->fix_dt > 0 ? st->fix_dt : st->dt;
+  st->clipped = 0;
+  if (st->run_mode) {
+    double remaining = st->t_end - st->t;
+    if (!(remaining > 1e-12 * fmax(st->run_duration, 1e-30))) { st->skip = 1; return; }
+    if (h >= remaining) { st->keep_dt = h; h = remaining; st->clipped = 1; }
+  }
+  st->skip = 0;
+  st->h = h;
+  st->hg = (float)(st->gamma * h);
+  st->err_bits = 0u;
+}
+
+// end: eps = h * max|...|; accept iff fixed step or eps <= MaxErr; on accept swap the roles
+// m <-> y7 and k1 <-> k7 (FSAL); dt <- dt * headroom * clamp((MaxErr/eps)^(1/5), 0.5, 2) (L372-L374,
+// DESIGN.md readings #7-#9).
+__global__ void k_ctrl_end(DevState* st) {
+  if (st->skip) return;
+  const float emax = __uint_as_float(st->err_bits);
+  const double h = st->h;
+  const double err = (double)emax * st->gamma * h;
+  st->last_err = (float)err;
+  st->evals += 6;
+  if (!(err == err) || isinf(err)) { st->status = MM_ENAN; st->last_accepted = 0; st->skip = 1; return; }
+  const bool fixed = st->fix_dt > 0;
+  const bool accept = fixed || err <= st->max_err;
+  st->last_accepted = accept ? 1 : 0;
+  if (accept) {
+    float* p = st->ptr[R_M]; st->ptr[R_M] = st->ptr[R_MNEW]; st->ptr[R_MNEW] = p;
+    p = st->ptr[R_K0]; st->ptr[R_K0] = st->ptr[R_K6]; st->ptr[R_K6] = p;
+    st->t = st->clipped ? st->t_end : st->t + h;
+    st->steps += 1;
+  } else {
+    st->rejected += 1;
+  }
+  if (!fixed) {
+    if (accept && st->clipped) {
+      st->dt = st->keep_dt;
+    } else {
+      double fac = (err == 0.0) ? 2.0 : fmin(2.0, fmax(0.5, pow(st->max_err / err, 0.2)));
+      double dt = h * st->headroom * fac;
+      dt = fmin(st->dt_max, fmax(st->dt_min, dt));
+      if (!accept && h <= st->dt_min) { st->status = MM_EDT; st->skip = 1; }
+      st->dt = dt;
+    }
+  }
+}
+
+// |m| = 1 on entry (L85); vacuum cells (Msat = 0) and zero vectors stay 0
+__global__ void k_normalise(long long N, float* __restrict__ m, const uint8_t* __restrict__ regions,
+                            const Luts* __restrict__ lut) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  float x = m[i], y = m[N + i], z = m[2 * N + i];
+  float n2 = x * x + y * y + z * z;
+  float inv = (n2 > 0.f ? rsqrtf(n2) : 0.f) * lut->live[regions[i]];
+  m[i] = x * inv; m[N + i] = y * inv; m[2 * N + i] = z * inv;
+}
+
+// plain mean of m (fp64 accumulation); out[3] must be zeroed first
+__global__ void k_sum3(long long N, const float* __restrict__ m, double* __restrict__ out) {
+  double s[3] = {0.0, 0.0, 0.0};
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+    s[0] += m[i]; s[1] += m[N + i]; s[2] += m[2 * N + i];
+  }
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s[c] += __shfl_xor_sync(0xffffffffu, s[c], o);
+    if ((threadIdx.x & 31) == 0) atomicAdd(&out[c], s[c]);
+  }
+}

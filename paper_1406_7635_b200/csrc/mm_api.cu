@@ -1,0 +1,614 @@
+// mm_api.cu - the C ABI of include/mm.h: handle, host-side planning, launch sequences.
+// Every step of the path runs in the kernels of this directory; nothing here computes fields on
+// the host and there is no CPU fallback.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "internal.cuh"
+#include "demag_conv.cuh"
+#include "local_rk.cuh"
+
+namespace {
+
+constexpr int kMaxFft = 8192;
+constexpr size_t kSmemMax = 232448;  // 227 KB opt-in limit per CTA on sm_100
+
+// Dormand-Prince 5(4) tableau (PAPER.md L365 names the method; coefficients: DESIGN.md)
+const double DP_A[7][6] = {
+    {0, 0, 0, 0, 0, 0},
+    {1.0 / 5, 0, 0, 0, 0, 0},
+    {3.0 / 40, 9.0 / 40, 0, 0, 0, 0},
+    {44.0 / 45, -56.0 / 15, 32.0 / 9, 0, 0, 0},
+    {19372.0 / 6561, -25360.0 / 2187, 64448.0 / 6561, -212.0 / 729, 0, 0},
+    {9017.0 / 3168, -355.0 / 33, 46732.0 / 5247, 49.0 / 176, -5103.0 / 18656, 0},
+    {35.0 / 384, 0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84}};
+const double DP_E[7] = {35.0 / 384 - 5179.0 / 57600, 0.0, 500.0 / 1113 - 7571.0 / 16695, 125.0 / 192 - 393.0 / 640,
+                        -2187.0 / 6784 + 92097.0 / 339200, 11.0 / 84 - 187.0 / 2100, -1.0 / 40};
+
+
+bool smooth5(int n) {
+  for (int f : {2, 3, 5}) while (n % f == 0) n /= f;
+  return n == 1;
+}
+
+int padded_length(int N, int periodic) {
+  if (periodic) return N;
+  if (N == 1) return 1;
+  int p = 2 * N - 1;
+  while (!smooth5(p)) ++p;
+  return p;
+}
+
+AxisPlan make_plan(int N, int P) {
+  AxisPlan pl;
+  memset(&pl, 0, sizeof(pl));
+  pl.N = N; pl.P = P;
+  int r = P;
+  for (int f : {8, 4, 2, 3, 5})
+    while (r % f == 0 && pl.npass < MM_MAX_PASSES) { pl.radix[pl.npass++] = f; r /= f; }
+  return pl;
+}
+
+}  // namespace
+
+
+namespace {
+
+bool is_device_ptr(const void* p) {
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+int copy_in(mm_sim* s, void* dst, const void* src, size_t bytes) {
+  CUDA_TRY(s, cudaMemcpyAsync(dst, src, bytes, is_device_ptr(src) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice,
+                              s->stream));
+  if (!is_device_ptr(src)) CUDA_TRY(s, cudaStreamSynchronize(s->stream));  // caller may free its buffer on return
+  return MM_OK;
+}
+
+int copy_out(mm_sim* s, void* dst, const void* src, size_t bytes) {
+  CUDA_TRY(s, cudaMemcpyAsync(dst, src, bytes, is_device_ptr(dst) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost,
+                              s->stream));
+  CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+  return MM_OK;
+}
+
+int pull_state(mm_sim* s) {
+  CUDA_TRY(s, cudaMemcpyAsync(&s->hst, s->dstate, sizeof(DevState), cudaMemcpyDeviceToHost, s->stream));
+  CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+  return MM_OK;
+}
+
+int push_state(mm_sim* s) {
+  CUDA_TRY(s, cudaMemcpyAsync(s->dstate, &s->hst, sizeof(DevState), cudaMemcpyHostToDevice, s->stream));
+  CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+  return MM_OK;
+}
+
+
+int upload_twiddles(mm_sim* s, int P, float2** out) {
+  std::vector<float2> tw(P);
+  for (int k = 0; k < P; ++k) {
+    double a = -2.0 * M_PI * (double)k / (double)P;
+    tw[k] = make_float2((float)cos(a), (float)sin(a));
+  }
+  *out = (float2*)mm_dev_alloc(s, sizeof(float2) * P);
+  if (!*out) return mm_fail(s, MM_ENOMEM, "twiddle table");
+  CUDA_TRY(s, cudaMemcpy(*out, tw.data(), sizeof(float2) * P, cudaMemcpyHostToDevice));
+  return MM_OK;
+}
+
+template <typename KernelT>
+int opt_in_smem(mm_sim* s, KernelT k) {
+  CUDA_TRY(s, cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax));
+  return MM_OK;
+}
+
+int configure_launches(mm_sim* s) {
+  const Geometry& g = s->g;
+  int rc;
+  if ((rc = opt_in_smem(s, k_x_fwd))) return rc;
+  if ((rc = opt_in_smem(s, k_x_inv))) return rc;
+  if ((rc = opt_in_smem(s, k_y_axis))) return rc;
+  if ((rc = opt_in_smem(s, k_last_fused<1>))) return rc;
+  if ((rc = opt_in_smem(s, k_last_fused<2>))) return rc;
+  if ((rc = opt_in_smem(s, k_last_fused<3>))) return rc;
+  auto pick = [](int P, int nbuf, int want_points, int cmax) {
+    size_t per = (size_t)nbuf * P * sizeof(float2);
+    int c = want_points / P;
+    if (c < 1) c = 1;
+    if (c > cmax) c = cmax;
+    while (c > 1 && per * c > 98304) --c;       // prefer >= 2 CTAs per SM
+    return c;
+  };
+  s->xL = pick(g.Px, 2, 4096, 64);
+  s->xSmem = (size_t)2 * s->xL * g.Px * sizeof(float2);
+  s->yC = pick(g.Py, 2, 4096, 32);
+  s->ySmem = (size_t)2 * s->yC * g.Py * sizeof(float2);
+  s->last_along_z = g.Pz > 1;
+  const int Pl = s->last_along_z ? g.Pz : g.Py;
+  const int ncs[3] = {2, 1, 3};  // coupled components of modes 0, 1, 2
+  for (int mode = 0; mode < 3; ++mode) {
+    s->lastC[mode] = pick(Pl, ncs[mode] + 1, 4096, 32);
+    s->lastSmem[mode] = (size_t)(ncs[mode] + 1) * s->lastC[mode] * Pl * sizeof(float2);
+    if (s->lastSmem[mode] > kSmemMax) return mm_fail(s, MM_EINVAL, "FFT length too large for shared memory");
+  }
+  if (s->xSmem > kSmemMax || s->ySmem > kSmemMax) return mm_fail(s, MM_EINVAL, "FFT length too large for shared memory");
+  return MM_OK;
+}
+
+// B_demag of the field in role `src` -> role R_B
+void launch_demag(mm_sim* s, int src_role) {
+  const Geometry& g = s->g;
+  const int rows = g.Ny * g.Nz, pairs = (rows + 1) / 2;
+  const int T = 256;
+  dim3 gx((pairs + s->xL - 1) / s->xL, 3);
+  k_x_fwd<<<gx, T, s->xSmem, s->stream>>>(s->conv, src_role, s->xL);
+  s->launches++;
+  if (s->last_along_z) {
+    dim3 gy((g.Cx + s->yC - 1) / s->yC, g.Nz, 3);
+    if (g.Py > 1) { k_y_axis<<<gy, T, s->ySmem, s->stream>>>(s->conv, 0, s->yC); s->launches++; }
+    dim3 gl((g.Cx + s->lastC[2] - 1) / s->lastC[2], g.Py);
+    k_last_fused<3><<<gl, T, s->lastSmem[2], s->stream>>>(s->conv, 2, s->lastC[2]);
+    s->launches++;
+    if (g.Py > 1) { k_y_axis<<<gy, T, s->ySmem, s->stream>>>(s->conv, 1, s->yC); s->launches++; }
+  } else {
+    dim3 g0((g.Cx + s->lastC[0] - 1) / s->lastC[0]);
+    k_last_fused<2><<<g0, T, s->lastSmem[0], s->stream>>>(s->conv, 0, s->lastC[0]);
+    dim3 g1((g.Cx + s->lastC[1] - 1) / s->lastC[1]);
+    k_last_fused<1><<<g1, T, s->lastSmem[1], s->stream>>>(s->conv, 1, s->lastC[1]);
+    s->launches += 2;
+  }
+  k_x_inv<<<gx, T, s->xSmem, s->stream>>>(s->conv, R_B, s->xL);
+  s->launches++;
+}
+
+// field (out_torque = 0) or torque over gamma (out_torque = 1) of role `src` into role `dst`
+void launch_eval(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_torque) {
+  if (mask & MM_DEMAG) launch_demag(s, src_role);
+  k_local<<<blocks_for(s->g.N, 256), 256, 0, s->stream>>>(s->g, s->regions, s->luts, s->dstate, src_role, R_B, dst_role,
+                                                         mask, out_torque);
+  s->launches++;
+}
+
+void enqueue_step(mm_sim* s) {
+  const long long N = s->g.N;
+  if (!s->have_k1) {
+    launch_eval(s, R_M, R_K0, s->terms, 1);
+    s->have_k1 = true;
+  }
+  k_ctrl_begin<<<1, 1, 0, s->stream>>>(s->dstate);
+  s->launches++;
+  for (int i = 1; i < 7; ++i) {
+    StageCoef sc;
+    sc.n = i;
+    for (int j = 0; j < 6; ++j) sc.a[j] = (float)DP_A[i][j];
+    const int yrole = (i == 6) ? R_MNEW : R_Y;
+    k_stage<<<blocks_for(N, 256), 256, 0, s->stream>>>(N, s->dstate, sc, yrole);
+    s->launches++;
+    launch_eval(s, yrole, R_K0 + i, s->terms, 1);
+  }
+  ErrCoef ec;
+  for (int j = 0; j < 7; ++j) ec.e[j] = (float)DP_E[j];
+  k_error<<<148 * 8, 256, 0, s->stream>>>(N, s->dstate, ec);
+  k_ctrl_end<<<1, 1, 0, s->stream>>>(s->dstate);
+  s->launches += 2;
+}
+
+int check_ready(mm_sim* s) {
+  if (!s) return MM_EINVAL;
+  if (!s->have_params) return mm_fail(s, MM_ESTATE, "mm_set_params has not been called");
+  if (!s->have_m) return mm_fail(s, MM_ESTATE, "mm_set_m has not been called");
+  return MM_OK;
+}
+
+int status_to_error(mm_sim* s) {
+  if (s->hst.status == MM_ENAN) return mm_fail(s, MM_ENAN, "non-finite error estimate");
+  if (s->hst.status == MM_EDT) return mm_fail(s, MM_EDT, "step size fell below dt_min");
+  return MM_OK;
+}
+
+}  // namespace
+
+
+void* mm_default_alloc(size_t bytes, void*) {
+  void* p = nullptr;
+  if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  return p;
+}
+void mm_default_free(void* p, void*) { cudaFree(p); }
+
+int mm_fail(mm_sim* s, int code, const std::string& msg) {
+  if (s) s->err = msg;
+  return code;
+}
+
+void* mm_dev_alloc(mm_sim* s, size_t bytes) {
+  void* p = s->alloc(bytes ? bytes : 16, s->alloc_ctx);
+  if (!p) return nullptr;
+  s->owned.emplace_back(p, bytes);
+  s->cur_bytes += bytes;
+  if (s->cur_bytes > s->peak_bytes) s->peak_bytes = s->cur_bytes;
+  return p;
+}
+
+void mm_dev_free(mm_sim* s, void* p) {
+  if (!p) return;
+  for (size_t i = 0; i < s->owned.size(); ++i)
+    if (s->owned[i].first == p) {
+      s->cur_bytes -= s->owned[i].second;
+      s->owned.erase(s->owned.begin() + i);
+      break;
+    }
+  s->dealloc(p, s->alloc_ctx);
+}
+
+extern "C" {
+
+int mm_create(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, double dz, int pbc_x, int pbc_y, int pbc_z) {
+  return mm_create_ex(out, Nx, Ny, Nz, dx, dy, dz, pbc_x, pbc_y, pbc_z, nullptr, nullptr, nullptr, nullptr);
+}
+
+int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, double dz, int pbc_x, int pbc_y, int pbc_z,
+                 void* (*dev_alloc_cb)(size_t, void*), void (*dev_free_cb)(void*, void*), void* alloc_ctx,
+                 void* cuda_stream) {
+  if (!out) return MM_EINVAL;
+  *out = nullptr;
+  if (Nx < 1 || Ny < 1 || Nz < 1 || !(dx > 0) || !(dy > 0) || !(dz > 0) || pbc_x < 0 || pbc_y < 0 || pbc_z < 0 ||
+      !std::isfinite(dx) || !std::isfinite(dy) || !std::isfinite(dz) || (dev_alloc_cb == nullptr) != (dev_free_cb == nullptr))
+    return MM_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return MM_ECUDA; }
+  mm_sim* s = new (std::nothrow) mm_sim();
+  if (!s) return MM_ENOMEM;
+  if (dev_alloc_cb) { s->alloc = dev_alloc_cb; s->dealloc = dev_free_cb; s->alloc_ctx = alloc_ctx; }
+  s->stream = (cudaStream_t)cuda_stream;
+  s->cell[0] = dx; s->cell[1] = dy; s->cell[2] = dz;
+  s->rep[0] = pbc_x; s->rep[1] = pbc_y; s->rep[2] = pbc_z;
+  Geometry& g = s->g;
+  g.Nx = Nx; g.Ny = Ny; g.Nz = Nz;
+  g.N = (long long)Nx * Ny * Nz;
+  g.Px = padded_length(Nx, pbc_x); g.Py = padded_length(Ny, pbc_y); g.Pz = padded_length(Nz, pbc_z);
+  g.pbc[0] = pbc_x > 0; g.pbc[1] = pbc_y > 0; g.pbc[2] = pbc_z > 0;
+  g.inv_dx2 = (float)(1.0 / (dx * dx)); g.inv_dy2 = (float)(1.0 / (dy * dy)); g.inv_dz2 = (float)(1.0 / (dz * dz));
+  auto bail = [&](int code, const char* msg) {
+    fprintf(stderr, "mm_create: %s\n", msg);
+    mm_destroy(s);
+    return code;
+  };
+  if (g.Px > kMaxFft || g.Py > kMaxFft || g.Pz > kMaxFft) return bail(MM_EINVAL, "padded FFT length above 8192");
+  if (!smooth5(g.Px) || !smooth5(g.Py) || !smooth5(g.Pz)) return bail(MM_EINVAL, "periodic axis length must be 2^a 3^b 5^c");
+  g.Cx = g.Px / 2 + 1;
+  g.pitch = g.Cx;
+  g.Hy = g.Py / 2 + 1; g.Hz = g.Pz / 2 + 1;
+  s->px = make_plan(Nx, g.Px); s->py = make_plan(Ny, g.Py); s->pz = make_plan(Nz, g.Pz);
+  int rc;
+  if ((rc = configure_launches(s))) { std::string m = s->err; return bail(rc, m.c_str()); }
+  // device memory
+  const size_t fbytes = sizeof(float) * 3 * (size_t)g.N;
+  for (int r = 0; r < R_COUNT; ++r) {
+    s->field[r] = (float*)mm_dev_alloc(s, fbytes);
+    if (!s->field[r]) return bail(MM_ENOMEM, "field arrays");
+  }
+  s->regions = (uint8_t*)mm_dev_alloc(s, (size_t)g.N);
+  s->luts = (Luts*)mm_dev_alloc(s, sizeof(Luts));
+  s->dstate = (DevState*)mm_dev_alloc(s, sizeof(DevState));
+  s->scratch3 = (double*)mm_dev_alloc(s, 3 * sizeof(double));
+  const int rowsS = (g.Pz == 1) ? g.Ny : g.Nz * g.Py;
+  s->spec = (float2*)mm_dev_alloc(s, sizeof(float2) * 3 * (size_t)rowsS * g.pitch);
+  if (!s->regions || !s->luts || !s->dstate || !s->spec || !s->scratch3) return bail(MM_ENOMEM, "device buffers");
+  if (cudaMemsetAsync(s->regions, 0, (size_t)g.N, s->stream) != cudaSuccess) return bail(MM_ECUDA, "memset");
+  for (int r = 0; r < R_COUNT; ++r) cudaMemsetAsync(s->field[r], 0, fbytes, s->stream);
+  if ((rc = upload_twiddles(s, g.Px, &s->twx)) || (rc = upload_twiddles(s, g.Py, &s->twy)) ||
+      (rc = upload_twiddles(s, g.Pz, &s->twz)))
+    return bail(rc, "twiddles");
+  if ((rc = mm_build_kernel_spectrum(s))) { std::string m = s->err; return bail(rc, m.c_str()); }
+  // convolution arguments
+  ConvArgs& c = s->conv;
+  c.g = g; c.px = s->px; c.py = s->py; c.pz = s->pz;
+  c.twx = s->twx; c.twy = s->twy; c.twz = s->twz;
+  c.spec = s->spec; c.rowsS = rowsS; c.cstride = (long long)rowsS * g.pitch;
+  c.K = s->K; c.kstride = (long long)g.Cx * g.Hy * g.Hz;
+  c.regions = s->regions; c.luts = s->luts; c.st = s->dstate;
+  // controller state
+  DevState& h = s->hst;
+  memset(&h, 0, sizeof(h));
+  for (int r = 0; r < R_COUNT; ++r) h.ptr[r] = s->field[r];
+  h.max_err = 1e-5; h.headroom = 0.8; h.fix_dt = 0.0; h.dt = 1e-14; h.dt_min = 1e-18; h.dt_max = 1e-9;
+  h.gamma = 1.7595e11;
+  h.status = MM_OK;
+  if ((rc = push_state(s))) { std::string m = s->err; return bail(rc, m.c_str()); }
+  *out = s;
+  return MM_OK;
+}
+
+int mm_destroy(mm_sim* s) {
+  if (!s) return MM_OK;
+  cudaStreamSynchronize(s->stream);
+  while (!s->owned.empty()) mm_dev_free(s, s->owned.back().first);
+  delete s;
+  return MM_OK;
+}
+
+int mm_set_regions(mm_sim* s, const uint8_t* regions) {
+  if (!s || !regions) return mm_fail(s, MM_EINVAL, "null argument");
+  // validate ids against the current table size on the host copy
+  std::vector<uint8_t> tmp;
+  const uint8_t* host = regions;
+  if (is_device_ptr(regions)) {
+    tmp.resize((size_t)s->g.N);
+    CUDA_TRY(s, cudaMemcpy(tmp.data(), regions, (size_t)s->g.N, cudaMemcpyDeviceToHost));
+    host = tmp.data();
+  }
+  if (s->have_params) {
+    for (long long i = 0; i < s->g.N; ++i)
+      if (host[i] >= s->nregions) return mm_fail(s, MM_EINVAL, "region id >= nregions");
+  }
+  int rc = copy_in(s, s->regions, regions, (size_t)s->g.N);
+  s->have_k1 = false;
+  return rc;
+}
+
+int mm_set_params(mm_sim* s, const mm_params* p) {
+  if (!s || !p) return mm_fail(s, MM_EINVAL, "null argument");
+  const int n = p->nregions;
+  if (n < 1 || n > MM_MAX_REGIONS) return mm_fail(s, MM_EINVAL, "nregions out of range");
+  for (int r = 0; r < n; ++r) {
+    if (!(p->Msat[r] >= 0) || !(p->Aex[r] >= 0) || !std::isfinite(p->Msat[r]) || !std::isfinite(p->Aex[r]) ||
+        !std::isfinite(p->alpha[r]) || !std::isfinite(p->Ku1[r]) || !std::isfinite(p->Ku2[r]) ||
+        !std::isfinite(p->Kc1[r]) || !std::isfinite(p->Kc2[r]) || !std::isfinite(p->Kc3[r]))
+      return mm_fail(s, MM_EINVAL, "non-finite or negative material parameter");
+  }
+  std::vector<uint8_t> reg((size_t)s->g.N);
+  CUDA_TRY(s, cudaMemcpyAsync(reg.data(), s->regions, (size_t)s->g.N, cudaMemcpyDeviceToHost, s->stream));
+  CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+  for (long long i = 0; i < s->g.N; ++i)
+    if (reg[i] >= n) return mm_fail(s, MM_EINVAL, "region map holds an id >= nregions");
+  Luts* L = new (std::nothrow) Luts();
+  if (!L) return mm_fail(s, MM_ENOMEM, "host LUT");
+  memset(L, 0, sizeof(Luts));
+  const double mu0 = 4e-7 * M_PI;
+  auto unit = [](const double* v, double* o) {
+    double nn = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+    for (int c = 0; c < 3; ++c) o[c] = nn > 0 ? v[c] / nn : 0.0;
+  };
+  L->nregions = n;
+  std::vector<double> q(n);
+  for (int r = 0; r < n; ++r) {
+    const double Ms = p->Msat[r], iMs = Ms > 0 ? 1.0 / Ms : 0.0;
+    q[r] = Ms > 0 ? p->Aex[r] / Ms : 0.0;
+    L->Bsat[r] = (float)(mu0 * Ms);
+    L->alpha[r] = (float)p->alpha[r];
+    L->live[r] = Ms > 0 ? 1.f : 0.f;
+    L->ku1[r] = (float)(2.0 * p->Ku1[r] * iMs);
+    L->ku2[r] = (float)(4.0 * p->Ku2[r] * iMs);
+    L->kc1[r] = (float)(-2.0 * p->Kc1[r] * iMs);
+    L->kc2[r] = (float)(-2.0 * p->Kc2[r] * iMs);
+    L->kc3[r] = (float)(-4.0 * p->Kc3[r] * iMs);
+    double u[3], c1[3], c2[3], c3[3];
+    unit(p->anisU[r], u); unit(p->anisC1[r], c1); unit(p->anisC2[r], c2);
+    c3[0] = c1[1] * c2[2] - c1[2] * c2[1]; c3[1] = c1[2] * c2[0] - c1[0] * c2[2]; c3[2] = c1[0] * c2[1] - c1[1] * c2[0];
+    for (int c = 0; c < 3; ++c) {
+      L->u[c][r] = (float)u[c]; L->c1[c][r] = (float)c1[c]; L->c2[c][r] = (float)c2[c]; L->c3[c][r] = (float)c3[c];
+    }
+    if (p->Ku1[r] != 0 || p->Ku2[r] != 0) L->has_uniaxial = 1;
+    if (p->Kc1[r] != 0 || p->Kc2[r] != 0 || p->Kc3[r] != 0) L->has_cubic = 1;
+  }
+  for (int i = 0; i < n; ++i)
+    for (int j = 0; j <= i; ++j) {
+      const double sum = q[i] + q[j];
+      const double hm = sum > 0 ? 2.0 * q[i] * q[j] / sum : 0.0;                 // Eq. 9
+      const double S = p->exch_scale ? p->exch_scale[i * (i + 1) / 2 + j] : 1.0;
+      L->exch[i * (i + 1) / 2 + j] = (float)(2.0 * S * hm);                       // the "2" of Eq. 6
+    }
+  for (int c = 0; c < 3; ++c) L->bext[c] = (float)p->B_ext[c];
+  cudaError_t e = cudaMemcpyAsync(s->luts, L, sizeof(Luts), cudaMemcpyHostToDevice, s->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  delete L;
+  CUDA_TRY(s, e);
+  int rc;
+  if ((rc = pull_state(s))) return rc;
+  s->hst.gamma = p->gamma_LL > 0 ? p->gamma_LL : 1.7595e11;
+  if ((rc = push_state(s))) return rc;
+  s->nregions = n;
+  s->have_params = true;
+  s->have_k1 = false;
+  return MM_OK;
+}
+
+int mm_set_terms(mm_sim* s, unsigned mask) {
+  if (!s) return MM_EINVAL;
+  s->terms = mask & MM_ALL;
+  s->have_k1 = false;
+  return MM_OK;
+}
+
+int mm_set_solver(mm_sim* s, double max_err, double headroom, double fix_dt, double dt_init, double dt_min, double dt_max) {
+  if (!s) return MM_EINVAL;
+  if (max_err < 0 || headroom < 0 || fix_dt < 0 || dt_init < 0 || dt_min < 0 || dt_max < 0)
+    return mm_fail(s, MM_EINVAL, "negative solver setting");
+  int rc;
+  if ((rc = pull_state(s))) return rc;
+  DevState& h = s->hst;
+  h.max_err = max_err > 0 ? max_err : 1e-5;
+  h.headroom = headroom > 0 ? headroom : 0.8;
+  h.fix_dt = fix_dt;
+  h.dt_min = dt_min > 0 ? dt_min : 1e-18;
+  h.dt_max = dt_max > 0 ? dt_max : 1e-9;
+  h.dt = fix_dt > 0 ? fix_dt : (dt_init > 0 ? dt_init : 1e-14);
+  h.status = MM_OK;
+  return push_state(s);
+}
+
+int mm_set_m(mm_sim* s, const float* m) {
+  if (!s || !m) return mm_fail(s, MM_EINVAL, "null argument");
+  if (!s->have_params) return mm_fail(s, MM_ESTATE, "mm_set_params must precede mm_set_m");
+  int rc;
+  if ((rc = pull_state(s))) return rc;
+  if ((rc = copy_in(s, s->hst.ptr[R_M], m, sizeof(float) * 3 * (size_t)s->g.N))) return rc;
+  k_normalise<<<blocks_for(s->g.N, 256), 256, 0, s->stream>>>(s->g.N, s->hst.ptr[R_M], s->regions, s->luts);
+  s->launches++;
+  CUDA_TRY(s, cudaGetLastError());
+  s->hst.status = MM_OK;
+  s->hst.skip = 0;
+  if ((rc = push_state(s))) return rc;
+  s->have_m = true;
+  s->have_k1 = false;
+  return MM_OK;
+}
+
+int mm_get_m(mm_sim* s, float* m_out) {
+  if (!s || !m_out) return mm_fail(s, MM_EINVAL, "null argument");
+  int rc;
+  if ((rc = pull_state(s))) return rc;
+  return copy_out(s, m_out, s->hst.ptr[R_M], sizeof(float) * 3 * (size_t)s->g.N);
+}
+
+int mm_b_eff(mm_sim* s, unsigned mask, float* B_out) {
+  int rc;
+  if ((rc = check_ready(s))) return rc;
+  if (!B_out) return mm_fail(s, MM_EINVAL, "null argument");
+  launch_eval(s, R_M, R_B, mask & MM_ALL, 0);
+  CUDA_TRY(s, cudaGetLastError());
+  if ((rc = pull_state(s))) return rc;
+  return copy_out(s, B_out, s->hst.ptr[R_B], sizeof(float) * 3 * (size_t)s->g.N);
+}
+
+int mm_torque(mm_sim* s, float* out) {
+  int rc;
+  if ((rc = check_ready(s))) return rc;
+  if (!out) return mm_fail(s, MM_EINVAL, "null argument");
+  launch_eval(s, R_M, R_Y, s->terms, 1);
+  CUDA_TRY(s, cudaGetLastError());
+  if ((rc = pull_state(s))) return rc;
+  return copy_out(s, out, s->hst.ptr[R_Y], sizeof(float) * 3 * (size_t)s->g.N);
+}
+
+int mm_step_rk45(mm_sim* s, mm_step_info* info) {
+  int rc;
+  if ((rc = check_ready(s))) return rc;
+  enqueue_step(s);
+  CUDA_TRY(s, cudaGetLastError());
+  if (!info) return MM_OK;
+  if ((rc = pull_state(s))) return rc;
+  const DevState& h = s->hst;
+  info->t = h.t; info->dt_taken = h.h; info->dt_next = h.fix_dt > 0 ? h.fix_dt : h.dt; info->err = h.last_err;
+  info->accepted = h.last_accepted; info->n_eval = (long)h.evals;
+  return status_to_error(s);
+}
+
+int mm_steps(mm_sim* s, int n) {
+  int rc;
+  if ((rc = check_ready(s))) return rc;
+  if (n < 0) return mm_fail(s, MM_EINVAL, "negative step count");
+  for (int i = 0; i < n; ++i) enqueue_step(s);
+  CUDA_TRY(s, cudaGetLastError());
+  if ((rc = pull_state(s))) return rc;
+  return status_to_error(s);
+}
+
+int mm_run(mm_sim* s, double duration) {
+  int rc;
+  if ((rc = check_ready(s))) return rc;
+  if (!(duration >= 0) || !std::isfinite(duration)) return mm_fail(s, MM_EINVAL, "bad duration");
+  if (duration == 0) return MM_OK;
+  if ((rc = pull_state(s))) return rc;
+  s->hst.run_mode = 1;
+  s->hst.t_end = s->hst.t + duration;
+  s->hst.run_duration = duration;
+  s->hst.skip = 0;
+  if ((rc = push_state(s))) return rc;
+  int batch = 4;
+  for (;;) {
+    for (int i = 0; i < batch; ++i) enqueue_step(s);
+    CUDA_TRY(s, cudaGetLastError());
+    if ((rc = pull_state(s))) return rc;
+    if (s->hst.skip || s->hst.status != MM_OK) break;
+    // size the next batch from the remaining time and the current step suggestion (host only polls)
+    double dt = s->hst.fix_dt > 0 ? s->hst.fix_dt : s->hst.dt;
+    double est = (s->hst.t_end - s->hst.t) / (dt > 0 ? dt : 1e-18);
+    batch = est > 256 ? 64 : (est > 32 ? 16 : 4);
+  }
+  const int st = s->hst.status;
+  s->hst.run_mode = 0;
+  s->hst.skip = 0;
+  if ((rc = push_state(s))) return rc;
+  s->hst.status = st;
+  return status_to_error(s);
+}
+
+int mm_get_time(mm_sim* s, double* t) {
+  if (!s || !t) return MM_EINVAL;
+  int rc;
+  if ((rc = pull_state(s))) return rc;
+  *t = s->hst.t;
+  return MM_OK;
+}
+
+int mm_set_time(mm_sim* s, double t) {
+  if (!s) return MM_EINVAL;
+  int rc;
+  if ((rc = pull_state(s))) return rc;
+  s->hst.t = t;
+  return push_state(s);
+}
+
+int mm_get_avg_m(mm_sim* s, double avg[3]) {
+  if (!s || !avg) return MM_EINVAL;
+  int rc;
+  if ((rc = pull_state(s))) return rc;
+  CUDA_TRY(s, cudaMemsetAsync(s->scratch3, 0, 3 * sizeof(double), s->stream));
+  k_sum3<<<148 * 4, 256, 0, s->stream>>>(s->g.N, s->hst.ptr[R_M], s->scratch3);
+  s->launches++;
+  CUDA_TRY(s, cudaGetLastError());
+  if ((rc = copy_out(s, avg, s->scratch3, 3 * sizeof(double)))) return rc;
+  for (int c = 0; c < 3; ++c) avg[c] /= (double)s->g.N;
+  return MM_OK;
+}
+
+int mm_get_stats(mm_sim* s, long* steps, long* rejected, long* evals, size_t* peak) {
+  if (!s) return MM_EINVAL;
+  int rc;
+  if ((rc = pull_state(s))) return rc;
+  if (steps) *steps = (long)s->hst.steps;
+  if (rejected) *rejected = (long)s->hst.rejected;
+  if (evals) *evals = (long)s->hst.evals;
+  if (peak) *peak = s->peak_bytes;
+  return MM_OK;
+}
+
+int mm_get_fft_size(mm_sim* s, int P[3]) {
+  if (!s || !P) return MM_EINVAL;
+  P[0] = s->g.Px; P[1] = s->g.Py; P[2] = s->g.Pz;
+  return MM_OK;
+}
+
+int mm_get_launch_count(mm_sim* s, long* launches) {
+  if (!s || !launches) return MM_EINVAL;
+  *launches = s->launches;
+  return MM_OK;
+}
+
+const char* mm_last_error(const mm_sim* s) { return s ? s->err.c_str() : "null handle"; }
+
+const char* mm_strerror(int code) {
+  switch (code) {
+    case MM_OK: return "ok";
+    case MM_EINVAL: return "invalid argument";
+    case MM_ENOMEM: return "out of device memory";
+    case MM_ECUDA: return "CUDA error (or no CUDA device)";
+    case MM_ESTATE: return "call sequence error";
+    case MM_ENAN: return "non-finite error estimate";
+    case MM_EDT: return "step size below dt_min";
+    default: return "unknown error";
+  }
+}
+
+const char* mm_version(void) { return "mm_b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,254 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 oracle on the same seeded inputs.
+
+Tolerances:
+  field   max|dB| <= 1e-4 * max|B|  (north_star), checked per term and for the sum;
+  <m>     |d<m>| <= 1e-3 at equal physical time (north_star, C2);
+  m(t)    element-wise bounds stated at each test (fp32 round-off amplified by the dynamics).
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from oracle import RefSim, MM_DEMAG, MM_EXCH, MM_ANIS, MM_ZEEMAN, MM_ALL
+from synth import (Params, random_unit_vectors, config_c1, config_c2, config_c3, config_c4, config_c5,
+                   voronoi_regions)
+
+FIELD_TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def mm():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1406_7635_b200 import build
+    build.build()
+    import paper_1406_7635_b200 as mm
+    return mm
+
+
+def _ref_from(cfg, demag_method=None):
+    ref = RefSim(cfg["grid"], cfg["cell"], cfg["pbc"], demag_method=demag_method)
+    if cfg.get("regions") is not None:
+        ref.set_regions(cfg["regions"])
+    ref.set_params(cfg["params"])
+    ref.set_m(cfg["m0"])
+    return ref
+
+
+def _field_check(sim, ref, masks=(MM_DEMAG, MM_EXCH, MM_ANIS, MM_ZEEMAN, MM_ALL)):
+    for mask in masks:
+        B = sim.b_eff(mask).astype(np.float64)
+        Br = ref.b_eff(mask)
+        scale = np.abs(Br).max()
+        if scale == 0:
+            assert np.abs(B).max() == 0
+            continue
+        err = np.abs(B - Br).max() / scale
+        assert err <= FIELD_TOL, (mask, err)
+
+
+def _rand_cfg(grid, cell, pbc=(0, 0, 0), nreg=1, seed=5, anis=False):
+    nx, ny, nz = grid
+    rng = np.random.default_rng(seed)
+    regions = rng.integers(0, nreg, size=(nz, ny, nx)).astype(np.uint8) if nreg > 1 else None
+    p = Params.uniform(nreg, Msat=rng.uniform(6e5, 1e6, nreg), Aex=rng.uniform(1e-11, 2e-11, nreg),
+                       alpha=rng.uniform(0.05, 0.5, nreg), B_ext=(0.01, -0.02, 0.005))
+    if nreg > 1:
+        p.exch_scale = rng.uniform(0.5, 1.0, nreg * (nreg + 1) // 2)
+    if anis:
+        p.Ku1 = rng.uniform(-3e5, 5e5, nreg); p.Ku2 = rng.uniform(-1e5, 1e5, nreg)
+        p.anisU = rng.normal(size=(nreg, 3))
+        p.Kc1 = rng.uniform(-5e4, 5e4, nreg); p.Kc2 = rng.uniform(-5e4, 5e4, nreg); p.Kc3 = rng.uniform(-5e4, 5e4, nreg)
+        c1 = rng.normal(size=(nreg, 3)); c1 /= np.linalg.norm(c1, axis=1, keepdims=True)
+        t = rng.normal(size=(nreg, 3)); c2 = t - (t * c1).sum(1, keepdims=True) * c1
+        p.anisC1, p.anisC2 = c1, c2
+    m0 = random_unit_vectors(seed, nx * ny * nz).reshape(3, nz, ny, nx)
+    return dict(grid=grid, cell=cell, pbc=pbc, regions=regions, params=p, m0=m0)
+
+
+# --------------------------------------------------------------------------- fields
+def test_c1_field_direct_sum(mm):
+    cfg = config_c1()
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "direct")          # O(N^2) Newell summation (BASELINE.json config 1)
+    _field_check(sim, ref, (MM_DEMAG, MM_EXCH, MM_DEMAG | MM_EXCH, MM_ALL))
+    assert sim.fft_size() == (128, 32, 1)
+
+
+@pytest.mark.parametrize("grid,cell,pbc", [
+    ((37, 23, 1), (3e-9, 4e-9, 2e-9), (0, 0, 0)),        # ragged, padded to 75 x 45 (radices 3, 5)
+    ((50, 30, 1), (4e-9, 4e-9, 3e-9), (0, 0, 0)),
+    ((1, 1, 1), (1e-9, 1e-9, 1e-9), (0, 0, 0)),          # single cell: every FFT has length 1
+    ((33, 1, 1), (2e-9, 2e-9, 2e-9), (0, 0, 0)),         # chain
+    ((1, 17, 3), (2e-9, 3e-9, 2e-9), (0, 0, 0)),
+    ((20, 12, 5), (2e-9, 2e-9, 2e-9), (0, 0, 0)),        # 3D
+    ((16, 12, 3), (2e-9, 2e-9, 3e-9), (2, 0, 0)),        # PBC in x
+    ((12, 10, 4), (2e-9, 2e-9, 2e-9), (1, 2, 0)),        # PBC in x and y
+    ((6, 5, 8), (3e-9, 2e-9, 1e-9), (0, 0, 3)),          # PBC in z
+    ((9, 1, 1), (2e-9, 2e-9, 2e-9), (4, 0, 0)),
+])
+def test_small_grids_all_terms(mm, grid, cell, pbc):
+    n = grid[0] * grid[1] * grid[2]
+    cfg = _rand_cfg(grid, cell, pbc, nreg=4 if n > 8 else 1, anis=True)
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "direct" if n <= 1500 else "fft")
+    _field_check(sim, ref)
+
+
+def test_multi_tile_2d_and_3d_fields(mm):
+    # several CTAs per kernel and a ragged tail in every direction
+    for grid, cell in (((300, 150, 1), (4e-9, 4e-9, 2e-9)), ((70, 45, 20), (2e-9, 2e-9, 2e-9))):
+        cfg = _rand_cfg(grid, cell, nreg=7, anis=True, seed=9)
+        sim = mm.from_config(cfg)
+        ref = _ref_from(cfg, "fft")
+        _field_check(sim, ref)
+
+
+def test_uniform_m_has_no_exchange_field_and_film_limit(mm):
+    cfg = _rand_cfg((64, 64, 1), (5e-9, 5e-9, 1e-9), pbc=(32, 32, 0), nreg=1)
+    cfg["m0"][:] = 0; cfg["m0"][2] = 1.0
+    sim = mm.from_config(cfg)
+    assert np.abs(sim.b_eff(MM_EXCH)).max() == 0.0
+    Bd = sim.b_eff(MM_DEMAG)
+    bsat = 4e-7 * np.pi * cfg["params"].Msat[0]
+    assert np.allclose(Bd[2], -bsat, rtol=1e-2) and np.abs(Bd[:2]).max() < 1e-6 * bsat   # thin film: -mu0 Msat mz
+
+
+def test_c3_field_full_size(mm):
+    cfg = config_c3()
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    _field_check(sim, ref)
+
+
+def test_c5_field_with_and_without_pbc(mm):
+    for pbc in (False, True):
+        cfg = config_c5(64, pbc=pbc)
+        sim = mm.from_config(cfg)
+        ref = _ref_from(cfg, "fft")
+        _field_check(sim, ref, (MM_DEMAG, MM_EXCH, MM_ANIS, MM_ALL))
+        assert sim.fft_size() == ((64, 64, 128) if pbc else (128, 128, 128))
+
+
+def test_torque_matches_eq2(mm):
+    cfg = _rand_cfg((24, 10, 3), (2e-9, 2e-9, 2e-9), nreg=3, anis=True)
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg)
+    tau = sim.torque().astype(np.float64) * cfg["params"].gamma_LL
+    tr = ref.torque(ref.m)
+    assert np.abs(tau - tr).max() <= FIELD_TOL * np.abs(tr).max()
+
+
+# --------------------------------------------------------------------------- time stepping
+def test_macrospin_larmor_precession(mm):
+    # Fig. 3 (L97): m_x = cos(gamma B t) in B = 0.1 T, no damping, demag off
+    p = Params.uniform(1, Msat=1 / (4e-7 * np.pi), Aex=10e-12, alpha=0.0, B_ext=(0, 0, 0.1))
+    sim = mm.Sim((1, 1, 1), (1e-9, 1e-9, 1e-9))
+    sim.set_params(p); sim.set_terms(MM_EXCH | MM_ANIS | MM_ZEEMAN)
+    sim.set_m(np.array([1, 0, 0], dtype=np.float32).reshape(3, 1, 1, 1))
+    sim.set_solver(max_err=1e-6)
+    for t in (0.1e-9, 0.5e-9, 1e-9):
+        sim.run(t - sim.t)
+        assert abs(sim.t - t) < 1e-21
+        m = sim.get_m().ravel()
+        w = 1.7595e11 * 0.1 * t
+        assert abs(m[0] - np.cos(w)) < 2e-4 and abs(m[1] - np.sin(w)) < 2e-4 and abs(m[2]) < 1e-6
+        assert abs(np.linalg.norm(m) - 1) < 1e-6
+
+
+def test_c1_fixed_step_trajectory(mm):
+    # BASELINE.json config 1: one B_eff, then 200 fixed steps of 1e-13 s; oracle demag by direct sum
+    cfg = config_c1()
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "direct")
+    sim.set_solver(fix_dt=cfg["fix_dt"]); ref.set_solver(fix_dt=cfg["fix_dt"])
+    sim.steps(cfg["nsteps"])
+    for _ in range(cfg["nsteps"]):
+        ref.step()
+    assert abs(sim.t - ref.t) < 1e-24 and sim.stats()["steps"] == 200
+    m = sim.get_m().astype(np.float64)
+    assert np.abs(np.sqrt((m ** 2).sum(0)) - 1).max() < 1e-6
+    # 1200 fp32 torque evaluations on a random (rough) state: element-wise drift stays ~1e-4
+    assert np.abs(m - ref.m).max() < 2e-3
+    assert np.abs(sim.avg_m() - ref.avg_m()).max() < 1e-4
+
+
+def test_adaptive_run_equal_time_and_controller(mm):
+    cfg = _rand_cfg((40, 24, 1), (4e-9, 4e-9, 3e-9), nreg=1, seed=13)
+    cfg["params"].alpha[:] = 0.3
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    sim.run(20e-12); ref.run(20e-12)
+    assert abs(sim.t - 20e-12) < 1e-24
+    st = sim.stats()
+    assert st["steps"] > 10 and abs(st["steps"] - ref.n_steps) <= max(3, ref.n_steps // 10)
+    m = sim.get_m().astype(np.float64)
+    assert np.abs(m - ref.m).max() < 2e-3 and np.abs(sim.avg_m() - ref.avg_m()).max() < 2e-4
+    # a single further attempt reports a consistent error estimate and step suggestion
+    a, b = sim.step(), ref.step()
+    assert a["accepted"] == b["accepted"]
+    assert abs(a["dt_taken"] - b["dt_taken"]) < 0.1 * b["dt_taken"] and abs(a["err"] - b["err"]) < 0.2 * b["err"]
+
+
+def test_c2_reduced_relax_then_reversal(mm):
+    # the C2 protocol (alpha = 1 relax, then alpha = 0.02 with the reversal field), shortened
+    cfg = config_c2()
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    sim.run(0.3e-9); ref.run(0.3e-9)
+    assert np.abs(sim.avg_m() - ref.avg_m()).max() < 1e-3
+    p = cfg["params"]
+    p.alpha[:] = cfg["alpha_dyn"]; p.B_ext = np.array(cfg["B_ext_dyn"])
+    sim.set_params(p); ref.set_params(p)
+    for _ in range(10):
+        sim.run(cfg["sample_dt"]); ref.run(cfg["sample_dt"])
+        assert np.abs(sim.avg_m() - ref.avg_m()).max() < 1e-3
+
+
+def test_c3_reduced_adaptive_steps(mm):
+    cfg = config_c3(grid=(32, 32, 8), ngrains=12)
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    _field_check(sim, ref)
+    sim.steps(30)
+    ref.run(sim.t)                       # several dt sequences are valid: compare at equal time (#10)
+    m = sim.get_m().astype(np.float64)
+    assert np.abs(m - ref.m).max() < 5e-3 and np.abs(sim.avg_m() - ref.avg_m()).max() < 1e-3
+
+
+# --------------------------------------------------------------------------- boundary behaviour
+def test_error_codes_and_state(mm):
+    sim = mm.Sim((8, 4, 1), (2e-9, 2e-9, 2e-9))
+    with pytest.raises(mm.MMError) as e:
+        sim.step()
+    assert e.value.code == mm.MM_ESTATE
+    p = Params.uniform(2, Msat=8e5, Aex=1.3e-11, alpha=0.1)
+    sim.set_params(p)
+    with pytest.raises(mm.MMError) as e:
+        sim.set_regions(np.full((1, 4, 8), 3, dtype=np.uint8))
+    assert e.value.code == mm.MM_EINVAL
+    bad = Params.uniform(1, Msat=-1.0)
+    with pytest.raises(mm.MMError) as e:
+        sim.set_params(bad)
+    assert e.value.code == mm.MM_EINVAL
+    with pytest.raises(mm.MMError):
+        mm.Sim((5000, 4, 1), (2e-9, 2e-9, 2e-9))      # padded length above the supported maximum
+
+
+def test_device_pointers_and_vacuum_cells(mm):
+    import torch
+    cfg = _rand_cfg((16, 8, 2), (2e-9, 2e-9, 2e-9), nreg=2)
+    cfg["params"].Msat[1] = 0.0                        # region 1 is vacuum (reading #12)
+    sim = mm.from_config(cfg)
+    m_dev = torch.from_numpy(cfg["m0"]).cuda()
+    sim.set_m(m_dev)                                   # device pointer in
+    out = torch.empty_like(m_dev)
+    sim.b_eff(MM_ALL, out=out)                         # device pointer out
+    ref = _ref_from(cfg)
+    Br = ref.b_eff(MM_ALL)
+    assert np.abs(out.cpu().numpy() - Br).max() <= FIELD_TOL * np.abs(Br).max()
+    m = sim.get_m()
+    assert np.all(m[:, cfg["regions"] == 1] == 0)
+    sim.steps(3)
+    assert np.all(sim.get_m()[:, cfg["regions"] == 1] == 0)
