@@ -1,0 +1,295 @@
+#!/usr/bin/env python
+"""bench.py - throughput of the micromagnetic hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--size 4096] [--impl ours|reference]
+
+A "step" is one Dormand-Prince RK45 step (6 torque evaluations: demag FFT convolution + exchange +
+Zeeman, torque, stage combinations, error norm, controller) of the C4 workload of BASELINE.json: a
+size x size x 1 Permalloy film, 4x4x2 nm cells, seeded random m, B_ext = 10 mT, fixed dt = 1e-13 s
+(deterministic count, no rejections).  metric: cell-updates/s = cells * steps / time, whole job.
+N > 1 runs N independent replicas (the path does not shard): weak scaling.
+Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "LLG cell-updates/s per RK45 step (demag+exchange)"
+UNIT = "cell-updates/s"
+STEP_BYTES_PER_CELL = 1272.0      # algorithmic bytes per cell per RK45 step, 2D open
+
+
+def measured_peak_gbs():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured"
+    except Exception:
+        return 6650.0, "fallback"       # B200_PROFILING.md fallback
+
+
+def kernel_bytes(kind, n, P):
+    """Algorithmic bytes of ONE launch of a kernel class of the 2D path.
+    n = cells per side, P = padded FFT length; Cx = P/2+1 stored kx, Hy = P/2+1 kernel rows."""
+    N, Cx, Hy = n * n, P // 2 + 1, P // 2 + 1
+    spec = n * Cx * 8               # one component of the half spectrum, rows y < n
+    table = {
+        "x_fwd": 12 * N + N + 3 * spec,
+        "last_xy": 2 * spec + 3 * Hy * Cx * 4 + 2 * spec,
+        "last_z": spec + Hy * Cx * 4 + spec,
+        "x_inv": 3 * spec + 12 * N,
+        "local": 12 * N + 12 * N + N + 12 * N,
+        "rk_stage": 12 * N * (1 + 26.0 / 6.0) + 12 * N,      # m0 + on average 26/6 slopes in, y out
+        "rk_error": 12 * N * 6,
+        # fused kernels of the fast 2D path
+        "kA": 12 * N * (1 + 26.0 / 6.0) + N + 12 * N + 3 * spec,
+        "kB": 6 * spec + 4 * Hy * Cx * 4,
+        "kC": 3 * spec + 12 * N + N + 12 * N,
+    }
+    return float(table.get(kind, 0.0))
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "200"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        time.sleep(0.25)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        self.f.close()
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            out = {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                   "samples": len(sm)}
+        return out
+
+
+def run_reference(args, rank):
+    """The oracle as it stands, on the host cores: a bounded sample of the same workload."""
+    if rank != 0:
+        return
+    from oracle import RefSim
+    from synth import config_c4
+    n = args.cpu_size
+    cfg = config_c4(n)
+    ref = RefSim(cfg["grid"], cfg["cell"], cfg["pbc"], demag_method="fft")
+    ref.set_params(cfg["params"]); ref.set_m(cfg["m0"]); ref.set_solver(fix_dt=cfg["fix_dt"])
+    steps = max(1, min(args.steps, args.cpu_steps))
+    for _ in range(min(args.warmup, 1)):
+        ref.step()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        ref.step()
+    dt = time.perf_counter() - t0
+    value = n * n * steps / dt
+    sample = "C4 recipe at %dx%dx1, %d RK45 steps (numpy fp64, FFT demag)" % (n, n, steps)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * dt / steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "C4 film %dx%dx1 (bounded sample of the %d^2 workload)" % (n, n, args.size),
+                       "cells": n * n, "fix_dt": cfg["fix_dt"]},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def cpu_baseline(args):
+    from oracle import RefSim
+    from synth import config_c4
+    n = args.cpu_size
+    cfg = config_c4(n)
+    ref = RefSim(cfg["grid"], cfg["cell"], cfg["pbc"], demag_method="fft")
+    ref.set_params(cfg["params"]); ref.set_m(cfg["m0"]); ref.set_solver(fix_dt=cfg["fix_dt"])
+    ref.step()
+    t0 = time.perf_counter()
+    for _ in range(args.cpu_steps):
+        ref.step()
+    dt = time.perf_counter() - t0
+    return {"value": n * n * args.cpu_steps / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": "C4 recipe at %dx%dx1, %d RK45 steps (numpy fp64, FFT demag, single thread)" % (n, n, args.cpu_steps)}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--size", type=int, default=4096)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-size", type=int, default=256)
+    ap.add_argument("--cpu-steps", type=int, default=12)
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the mm_b200 path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    from paper_1406_7635_b200 import build
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    import paper_1406_7635_b200 as mm
+    from synth import config_c4
+
+    n = args.size
+    cfg = config_c4(n)
+    sim = mm.from_config(cfg)
+    sim.set_solver(fix_dt=cfg["fix_dt"])
+    P = sim.fft_size()[0]
+    cells = n * n
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps between two events
+    sim.steps(args.warmup)
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    l0 = sim.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        sim.step(want_info=False)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = sim.launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    if world > 1:
+        t = torch.tensor([ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * cells * args.steps / (ms * 1e-3)
+
+    # ---- per-kernel CUDA-event timing of the same K steps (separate pass: events bracket every launch)
+    sim.profile(True)
+    for _ in range(args.steps):
+        sim.step(want_info=False)
+    prof = sim.profile_read()
+    sim.profile(False)
+    peak, peak_src = measured_peak_gbs()
+    roofline, kernels = None, {}
+    tot_ms = sum(v[0] for v in prof.values()) or 1.0
+    for name, (kms, cnt) in prof.items():
+        b = kernel_bytes(name, n, P)
+        kernels[name] = {"ms_per_launch": kms / cnt, "launches_per_step": cnt / args.steps, "share": kms / tot_ms,
+                         "GBps": (b / (kms / cnt * 1e-3) / 1e9) if b else None}
+    if prof:
+        top = max(prof, key=lambda k: prof[k][0])
+        b = kernel_bytes(top, n, P)
+        ach = b / (prof[top][0] / prof[top][1] * 1e-3) / 1e9
+        traffic = None
+        try:
+            with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+                traffic = json.load(f).get("%s@%d" % (top, n))
+        except Exception:
+            pass
+        roofline = {"bound": "hbm", "kernel": top, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                    "traffic": traffic, "peak_source": peak_src, "algorithmic_bytes_per_launch": b,
+                    "share_of_step": prof[top][0] / tot_ms}
+    step_gbs = STEP_BYTES_PER_CELL * cells * args.steps / (ms * 1e-3) / 1e9
+    step_roofline = {"achieved": step_gbs, "peak": peak, "unit": "GB/s", "frac": step_gbs / peak,
+                     "frac_of_8TBps": step_gbs / 8000.0, "bytes_per_cell_step": STEP_BYTES_PER_CELL}
+
+    # ---- end to end through the C ABI with HOST buffers: per step H2D of m, one RK45 step, D2H of m
+    host_in = torch.from_numpy(cfg["m0"].copy()).pin_memory()
+    host_out = torch.empty_like(host_in).pin_memory()
+    ke = max(1, min(args.e2e_steps, args.steps))
+    sim.set_m(host_in); sim.step(want_info=False); sim.get_m(host_out)       # warm the path
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(ke):
+        sim.set_m(host_in)                  # host -> device, normalise
+        sim.step(want_info=False)           # FSAL slope is stale after set_m: 7 evaluations
+        sim.get_m(host_out)                 # device -> host (synchronises)
+        host_in, host_out = host_out, host_in
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    nbytes = int(host_in.numel() * 4)
+    e2e = {"value": world * cells * ke / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+           "steps": ke, "ms_per_step": 1e3 * e2e_s / ke}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": "C4 film %dx%dx1, 4x4x2 nm, Permalloy, random m, B_ext 10 mT, fix_dt 1e-13 s" % (n, n),
+                           "cells": cells, "fft": list(sim.fft_size()), "parallelism": "replicas x%d" % world,
+                           "l2": "working set %.1f GB >> 126 MB L2 (no flush needed)" % (sim.stats()["peak_device_bytes"] / 1e9),
+                           "evals_per_step": 6},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+                "step_roofline": step_roofline, "kernels": kernels,
+                "peak_device_bytes": sim.stats()["peak_device_bytes"]}
+        line["cpu_baseline"] = None if (args.no_cpu_baseline or world > 1) else cpu_baseline(args)
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -148,6 +148,13 @@ int mm_get_fft_size(mm_sim* sim, int P[3]);
 /* Number of kernel launches the library has issued on this handle (for bench.py). */
 int mm_get_launch_count(mm_sim* sim, long* launches);
 
+/* Per-kernel timing with CUDA events on the handle's stream (used by bench.py for the roofline
+ * line). mm_profile(sim, 1) clears the counters and starts bracketing every launch with a pair of
+ * events; mm_profile(sim, 0) stops. mm_profile_read returns, for kernel class `kind`
+ * (0 <= kind < 12; MM_EINVAL beyond), its name, the summed duration in ms and the launch count. */
+int mm_profile(mm_sim* sim, int enable);
+int mm_profile_read(mm_sim* sim, int kind, const char** name, double* total_ms, long* launches);
+
 const char* mm_last_error(const mm_sim* sim);
 const char* mm_strerror(int code);
 const char* mm_version(void);

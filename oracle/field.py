@@ -31,25 +31,34 @@ def b_demag_direct(M, K, origin, pbc):
     return B
 
 
-def b_demag_fft(M, K, origin, pbc):
-    """The same sum through the convolution theorem (L123) with numpy's fp64 FFT.
+def padded_shape(shape, pbc):
+    """FFT lengths (z, y, x): open axes zero-padded to 2N (any length >= 2N-1 gives the identical
+    linear convolution, SURVEY.md 8(c) #4); periodic axes not padded (L509); 1 stays 1."""
+    n = tuple(shape)
+    return tuple(n[a] if pbc[2 - a] else (2 * n[a] if n[a] > 1 else 1) for a in range(3))
 
-    Open axes are zero-padded to 2N (any length >= 2N-1 gives the identical linear
-    convolution); periodic axes are not padded (L509).
-    """
-    _, nz, ny, nx = M.shape
-    n = (nz, ny, nx)
-    P = tuple(n[a] if pbc[2 - a] else (2 * n[a] if n[a] > 1 else 1) for a in range(3))
+
+def kernel_spectrum(K, origin, P):
+    """rfftn of every kernel component laid out on the padded, wrapped displacement grid."""
     Kp = {}
     for k, arr in K.items():
         buf = np.zeros(P)
         idx = []
         for a in range(3):
-            L = arr.shape[a]
-            d = np.arange(L) - origin[a]          # displacement of every stored entry
+            d = np.arange(arr.shape[a]) - origin[a]          # displacement of every stored entry
             idx.append(np.mod(d, P[a]))
         buf[np.ix_(*idx)] = arr
         Kp[k] = np.fft.rfftn(buf)
+    return Kp
+
+
+def b_demag_fft(M, K, origin, pbc, Kp=None):
+    """The same sum through the convolution theorem (L123) with numpy's fp64 FFT.
+    `Kp` may carry the kernel spectrum computed once by kernel_spectrum()."""
+    _, nz, ny, nx = M.shape
+    P = padded_shape((nz, ny, nx), pbc)
+    if Kp is None:
+        Kp = kernel_spectrum(K, origin, P)
     Mf = [np.fft.rfftn(M[j], s=P, axes=(0, 1, 2)) for j in range(3)]
     B = np.empty_like(M)
     for i in range(3):

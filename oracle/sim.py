@@ -52,6 +52,7 @@ class RefSim:
         self.n_eval = self.n_steps = self.n_rejected = 0
         self.demag_method = demag_method or ("direct" if self.ncells <= DIRECT_SUM_MAX_CELLS else "fft")
         self._K = None
+        self._Kp = None
         self.terms = MM_ALL
 
     # ---- setup
@@ -88,8 +89,11 @@ class RefSim:
     def b_demag(self, m):
         K, origin = self.kernel()
         M = (fld.MU0 * self.p.Msat)[self.regions][None] * m
-        fn = fld.b_demag_direct if self.demag_method == "direct" else fld.b_demag_fft
-        return fn(M, K, origin, self.pbc)
+        if self.demag_method == "direct":
+            return fld.b_demag_direct(M, K, origin, self.pbc)
+        if self._Kp is None:                      # kernel spectrum: computed once per box
+            self._Kp = fld.kernel_spectrum(K, origin, fld.padded_shape(self.shape, self.pbc))
+        return fld.b_demag_fft(M, K, origin, self.pbc, self._Kp)
 
     def b_eff(self, term_mask=MM_ALL, m=None):
         m = self.m if m is None else m

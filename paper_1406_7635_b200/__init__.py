@@ -73,6 +73,9 @@ _SIGNATURES = {
                                C.POINTER(C.c_size_t)]),
     "mm_get_fft_size": (C.c_int, [C.c_void_p, C.POINTER(C.c_int)]),
     "mm_get_launch_count": (C.c_int, [C.c_void_p, C.POINTER(C.c_long)]),
+    "mm_profile": (C.c_int, [C.c_void_p, C.c_int]),
+    "mm_profile_read": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_double),
+                                  C.POINTER(C.c_long)]),
     "mm_last_error": (C.c_char_p, [C.c_void_p]),
     "mm_strerror": (C.c_char_p, [C.c_int]),
     "mm_version": (C.c_char_p, []),
@@ -263,6 +266,20 @@ class Sim:
         v = (C.c_int * 3)()
         _check(lib().mm_get_fft_size(self._h, v), self._h)
         return tuple(v[:])
+
+    def profile(self, enable):
+        _check(lib().mm_profile(self._h, 1 if enable else 0), self._h)
+
+    def profile_read(self):
+        """{kernel class: (total ms, launches)} accumulated since profile(True)."""
+        out = {}
+        for kind in range(64):
+            name, ms, n = C.c_char_p(), C.c_double(), C.c_long()
+            if lib().mm_profile_read(self._h, kind, C.byref(name), C.byref(ms), C.byref(n)) != MM_OK:
+                break
+            if n.value:
+                out[name.value.decode()] = (ms.value, n.value)
+        return out
 
     def launch_count(self):
         v = C.c_long()

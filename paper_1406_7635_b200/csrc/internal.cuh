@@ -9,6 +9,11 @@
 void* mm_default_alloc(size_t bytes, void*);
 void mm_default_free(void* p, void*);
 
+// kernel classes for launch counting and per-kernel CUDA-event timing (mm_profile)
+enum KernelKind { KK_XFWD = 0, KK_YFWD, KK_YINV, KK_LAST_XY, KK_LAST_Z, KK_LAST_3D, KK_XINV, KK_LOCAL, KK_STAGE,
+                  KK_ERROR, KK_CTRL, KK_OTHER, KK_COUNT };
+struct ProfEntry { int kind; cudaEvent_t a, b; };
+
 struct mm_sim {
   Geometry g;
   AxisPlan px, py, pz;
@@ -36,6 +41,12 @@ struct mm_sim {
   unsigned terms = MM_ALL;
   int nregions = 1;
   long launches = 0;
+  long extra_evals = 0;
+  bool prof_on = false;
+  std::vector<ProfEntry> prof;
+  std::vector<cudaEvent_t> ev_pool;
+  double prof_ms[KK_COUNT] = {};
+  long prof_n[KK_COUNT] = {};
   std::string err;
   // launch configuration
   int xL = 1, yC = 1, lastC[3] = {1, 1, 1};
@@ -58,3 +69,20 @@ int mm_build_kernel_spectrum(mm_sim* s);   // setup.cu
   } while (0)
 
 inline unsigned blocks_for(long long n, int threads) { return (unsigned)((n + threads - 1) / threads); }
+
+// RAII bracket around one kernel launch: counts it and, while profiling, records a CUDA event
+// on the launching stream before and after it.
+struct Launch {
+  mm_sim* s; int kind; cudaEvent_t a = nullptr, b = nullptr;
+  static cudaEvent_t get(mm_sim* s) {
+    if (!s->ev_pool.empty()) { cudaEvent_t e = s->ev_pool.back(); s->ev_pool.pop_back(); return e; }
+    cudaEvent_t e; cudaEventCreate(&e); return e;
+  }
+  Launch(mm_sim* s_, int kind_) : s(s_), kind(kind_) {
+    s->launches++;
+    if (s->prof_on) { a = get(s); b = get(s); cudaEventRecord(a, s->stream); }
+  }
+  ~Launch() {
+    if (a) { cudaEventRecord(b, s->stream); s->prof.push_back({kind, a, b}); }
+  }
+};

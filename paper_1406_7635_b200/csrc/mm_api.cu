@@ -136,7 +136,8 @@ int configure_launches(mm_sim* s) {
   for (int mode = 0; mode < 3; ++mode) {
     s->lastC[mode] = pick(Pl, ncs[mode] + 1, 4096, 32);
     s->lastSmem[mode] = (size_t)(ncs[mode] + 1) * s->lastC[mode] * Pl * sizeof(float2);
-    if (s->lastSmem[mode] > kSmemMax) return mm_fail(s, MM_EINVAL, "FFT length too large for shared memory");
+    const bool used = s->last_along_z ? (mode == 2) : (mode != 2);
+    if (used && s->lastSmem[mode] > kSmemMax) return mm_fail(s, MM_EINVAL, "FFT length too large for shared memory");
   }
   if (s->xSmem > kSmemMax || s->ySmem > kSmemMax) return mm_fail(s, MM_EINVAL, "FFT length too large for shared memory");
   return MM_OK;
@@ -148,32 +149,28 @@ void launch_demag(mm_sim* s, int src_role) {
   const int rows = g.Ny * g.Nz, pairs = (rows + 1) / 2;
   const int T = 256;
   dim3 gx((pairs + s->xL - 1) / s->xL, 3);
-  k_x_fwd<<<gx, T, s->xSmem, s->stream>>>(s->conv, src_role, s->xL);
-  s->launches++;
+  { Launch l(s, KK_XFWD); k_x_fwd<<<gx, T, s->xSmem, s->stream>>>(s->conv, src_role, s->xL); }
   if (s->last_along_z) {
     dim3 gy((g.Cx + s->yC - 1) / s->yC, g.Nz, 3);
-    if (g.Py > 1) { k_y_axis<<<gy, T, s->ySmem, s->stream>>>(s->conv, 0, s->yC); s->launches++; }
+    if (g.Py > 1) { Launch l(s, KK_YFWD); k_y_axis<<<gy, T, s->ySmem, s->stream>>>(s->conv, 0, s->yC); }
     dim3 gl((g.Cx + s->lastC[2] - 1) / s->lastC[2], g.Py);
-    k_last_fused<3><<<gl, T, s->lastSmem[2], s->stream>>>(s->conv, 2, s->lastC[2]);
-    s->launches++;
-    if (g.Py > 1) { k_y_axis<<<gy, T, s->ySmem, s->stream>>>(s->conv, 1, s->yC); s->launches++; }
+    { Launch l(s, KK_LAST_3D); k_last_fused<3><<<gl, T, s->lastSmem[2], s->stream>>>(s->conv, 2, s->lastC[2]); }
+    if (g.Py > 1) { Launch l(s, KK_YINV); k_y_axis<<<gy, T, s->ySmem, s->stream>>>(s->conv, 1, s->yC); }
   } else {
     dim3 g0((g.Cx + s->lastC[0] - 1) / s->lastC[0]);
-    k_last_fused<2><<<g0, T, s->lastSmem[0], s->stream>>>(s->conv, 0, s->lastC[0]);
+    { Launch l(s, KK_LAST_XY); k_last_fused<2><<<g0, T, s->lastSmem[0], s->stream>>>(s->conv, 0, s->lastC[0]); }
     dim3 g1((g.Cx + s->lastC[1] - 1) / s->lastC[1]);
-    k_last_fused<1><<<g1, T, s->lastSmem[1], s->stream>>>(s->conv, 1, s->lastC[1]);
-    s->launches += 2;
+    { Launch l(s, KK_LAST_Z); k_last_fused<1><<<g1, T, s->lastSmem[1], s->stream>>>(s->conv, 1, s->lastC[1]); }
   }
-  k_x_inv<<<gx, T, s->xSmem, s->stream>>>(s->conv, R_B, s->xL);
-  s->launches++;
+  { Launch l(s, KK_XINV); k_x_inv<<<gx, T, s->xSmem, s->stream>>>(s->conv, R_B, s->xL); }
 }
 
 // field (out_torque = 0) or torque over gamma (out_torque = 1) of role `src` into role `dst`
 void launch_eval(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_torque) {
   if (mask & MM_DEMAG) launch_demag(s, src_role);
+  Launch l(s, KK_LOCAL);
   k_local<<<blocks_for(s->g.N, 256), 256, 0, s->stream>>>(s->g, s->regions, s->luts, s->dstate, src_role, R_B, dst_role,
                                                          mask, out_torque);
-  s->launches++;
 }
 
 void enqueue_step(mm_sim* s) {
@@ -181,23 +178,21 @@ void enqueue_step(mm_sim* s) {
   if (!s->have_k1) {
     launch_eval(s, R_M, R_K0, s->terms, 1);
     s->have_k1 = true;
+    s->extra_evals++;
   }
-  k_ctrl_begin<<<1, 1, 0, s->stream>>>(s->dstate);
-  s->launches++;
+  { Launch l(s, KK_CTRL); k_ctrl_begin<<<1, 1, 0, s->stream>>>(s->dstate); }
   for (int i = 1; i < 7; ++i) {
     StageCoef sc;
     sc.n = i;
     for (int j = 0; j < 6; ++j) sc.a[j] = (float)DP_A[i][j];
     const int yrole = (i == 6) ? R_MNEW : R_Y;
-    k_stage<<<blocks_for(N, 256), 256, 0, s->stream>>>(N, s->dstate, sc, yrole);
-    s->launches++;
+    { Launch l(s, KK_STAGE); k_stage<<<blocks_for(N, 256), 256, 0, s->stream>>>(N, s->dstate, sc, yrole); }
     launch_eval(s, yrole, R_K0 + i, s->terms, 1);
   }
   ErrCoef ec;
   for (int j = 0; j < 7; ++j) ec.e[j] = (float)DP_E[j];
-  k_error<<<148 * 8, 256, 0, s->stream>>>(N, s->dstate, ec);
-  k_ctrl_end<<<1, 1, 0, s->stream>>>(s->dstate);
-  s->launches += 2;
+  { Launch l(s, KK_ERROR); k_error<<<148 * 8, 256, 0, s->stream>>>(N, s->dstate, ec); }
+  { Launch l(s, KK_CTRL); k_ctrl_end<<<1, 1, 0, s->stream>>>(s->dstate); }
 }
 
 int check_ready(mm_sim* s) {
@@ -330,6 +325,8 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
 int mm_destroy(mm_sim* s) {
   if (!s) return MM_OK;
   cudaStreamSynchronize(s->stream);
+  for (auto& e : s->prof) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+  for (auto& e : s->ev_pool) cudaEventDestroy(e);
   while (!s->owned.empty()) mm_dev_free(s, s->owned.back().first);
   delete s;
   return MM_OK;
@@ -451,8 +448,7 @@ int mm_set_m(mm_sim* s, const float* m) {
   int rc;
   if ((rc = pull_state(s))) return rc;
   if ((rc = copy_in(s, s->hst.ptr[R_M], m, sizeof(float) * 3 * (size_t)s->g.N))) return rc;
-  k_normalise<<<blocks_for(s->g.N, 256), 256, 0, s->stream>>>(s->g.N, s->hst.ptr[R_M], s->regions, s->luts);
-  s->launches++;
+  { Launch l(s, KK_OTHER); k_normalise<<<blocks_for(s->g.N, 256), 256, 0, s->stream>>>(s->g.N, s->hst.ptr[R_M], s->regions, s->luts); }
   CUDA_TRY(s, cudaGetLastError());
   s->hst.status = MM_OK;
   s->hst.skip = 0;
@@ -498,7 +494,7 @@ int mm_step_rk45(mm_sim* s, mm_step_info* info) {
   if ((rc = pull_state(s))) return rc;
   const DevState& h = s->hst;
   info->t = h.t; info->dt_taken = h.h; info->dt_next = h.fix_dt > 0 ? h.fix_dt : h.dt; info->err = h.last_err;
-  info->accepted = h.last_accepted; info->n_eval = (long)h.evals;
+  info->accepted = h.last_accepted; info->n_eval = (long)h.evals + s->extra_evals;
   return status_to_error(s);
 }
 
@@ -563,8 +559,7 @@ int mm_get_avg_m(mm_sim* s, double avg[3]) {
   int rc;
   if ((rc = pull_state(s))) return rc;
   CUDA_TRY(s, cudaMemsetAsync(s->scratch3, 0, 3 * sizeof(double), s->stream));
-  k_sum3<<<148 * 4, 256, 0, s->stream>>>(s->g.N, s->hst.ptr[R_M], s->scratch3);
-  s->launches++;
+  { Launch l(s, KK_OTHER); k_sum3<<<148 * 4, 256, 0, s->stream>>>(s->g.N, s->hst.ptr[R_M], s->scratch3); }
   CUDA_TRY(s, cudaGetLastError());
   if ((rc = copy_out(s, avg, s->scratch3, 3 * sizeof(double)))) return rc;
   for (int c = 0; c < 3; ++c) avg[c] /= (double)s->g.N;
@@ -577,7 +572,7 @@ int mm_get_stats(mm_sim* s, long* steps, long* rejected, long* evals, size_t* pe
   if ((rc = pull_state(s))) return rc;
   if (steps) *steps = (long)s->hst.steps;
   if (rejected) *rejected = (long)s->hst.rejected;
-  if (evals) *evals = (long)s->hst.evals;
+  if (evals) *evals = (long)s->hst.evals + s->extra_evals;
   if (peak) *peak = s->peak_bytes;
   return MM_OK;
 }
@@ -591,6 +586,36 @@ int mm_get_fft_size(mm_sim* s, int P[3]) {
 int mm_get_launch_count(mm_sim* s, long* launches) {
   if (!s || !launches) return MM_EINVAL;
   *launches = s->launches;
+  return MM_OK;
+}
+
+int mm_profile(mm_sim* s, int enable) {
+  if (!s) return MM_EINVAL;
+  CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+  for (auto& e : s->prof) { s->ev_pool.push_back(e.a); s->ev_pool.push_back(e.b); }
+  s->prof.clear();
+  for (int k = 0; k < KK_COUNT; ++k) { s->prof_ms[k] = 0; s->prof_n[k] = 0; }
+  s->prof_on = enable != 0;
+  return MM_OK;
+}
+
+int mm_profile_read(mm_sim* s, int kind, const char** name, double* total_ms, long* launches) {
+  static const char* names[KK_COUNT] = {"x_fwd", "y_fwd", "y_inv", "last_xy", "last_z", "last_3d", "x_inv", "local",
+                                        "rk_stage", "rk_error", "rk_ctrl", "other"};
+  if (!s || kind < 0 || kind >= KK_COUNT) return MM_EINVAL;
+  if (!s->prof.empty()) {
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    for (auto& e : s->prof) {
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, e.a, e.b);
+      s->prof_ms[e.kind] += ms; s->prof_n[e.kind] += 1;
+      s->ev_pool.push_back(e.a); s->ev_pool.push_back(e.b);
+    }
+    s->prof.clear();
+  }
+  if (name) *name = names[kind];
+  if (total_ms) *total_ms = s->prof_ms[kind];
+  if (launches) *launches = s->prof_n[kind];
   return MM_OK;
 }
 
