@@ -104,6 +104,11 @@ int mm_set_params(mm_sim* sim, const mm_params* params);
 /* Which B_eff terms drive the dynamics (default MM_ALL). */
 int mm_set_terms(mm_sim* sim, unsigned term_mask);
 
+/* Implementation switches. MM_OPT_GENERIC_FFT = 1 forces the generic any-size convolution kernels
+ * even where a specialised path exists (used by the tests to check the two against each other). */
+enum { MM_OPT_GENERIC_FFT = 1 };
+int mm_set_option(mm_sim* sim, int option, int value);
+
 /* Solver settings (L372-L374). max_err: MaxErr eps0 (default 1e-5); headroom (default 0.8);
  * fix_dt > 0 selects a fixed step (every step accepted), 0 = adaptive; dt_init: first trial step
  * (default 1e-14 s); dt_min/dt_max clip the controller (defaults 1e-18, 1e-9).
@@ -151,7 +156,7 @@ int mm_get_launch_count(mm_sim* sim, long* launches);
 /* Per-kernel timing with CUDA events on the handle's stream (used by bench.py for the roofline
  * line). mm_profile(sim, 1) clears the counters and starts bracketing every launch with a pair of
  * events; mm_profile(sim, 0) stops. mm_profile_read returns, for kernel class `kind`
- * (0 <= kind < 12; MM_EINVAL beyond), its name, the summed duration in ms and the launch count. */
+ * (0 <= kind < 15; MM_EINVAL beyond), its name, the summed duration in ms and the launch count. */
 int mm_profile(mm_sim* sim, int enable);
 int mm_profile_read(mm_sim* sim, int kind, const char** name, double* total_ms, long* launches);
 

@@ -13,6 +13,7 @@ import numpy as np
 MM_OK, MM_EINVAL, MM_ENOMEM, MM_ECUDA, MM_ESTATE, MM_ENAN, MM_EDT = 0, -1, -2, -3, -4, -5, -6
 MM_DEMAG, MM_EXCH, MM_ANIS, MM_ZEEMAN, MM_ALL = 1, 2, 4, 8, 15
 MM_MAX_REGIONS = 256
+MM_OPT_GENERIC_FFT = 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmm_b200.so")
@@ -58,6 +59,7 @@ _SIGNATURES = {
     "mm_set_regions": (C.c_int, [C.c_void_p, C.c_void_p]),
     "mm_set_params": (C.c_int, [C.c_void_p, C.POINTER(mm_params)]),
     "mm_set_terms": (C.c_int, [C.c_void_p, C.c_uint]),
+    "mm_set_option": (C.c_int, [C.c_void_p, C.c_int, C.c_int]),
     "mm_set_solver": (C.c_int, [C.c_void_p] + [C.c_double] * 6),
     "mm_set_m": (C.c_int, [C.c_void_p, C.c_void_p]),
     "mm_get_m": (C.c_int, [C.c_void_p, C.c_void_p]),
@@ -199,6 +201,9 @@ class Sim:
 
     def set_terms(self, mask):
         _check(lib().mm_set_terms(self._h, int(mask)), self._h)
+
+    def set_option(self, option, value):
+        _check(lib().mm_set_option(self._h, int(option), int(value)), self._h)
 
     def set_solver(self, max_err=0.0, headroom=0.0, fix_dt=0.0, dt_init=0.0, dt_min=0.0, dt_max=0.0):
         _check(lib().mm_set_solver(self._h, max_err, headroom, fix_dt, dt_init, dt_min, dt_max), self._h)

@@ -17,3 +17,20 @@ struct ConvArgs {
   const Luts* luts;
   DevState* st;
 };
+
+// argument block of the fast 2D path (fast2d.cuh)
+struct Fast2DArgs {
+  int Nx, Ny, Cx;        // Cx = Nx + 1 stored kx (0 .. Nx)
+  long long ncell;       // Nx * Ny
+  float2* spec;          // [3][Cx][Ny]
+  long long cstride;     // Cx * Ny
+  const float* Kt;       // [4][Cx][Ny + 1]: per (component, kx) the even-ky entries ky = 0,2,..,Ny
+                         // (Ny/2 + 1) followed by the odd ones ky = 1,3,..,Ny-1; comps xx, yy, zz, xy
+  long long kstride;     // Cx * (Ny + 1)
+  const float2 *twx, *twx_r;   // plan tables, length Nx: forward plan / reversed plan
+  const float2 *twy, *twy_r;   // same for length Ny
+  const float2 *twox, *twoy;   // exp(-2 pi i n / (2Nx)), n < Nx ; same for y
+  const uint8_t* regions;
+  const Luts* luts;
+  DevState* st;
+};

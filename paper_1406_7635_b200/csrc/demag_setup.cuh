@@ -226,4 +226,15 @@ __global__ void k_pack_spectrum(TensorGrid tg, const double2* __restrict__ full,
   if (im > 1e-9) atomicMax((unsigned long long*)max_imag, (unsigned long long)__double_as_longlong(im));
 }
 
+// 2D fast-path layout (fast2d.cuh): out[kx][pos], pos = even ky (0,2,..,Ny) then odd ky (1,3,..,Ny-1)
+__global__ void k_pack_spectrum_2dfast(TensorGrid tg, const double2* __restrict__ full, float* __restrict__ out, int Cx,
+                                       int Ny, double scale) {
+  const long long total = (long long)Cx * (Ny + 1);
+  const long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (id >= total) return;
+  const int kx = (int)(id / (Ny + 1)), pos = (int)(id % (Ny + 1));
+  const int ky = pos <= Ny / 2 ? 2 * pos : 2 * (pos - Ny / 2 - 1) + 1;
+  out[id] = (float)(full[(size_t)ky * tg.P[0] + kx].x * scale);
+}
+
 }  // namespace setup

@@ -1,0 +1,160 @@
+// fast2d.cu - host side of the fast 2D demag path: plan tables, kernel-table layout, launches.
+#include <cmath>
+#include <vector>
+#include "internal.cuh"
+#include "fast2d.cuh"
+
+namespace {
+
+template <int N> struct PlanFor;
+template <> struct PlanFor<4096> { using P = rf::Plan<4096, 256, 16, 16, 16>; static constexpr int NTX = 512, RG = 8, NTY = 256; };
+template <> struct PlanFor<2048> { using P = rf::Plan<2048, 128, 16, 8, 16>; static constexpr int NTX = 256, RG = 8, NTY = 256; };
+template <> struct PlanFor<1024> { using P = rf::Plan<1024, 64, 16, 4, 16>; static constexpr int NTX = 256, RG = 8, NTY = 256; };
+template <> struct PlanFor<512> { using P = rf::Plan<512, 32, 16, 2, 16>; static constexpr int NTX = 256, RG = 16, NTY = 256; };
+template <> struct PlanFor<256> { using P = rf::Plan<256, 16, 16, 16, 1>; static constexpr int NTX = 256, RG = 32, NTY = 256; };
+
+// forward twiddles of a plan, laid out as fft_reg.cuh reads them
+template <class P>
+std::vector<float2> plan_table() {
+  std::vector<float2> tw(P::TW);
+  const int N = P::N;
+  auto put = [&](size_t i, double turns) {
+    const double ang = -2.0 * M_PI * turns;
+    tw[i] = make_float2((float)cos(ang), (float)sin(ang));
+  };
+  for (int s = 1; s < P::RA; ++s)
+    for (int bf = 0; bf < N / P::RA; ++bf) put((size_t)(s - 1) * (N / P::RA) + bf, (double)((long long)s * bf % N) / N);
+  if (P::NPASS == 3)
+    for (int s = 1; s < P::RB; ++s)
+      for (int bf = 0; bf < N / P::RB; ++bf)
+        put((size_t)P::TW1 + (size_t)(s - 1) * (N / P::RB) + bf, (double)((long long)s * P::RA * (bf % P::M2) % N) / N);
+  return tw;
+}
+
+int upload(mm_sim* s, const std::vector<float2>& h, float2** out) {
+  *out = (float2*)mm_dev_alloc(s, sizeof(float2) * h.size());
+  if (!*out) return mm_fail(s, MM_ENOMEM, "fast path twiddles");
+  CUDA_TRY(s, cudaMemcpy(*out, h.data(), sizeof(float2) * h.size(), cudaMemcpyHostToDevice));
+  return MM_OK;
+}
+
+template <int N>
+int make_axis_tables(mm_sim* s, float2** fwd, float2** rev, float2** half) {
+  using P = typename PlanFor<N>::P;
+  int rc;
+  if ((rc = upload(s, plan_table<P>(), fwd))) return rc;
+  if ((rc = upload(s, plan_table<typename P::Reversed>(), rev))) return rc;
+  std::vector<float2> w(N);
+  for (int n = 0; n < N; ++n) {
+    const double ang = -M_PI * (double)n / (double)N;      // exp(-2 pi i n / (2N))
+    w[n] = make_float2((float)cos(ang), (float)sin(ang));
+  }
+  return upload(s, w, half);
+}
+
+int axis_tables(mm_sim* s, int N, float2** fwd, float2** rev, float2** half) {
+  switch (N) {
+    case 4096: return make_axis_tables<4096>(s, fwd, rev, half);
+    case 2048: return make_axis_tables<2048>(s, fwd, rev, half);
+    case 1024: return make_axis_tables<1024>(s, fwd, rev, half);
+    case 512: return make_axis_tables<512>(s, fwd, rev, half);
+    case 256: return make_axis_tables<256>(s, fwd, rev, half);
+  }
+  return mm_fail(s, MM_EINVAL, "fast 2D path: unsupported length");
+}
+
+template <int N>
+int x_attrs(mm_sim* s) {
+  using F = PlanFor<N>;
+  const int bytes = (int)k2_x_smem<typename F::P, F::NTX, F::RG>();
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd<typename F::P, F::NTX, F::RG>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv<typename F::P, F::NTX, F::RG>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  return MM_OK;
+}
+template <int N>
+int y_attrs(mm_sim* s) {
+  using F = PlanFor<N>;
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_ycol<typename F::P, F::NTY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)k2_y_smem<typename F::P, F::NTY>()));
+  return MM_OK;
+}
+
+template <int N>
+void launch_x(mm_sim* s, bool inverse, int role) {
+  using F = PlanFor<N>;
+  const dim3 grid(s->g.Ny / F::RG, 3);
+  const size_t bytes = k2_x_smem<typename F::P, F::NTX, F::RG>();
+  if (!inverse) k2_xfwd<typename F::P, F::NTX, F::RG><<<grid, F::NTX, bytes, s->stream>>>(s->f2, role);
+  else k2_xinv<typename F::P, F::NTX, F::RG><<<grid, F::NTX, bytes, s->stream>>>(s->f2, role);
+}
+template <int N>
+void launch_y(mm_sim* s) {
+  using F = PlanFor<N>;
+  constexpr int G = F::NTY / F::P::T;
+  k2_ycol<typename F::P, F::NTY><<<(s->f2.Cx + G - 1) / G, F::NTY, k2_y_smem<typename F::P, F::NTY>(), s->stream>>>(s->f2);
+}
+
+int rows_per_cta(int N) {
+  switch (N) {
+    case 4096: return PlanFor<4096>::RG;
+    case 2048: return PlanFor<2048>::RG;
+    case 1024: return PlanFor<1024>::RG;
+    case 512: return PlanFor<512>::RG;
+    case 256: return PlanFor<256>::RG;
+  }
+  return 0;
+}
+
+}  // namespace
+
+#define F2_SWITCH(N, CALL)                    \
+  switch (N) {                                \
+    case 4096: { CALL(4096); break; }         \
+    case 2048: { CALL(2048); break; }         \
+    case 1024: { CALL(1024); break; }         \
+    case 512: { CALL(512); break; }           \
+    case 256: { CALL(256); break; }           \
+  }
+
+bool mm_fast2d_supported(int Nx, int Ny, int Nz, const int* pbc) {
+  if (Nz != 1 || pbc[0] || pbc[1] || pbc[2]) return false;
+  const int rg = rows_per_cta(Nx);
+  return rg > 0 && rows_per_cta(Ny) > 0 && Ny % rg == 0;
+}
+
+int mm_fast2d_init(mm_sim* s) {
+  const Geometry& g = s->g;
+  Fast2DArgs& a = s->f2;
+  a.Nx = g.Nx; a.Ny = g.Ny; a.Cx = g.Nx + 1;
+  a.ncell = g.N;
+  a.spec = s->spec;
+  a.cstride = (long long)a.Cx * g.Ny;
+  a.Kt = s->Kt;
+  a.kstride = (long long)a.Cx * (g.Ny + 1);
+  a.regions = s->regions; a.luts = s->luts; a.st = s->dstate;
+  float2 *fx, *rx, *hx, *fy, *ry, *hy;
+  int rc;
+  if ((rc = axis_tables(s, g.Nx, &fx, &rx, &hx))) return rc;
+  if ((rc = axis_tables(s, g.Ny, &fy, &ry, &hy))) return rc;
+  a.twx = fx; a.twx_r = rx; a.twox = hx; a.twy = fy; a.twy_r = ry; a.twoy = hy;
+#define XA(N) if ((rc = x_attrs<N>(s))) return rc
+#define YA(N) if ((rc = y_attrs<N>(s))) return rc
+  F2_SWITCH(g.Nx, XA)
+  F2_SWITCH(g.Ny, YA)
+#undef XA
+#undef YA
+  return MM_OK;
+}
+
+// B_demag of the field in role `src` -> role R_B
+void mm_fast2d_demag(mm_sim* s, int src_role) {
+#define XF(N) launch_x<N>(s, false, src_role)
+#define XI(N) launch_x<N>(s, true, R_B)
+#define YC(N) launch_y<N>(s)
+  { Launch l(s, KK_F2_XFWD); F2_SWITCH(s->g.Nx, XF) }
+  { Launch l(s, KK_F2_YCOL); F2_SWITCH(s->g.Ny, YC) }
+  { Launch l(s, KK_F2_XINV); F2_SWITCH(s->g.Nx, XI) }
+#undef XF
+#undef XI
+#undef YC
+}

@@ -1,0 +1,215 @@
+// fft_reg.cuh - register-resident power-of-two FFT engine of the fast demag path (sm_100a).
+//
+// One length-N complex transform is computed by a group of T threads, E = N/T points per thread
+// held in registers, in 2 or 3 passes of radix RA, RB[, RC] (N = RA*RB*RC). Between two passes the
+// points are exchanged through a (padded, bank-conflict-free) shared-memory buffer; the first
+// pass reads and the last pass leaves the data in the striped "natural" layout
+//     point index = bf + (N/R) * s,   bf = t + T*b,   register v[b*R + s]
+// (R = RA on input, R = last radix on output), so that global loads/stores of consecutive threads
+// are contiguous and no digit-reversal pass is ever needed (PAPER.md L123 only asks for "the
+// well-known convolution theorem"; how the transforms are organised is ours).
+//
+// Decomposition (decimation in frequency): n = n1*M1 + n2*M2 + n3, k = k1 + RA*k2 + RA*RB*k3,
+// M1 = N/RA, M2 = M1/RB. Pass i transforms digit n_i -> k_i and multiplies by
+// w_N^{k_i * (RA..R_{i-1}) * rest_i}, rest_i = the not yet transformed low digits.
+#pragma once
+#include "common.cuh"
+
+namespace rf {
+
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+
+// a * w (DIR < 0) or a * conj(w) (DIR > 0): tables hold the forward twiddles exp(-i phi)
+template <int DIR>
+__device__ __forceinline__ float2 cmul_tw(float2 a, float2 w) {
+  if (DIR < 0) return make_float2(a.x * w.x - a.y * w.y, a.x * w.y + a.y * w.x);
+  return make_float2(a.x * w.x + a.y * w.y, a.y * w.x - a.x * w.y);
+}
+
+// multiply by exp(DIR * i * pi/2)
+template <int DIR>
+__device__ __forceinline__ float2 rot90(float2 a) {
+  return DIR < 0 ? make_float2(a.y, -a.x) : make_float2(-a.y, a.x);
+}
+// multiply by exp(DIR * i * pi/4)
+template <int DIR>
+__device__ __forceinline__ float2 rot45(float2 a) {
+  const float h = 0.70710678118654752f;
+  return DIR < 0 ? make_float2(h * (a.x + a.y), h * (a.y - a.x)) : make_float2(h * (a.x - a.y), h * (a.x + a.y));
+}
+// multiply by exp(DIR * i * 3 pi/4)
+template <int DIR>
+__device__ __forceinline__ float2 rot135(float2 a) {
+  const float h = 0.70710678118654752f;
+  return DIR < 0 ? make_float2(h * (a.y - a.x), -h * (a.x + a.y)) : make_float2(-h * (a.x + a.y), h * (a.x - a.y));
+}
+// multiply by exp(DIR * i * phi) with cos(phi) = C, sin(phi) = S given as literals
+template <int DIR>
+__device__ __forceinline__ float2 rotcs(float2 a, const float C, const float S) {
+  return DIR < 0 ? make_float2(a.x * C + a.y * S, a.y * C - a.x * S) : make_float2(a.x * C - a.y * S, a.y * C + a.x * S);
+}
+
+template <int R, int DIR>
+struct Bfly;
+
+template <int DIR>
+struct Bfly<2, DIR> {
+  static __device__ __forceinline__ void run(float2* v) {
+    float2 a = v[0], b = v[1];
+    v[0] = cadd(a, b);
+    v[1] = csub(a, b);
+  }
+};
+
+template <int DIR>
+struct Bfly<4, DIR> {
+  static __device__ __forceinline__ void run(float2& v0, float2& v1, float2& v2, float2& v3) {
+    float2 t0 = cadd(v0, v2), t1 = csub(v0, v2), t2 = cadd(v1, v3), t3 = rot90<DIR>(csub(v1, v3));
+    v0 = cadd(t0, t2);
+    v2 = csub(t0, t2);
+    v1 = cadd(t1, t3);
+    v3 = csub(t1, t3);
+  }
+  static __device__ __forceinline__ void run(float2* v) { run(v[0], v[1], v[2], v[3]); }
+};
+
+// 8 = 2 x 4: n = 4a + b, k = c + 2d
+template <int DIR>
+struct Bfly<8, DIR> {
+  static __device__ __forceinline__ void run(float2* v) {
+    float2 A0[4], A1[4];
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+      A0[b] = cadd(v[b], v[b + 4]);
+      A1[b] = csub(v[b], v[b + 4]);
+    }
+    A1[1] = rot45<DIR>(A1[1]);
+    A1[2] = rot90<DIR>(A1[2]);
+    A1[3] = rot135<DIR>(A1[3]);
+    Bfly<4, DIR>::run(A0[0], A0[1], A0[2], A0[3]);
+    Bfly<4, DIR>::run(A1[0], A1[1], A1[2], A1[3]);
+#pragma unroll
+    for (int d = 0; d < 4; ++d) {
+      v[2 * d] = A0[d];
+      v[2 * d + 1] = A1[d];
+    }
+  }
+};
+
+// 16 = 4 x 4: n = 4a + b, k = c + 4d; twiddles W16^{bc}
+template <int DIR>
+struct Bfly<16, DIR> {
+  static __device__ __forceinline__ void run(float2* v) {
+    const float C1 = 0.92387953251128674f, S1 = 0.38268343236508977f;  // cos, sin of pi/8
+#pragma unroll
+    for (int b = 0; b < 4; ++b) Bfly<4, DIR>::run(v[b], v[b + 4], v[b + 8], v[b + 12]);
+    // after the radix-4 over a, element (b, c) sits in v[b + 4c]
+    v[1 + 4] = rotcs<DIR>(v[1 + 4], C1, S1);     // W^1
+    v[1 + 8] = rot45<DIR>(v[1 + 8]);             // W^2
+    v[1 + 12] = rotcs<DIR>(v[1 + 12], S1, C1);   // W^3
+    v[2 + 4] = rot45<DIR>(v[2 + 4]);             // W^2
+    v[2 + 8] = rot90<DIR>(v[2 + 8]);             // W^4
+    v[2 + 12] = rot135<DIR>(v[2 + 12]);          // W^6
+    v[3 + 4] = rotcs<DIR>(v[3 + 4], S1, C1);     // W^3
+    v[3 + 8] = rot135<DIR>(v[3 + 8]);            // W^6
+    v[3 + 12] = rotcs<DIR>(v[3 + 12], -C1, -S1); // W^9
+    // radix-4 over b for each c: (v[4c], v[4c+1], v[4c+2], v[4c+3]) -> X[c + 4d] in slot 4c + d
+#pragma unroll
+    for (int c = 0; c < 4; ++c) Bfly<4, DIR>::run(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
+    // transpose slots (4c + d) -> (c + 4d)
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+#pragma unroll
+      for (int d = c + 1; d < 4; ++d) {
+        float2 tmp = v[4 * c + d];
+        v[4 * c + d] = v[4 * d + c];
+        v[4 * d + c] = tmp;
+      }
+  }
+};
+
+template <int N_, int T_, int RA_, int RB_, int RC_>
+struct Plan {
+  static constexpr int N = N_, T = T_, E = N_ / T_, RA = RA_, RB = RB_, RC = RC_;
+  static constexpr int NPASS = RC_ > 1 ? 3 : 2;
+  static constexpr int RLAST = RC_ > 1 ? RC_ : RB_;
+  static constexpr int M1 = N_ / RA_, M2 = M1 / RB_;
+  static constexpr int XB = N_ + N_ / 16;                       // padded exchange buffer (float2)
+  static constexpr int TW1 = (RA_ - 1) * (N_ / RA_);            // twiddle entries after pass 1
+  static constexpr int TW2 = RC_ > 1 ? (RB_ - 1) * (N_ / RB_) : 0;
+  static constexpr int TW = TW1 + TW2;
+  static_assert(RA_ * RB_ * RC_ == N_, "radices must multiply to N");
+  static_assert(E % RA_ == 0 && E % RB_ == 0 && E % RC_ == 0, "every radix must divide the points per thread");
+  typedef Plan<N_, T_, (RC_ > 1 ? RC_ : RB_), (RC_ > 1 ? RB_ : RA_), (RC_ > 1 ? RA_ : 1)> Reversed;
+};
+
+__device__ __forceinline__ int xpad(int a) { return a + (a >> 4); }
+
+// synchronise the T threads of FFT group `gid` of a CTA with NT threads
+template <int T, int NT>
+__device__ __forceinline__ void group_sync(int gid) {
+  if (T == NT) __syncthreads();
+  else if (T >= 32) asm volatile("bar.sync %0, %1;" ::"r"(gid + 1), "r"(T) : "memory");
+  else __syncwarp();
+}
+
+// point index of register slot e in the striped layout with radix R
+template <class P, int R>
+__device__ __forceinline__ int slot_index(int t, int e) {
+  return t + P::T * (e / R) + (P::N / R) * (e % R);
+}
+
+template <class P, int R, int DIR>
+__device__ __forceinline__ void pass_butterflies(float2* v) {
+#pragma unroll
+  for (int b = 0; b < P::E / R; ++b) Bfly<R, DIR>::run(v + b * R);
+}
+
+template <class P, int R, int DIR>
+__device__ __forceinline__ void pass_twiddle(float2* v, int t, const float2* __restrict__ tw) {
+#pragma unroll
+  for (int b = 0; b < P::E / R; ++b) {
+    const int bf = t + P::T * b;
+#pragma unroll
+    for (int s = 1; s < R; ++s) v[b * R + s] = cmul_tw<DIR>(v[b * R + s], __ldg(&tw[(s - 1) * (P::N / R) + bf]));
+  }
+}
+
+// write the state after a radix-R pass, read the operands of the next radix-RN pass
+// (MP = rest size after the finished pass, MN = MP / RN)
+template <class P, int R, int RN, int MP, int NT>
+__device__ __forceinline__ void exchange(float2* v, float2* xb, int t, int gid) {
+  constexpr int MN = MP / RN;
+  group_sync<P::T, NT>(gid);
+#pragma unroll
+  for (int b = 0; b < P::E / R; ++b)
+#pragma unroll
+    for (int s = 0; s < R; ++s) xb[xpad(t + P::T * b + (P::N / R) * s)] = v[b * R + s];
+  group_sync<P::T, NT>(gid);
+#pragma unroll
+  for (int b = 0; b < P::E / RN; ++b) {
+    const int bf = t + P::T * b;
+    const int base = (bf / MN) * MP + (bf % MN);
+#pragma unroll
+    for (int s = 0; s < RN; ++s) v[b * RN + s] = xb[xpad(base + s * MN)];
+  }
+}
+
+// In-register transform of the group's line: DIR = -1 forward exp(-i...), +1 inverse (unscaled).
+// v: E points in the RA-striped layout on entry, RLAST-striped on exit. xb: the group's exchange
+// buffer (P::XB float2). tw: P::TW forward twiddles of this plan. t: thread index inside the group.
+template <class P, int DIR, int NT>
+__device__ __forceinline__ void fft(float2* v, float2* xb, int t, int gid, const float2* __restrict__ tw) {
+  pass_butterflies<P, P::RA, DIR>(v);
+  pass_twiddle<P, P::RA, DIR>(v, t, tw);
+  exchange<P, P::RA, P::RB, P::M1, NT>(v, xb, t, gid);
+  pass_butterflies<P, P::RB, DIR>(v);
+  if constexpr (P::NPASS == 3) {
+    pass_twiddle<P, P::RB, DIR>(v, t, tw + P::TW1);
+    exchange<P, P::RB, P::RC, P::M2, NT>(v, xb, t, gid);
+    pass_butterflies<P, P::RC, DIR>(v);
+  }
+}
+
+}  // namespace rf

@@ -11,7 +11,7 @@ void mm_default_free(void* p, void*);
 
 // kernel classes for launch counting and per-kernel CUDA-event timing (mm_profile)
 enum KernelKind { KK_XFWD = 0, KK_YFWD, KK_YINV, KK_LAST_XY, KK_LAST_Z, KK_LAST_3D, KK_XINV, KK_LOCAL, KK_STAGE,
-                  KK_ERROR, KK_CTRL, KK_OTHER, KK_COUNT };
+                  KK_ERROR, KK_CTRL, KK_OTHER, KK_F2_XFWD, KK_F2_YCOL, KK_F2_XINV, KK_COUNT };
 struct ProfEntry { int kind; cudaEvent_t a, b; };
 
 struct mm_sim {
@@ -35,6 +35,10 @@ struct mm_sim {
   float2 *twx = nullptr, *twy = nullptr, *twz = nullptr;
   double* scratch3 = nullptr;
   ConvArgs conv;
+  float* Kt = nullptr;         // kernel spectrum in the fast 2D layout
+  Fast2DArgs f2;
+  bool fast2d = false;         // fast 2D path available for this box
+  bool force_generic = false;  // mm_set_option(MM_OPT_GENERIC_FFT)
   // host state
   DevState hst;
   bool have_params = false, have_m = false, have_k1 = false;
@@ -58,6 +62,9 @@ int mm_fail(mm_sim* s, int code, const std::string& msg);
 void* mm_dev_alloc(mm_sim* s, size_t bytes);
 void mm_dev_free(mm_sim* s, void* p);
 int mm_build_kernel_spectrum(mm_sim* s);   // setup.cu
+bool mm_fast2d_supported(int Nx, int Ny, int Nz, const int* pbc);   // fast2d.cu
+int mm_fast2d_init(mm_sim* s);
+void mm_fast2d_demag(mm_sim* s, int src_role);
 
 #define CUDA_TRY(s, expr)                                                                       \
   do {                                                                                          \

@@ -145,6 +145,7 @@ int configure_launches(mm_sim* s) {
 
 // B_demag of the field in role `src` -> role R_B
 void launch_demag(mm_sim* s, int src_role) {
+  if (s->fast2d && !s->force_generic) { mm_fast2d_demag(s, src_role); return; }
   const Geometry& g = s->g;
   const int rows = g.Ny * g.Nz, pairs = (rows + 1) / 2;
   const int T = 256;
@@ -302,6 +303,7 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
   if ((rc = upload_twiddles(s, g.Px, &s->twx)) || (rc = upload_twiddles(s, g.Py, &s->twy)) ||
       (rc = upload_twiddles(s, g.Pz, &s->twz)))
     return bail(rc, "twiddles");
+  s->fast2d = mm_fast2d_supported(Nx, Ny, Nz, s->rep);
   if ((rc = mm_build_kernel_spectrum(s))) { std::string m = s->err; return bail(rc, m.c_str()); }
   // convolution arguments
   ConvArgs& c = s->conv;
@@ -310,6 +312,7 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
   c.spec = s->spec; c.rowsS = rowsS; c.cstride = (long long)rowsS * g.pitch;
   c.K = s->K; c.kstride = (long long)g.Cx * g.Hy * g.Hz;
   c.regions = s->regions; c.luts = s->luts; c.st = s->dstate;
+  if (s->fast2d && (rc = mm_fast2d_init(s))) { std::string m = s->err; return bail(rc, m.c_str()); }
   // controller state
   DevState& h = s->hst;
   memset(&h, 0, sizeof(h));
@@ -423,6 +426,14 @@ int mm_set_terms(mm_sim* s, unsigned mask) {
   s->terms = mask & MM_ALL;
   s->have_k1 = false;
   return MM_OK;
+}
+
+int mm_set_option(mm_sim* s, int option, int value) {
+  if (!s) return MM_EINVAL;
+  switch (option) {
+    case MM_OPT_GENERIC_FFT: s->force_generic = value != 0; s->have_k1 = false; return MM_OK;
+    default: return mm_fail(s, MM_EINVAL, "unknown option");
+  }
 }
 
 int mm_set_solver(mm_sim* s, double max_err, double headroom, double fix_dt, double dt_init, double dt_min, double dt_max) {
@@ -601,7 +612,7 @@ int mm_profile(mm_sim* s, int enable) {
 
 int mm_profile_read(mm_sim* s, int kind, const char** name, double* total_ms, long* launches) {
   static const char* names[KK_COUNT] = {"x_fwd", "y_fwd", "y_inv", "last_xy", "last_z", "last_3d", "x_inv", "local",
-                                        "rk_stage", "rk_error", "rk_ctrl", "other"};
+                                        "rk_stage", "rk_error", "rk_ctrl", "other", "f2_xfwd", "f2_ycol", "f2_xinv"};
   if (!s || kind < 0 || kind >= KK_COUNT) return MM_EINVAL;
   if (!s->prof.empty()) {
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));

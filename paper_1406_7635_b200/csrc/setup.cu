@@ -20,6 +20,11 @@ int mm_build_kernel_spectrum(mm_sim* s) {
   const long long nk = (long long)g.Cx * g.Hy * g.Hz;
   s->K = (float*)mm_dev_alloc(s, sizeof(float) * nk * ncomp);
   if (!s->K) return mm_fail(s, MM_ENOMEM, "kernel spectrum");
+  const long long nkt = (long long)g.Cx * (g.Ny + 1);
+  if (s->fast2d) {
+    s->Kt = (float*)mm_dev_alloc(s, sizeof(float) * nkt * 4);
+    if (!s->Kt) return mm_fail(s, MM_ENOMEM, "kernel spectrum (fast layout)");
+  }
   double* oct = (double*)mm_dev_alloc(s, sizeof(double) * noct * 6);
   double2* bufA = (double2*)mm_dev_alloc(s, sizeof(double2) * nfull);
   double2* bufB = (double2*)mm_dev_alloc(s, sizeof(double2) * nfull);
@@ -53,6 +58,11 @@ int mm_build_kernel_spectrum(mm_sim* s) {
     setup::k_pack_spectrum<<<blocks_for(nk, 256), 256, 0, s->stream>>>(tg, src, s->K + (size_t)comp * nk, g.Cx, g.Hy, g.Hz,
                                                                        scale, maxim);
     s->launches++;
+    if (s->fast2d) {
+      setup::k_pack_spectrum_2dfast<<<blocks_for(nkt, 256), 256, 0, s->stream>>>(tg, src, s->Kt + (size_t)comp * nkt, g.Cx,
+                                                                                 g.Ny, scale);
+      s->launches++;
+    }
     CUDA_TRY(s, cudaGetLastError());
   }
   double him = 0.0;

@@ -105,6 +105,26 @@ def test_multi_tile_2d_and_3d_fields(mm):
         _field_check(sim, ref)
 
 
+@pytest.mark.parametrize("grid", [(256, 256, 1), (512, 256, 1), (256, 1024, 1), (2048, 256, 1), (256, 4096, 1),
+                                  (4096, 256, 1), (1024, 1024, 1)])
+def test_fast2d_path_fields(mm, grid):
+    # power-of-two open 2D films take the register-FFT kernels (fast2d.cuh); several CTAs per kernel,
+    # rectangular shapes exercise every plan on either axis; regions exercise the B_sat gather
+    cfg = _rand_cfg(grid, (4e-9, 4e-9, 2e-9), nreg=5, anis=True, seed=21)
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    sim.profile(True)
+    _field_check(sim, ref, (MM_DEMAG, MM_ALL))
+    prof = sim.profile_read()
+    sim.profile(False)
+    assert "f2_ycol" in prof and "f2_xfwd" in prof and "f2_xinv" in prof and "last_xy" not in prof
+    # the generic any-size kernels must agree with it
+    Bf = sim.b_eff(MM_DEMAG)
+    sim.set_option(mm.MM_OPT_GENERIC_FFT, 1)
+    Bg = sim.b_eff(MM_DEMAG)
+    assert np.abs(Bf - Bg).max() <= 2e-5 * np.abs(Bg).max()
+
+
 def test_uniform_m_has_no_exchange_field_and_film_limit(mm):
     cfg = _rand_cfg((64, 64, 1), (5e-9, 5e-9, 1e-9), pbc=(32, 32, 0), nreg=1)
     cfg["m0"][:] = 0; cfg["m0"][2] = 1.0
