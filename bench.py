@@ -49,10 +49,10 @@ def kernel_bytes(kind, n, P):
         "local": 12 * N + 12 * N + N + 12 * N,
         "rk_stage": 12 * N * (1 + 26.0 / 6.0) + 12 * N,      # m0 + on average 26/6 slopes in, y out
         "rk_error": 12 * N * 6,
-        # fused kernels of the fast 2D path
-        "kA": 12 * N * (1 + 26.0 / 6.0) + N + 12 * N + 3 * spec,
-        "kB": 6 * spec + 4 * Hy * Cx * 4,
-        "kC": 3 * spec + 12 * N + N + 12 * N,
+        # register-FFT kernels of the fast 2D path (transposed spectrum, Cx = n + 1 stored kx)
+        "f2_xfwd": 12 * N + N + 3 * spec,
+        "f2_ycol": 6 * spec + 4 * Hy * Cx * 4,
+        "f2_xinv": 3 * spec + 12 * N,
     }
     return float(table.get(kind, 0.0))
 
