@@ -6,12 +6,14 @@
 
 namespace {
 
+// per length: the radix plan (T threads and 16 points per thread for one pair of transforms) and
+// the CTA size NT; a CTA holds G = NT / T FFT groups and therefore 2G rows in the x kernels
 template <int N> struct PlanFor;
-template <> struct PlanFor<4096> { using P = rf::Plan<4096, 256, 16, 16, 16>; static constexpr int NTX = 512, RG = 8, NTY = 256; };
-template <> struct PlanFor<2048> { using P = rf::Plan<2048, 128, 16, 8, 16>; static constexpr int NTX = 256, RG = 8, NTY = 256; };
-template <> struct PlanFor<1024> { using P = rf::Plan<1024, 64, 16, 4, 16>; static constexpr int NTX = 256, RG = 8, NTY = 256; };
-template <> struct PlanFor<512> { using P = rf::Plan<512, 32, 16, 2, 16>; static constexpr int NTX = 256, RG = 16, NTY = 256; };
-template <> struct PlanFor<256> { using P = rf::Plan<256, 16, 16, 16, 1>; static constexpr int NTX = 256, RG = 32, NTY = 256; };
+template <> struct PlanFor<4096> { using P = rf::Plan<4096, 256, 16, 16, 16>; static constexpr int NT = 512; };
+template <> struct PlanFor<2048> { using P = rf::Plan<2048, 128, 16, 8, 16>; static constexpr int NT = 512; };
+template <> struct PlanFor<1024> { using P = rf::Plan<1024, 64, 16, 4, 16>; static constexpr int NT = 256; };
+template <> struct PlanFor<512> { using P = rf::Plan<512, 32, 16, 2, 16>; static constexpr int NT = 256; };
+template <> struct PlanFor<256> { using P = rf::Plan<256, 16, 16, 16, 1>; static constexpr int NT = 128; };
 
 // forward twiddles of a plan, laid out as fft_reg.cuh reads them
 template <class P>
@@ -66,41 +68,45 @@ int axis_tables(mm_sim* s, int N, float2** fwd, float2** rev, float2** half) {
 template <int N>
 int x_attrs(mm_sim* s) {
   using F = PlanFor<N>;
-  const int bytes = (int)k2_x_smem<typename F::P, F::NTX, F::RG>();
-  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd<typename F::P, F::NTX, F::RG>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-  CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv<typename F::P, F::NTX, F::RG>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  const int bytes = (int)k2_smem<typename F::P, F::NT>();
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd<typename F::P, F::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv<typename F::P, F::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   return MM_OK;
 }
 template <int N>
 int y_attrs(mm_sim* s) {
   using F = PlanFor<N>;
-  CUDA_TRY(s, cudaFuncSetAttribute(k2_ycol<typename F::P, F::NTY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   (int)k2_y_smem<typename F::P, F::NTY>()));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_ycol<typename F::P, F::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)k2_smem<typename F::P, F::NT>()));
   return MM_OK;
 }
 
 template <int N>
 void launch_x(mm_sim* s, bool inverse, int role) {
   using F = PlanFor<N>;
-  const dim3 grid(s->g.Ny / F::RG, 3);
-  const size_t bytes = k2_x_smem<typename F::P, F::NTX, F::RG>();
-  if (!inverse) k2_xfwd<typename F::P, F::NTX, F::RG><<<grid, F::NTX, bytes, s->stream>>>(s->f2, role);
-  else k2_xinv<typename F::P, F::NTX, F::RG><<<grid, F::NTX, bytes, s->stream>>>(s->f2, role);
+  constexpr int G = F::NT / F::P::T;
+  const dim3 grid(s->g.Ny / (2 * G), 3);
+  const size_t bytes = k2_smem<typename F::P, F::NT>();
+  if (!inverse) k2_xfwd<typename F::P, F::NT><<<grid, F::NT, bytes, s->stream>>>(s->f2, role);
+  else k2_xinv<typename F::P, F::NT><<<grid, F::NT, bytes, s->stream>>>(s->f2, role);
 }
+// one launch: XY jobs (G/2 columns per CTA) followed by Z jobs (G columns per CTA)
 template <int N>
 void launch_y(mm_sim* s) {
   using F = PlanFor<N>;
-  constexpr int G = F::NTY / F::P::T;
-  k2_ycol<typename F::P, F::NTY><<<(s->f2.Cx + G - 1) / G, F::NTY, k2_y_smem<typename F::P, F::NTY>(), s->stream>>>(s->f2);
+  constexpr int G = F::NT / F::P::T;
+  const int nxy = (s->f2.Cx + G / 2 - 1) / (G / 2), nz = (s->f2.Cx + G - 1) / G;
+  k2_ycol<typename F::P, F::NT><<<nxy + nz, F::NT, k2_smem<typename F::P, F::NT>(), s->stream>>>(s->f2, nxy);
 }
 
+template <int N> constexpr int rows_of() { return 2 * (PlanFor<N>::NT / PlanFor<N>::P::T); }
 int rows_per_cta(int N) {
   switch (N) {
-    case 4096: return PlanFor<4096>::RG;
-    case 2048: return PlanFor<2048>::RG;
-    case 1024: return PlanFor<1024>::RG;
-    case 512: return PlanFor<512>::RG;
-    case 256: return PlanFor<256>::RG;
+    case 4096: return rows_of<4096>();
+    case 2048: return rows_of<2048>();
+    case 1024: return rows_of<1024>();
+    case 512: return rows_of<512>();
+    case 256: return rows_of<256>();
   }
   return 0;
 }

@@ -1,9 +1,16 @@
 // fft_reg.cuh - register-resident power-of-two FFT engine of the fast demag path (sm_100a).
 //
-// One length-N complex transform is computed by a group of T threads, E = N/T points per thread
-// held in registers, in 2 or 3 passes of radix RA, RB[, RC] (N = RA*RB*RC). Between two passes the
-// points are exchanged through a (padded, bank-conflict-free) shared-memory buffer; the first
-// pass reads and the last pass leaves the data in the striped "natural" layout
+// TWO length-N complex transforms run in lockstep in the two lanes of Blackwell's packed fp32
+// instructions (FADD2 / FMUL2 / FFMA2 on 64-bit register pairs): every value is a C2 = (re, im)
+// with re = (re of transform 0, re of transform 1), im likewise, so each butterfly instruction
+// advances both transforms and every shared-memory exchange moves 16 bytes per point. The fast
+// path always has such a pair at hand: the even-bin and the odd-bin half of one zero-padded line
+// (fast2d.cuh). Twiddles are the same for both lanes and enter as broadcast scalars.
+//
+// One pair of transforms is computed by a group of T threads, E = N/T points per thread held in
+// registers, in 2 or 3 passes of radix RA, RB[, RC] (N = RA*RB*RC). Between two passes the points
+// are exchanged through a (padded, bank-conflict-free) shared-memory buffer; the first pass reads
+// and the last pass leaves the data in the striped "natural" layout
 //     point index = bf + (N/R) * s,   bf = t + T*b,   register v[b*R + s]
 // (R = RA on input, R = last radix on output), so that global loads/stores of consecutive threads
 // are contiguous and no digit-reversal pass is ever needed (PAPER.md L123 only asks for "the
@@ -17,37 +24,55 @@
 
 namespace rf {
 
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+struct C2 { float2 re, im; };   // two complex numbers: lane x = transform 0, lane y = transform 1
 
-// a * w (DIR < 0) or a * conj(w) (DIR > 0): tables hold the forward twiddles exp(-i phi)
+__device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }   // folds into the consumer
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __fadd2_rn(a, neg2(b)); }
+__device__ __forceinline__ float2 mul2(float2 a, float s) { return __fmul2_rn(a, make_float2(s, s)); }
+__device__ __forceinline__ float2 fma2(float2 a, float s, float2 c) { return __ffma2_rn(a, make_float2(s, s), c); }
+
+__device__ __forceinline__ C2 cadd(C2 a, C2 b) { return {add2(a.re, b.re), add2(a.im, b.im)}; }
+__device__ __forceinline__ C2 csub(C2 a, C2 b) { return {sub2(a.re, b.re), sub2(a.im, b.im)}; }
+
+// a * w (DIR < 0) or a * conj(w) (DIR > 0): tables hold the forward twiddles w = exp(-i phi)
 template <int DIR>
-__device__ __forceinline__ float2 cmul_tw(float2 a, float2 w) {
+__device__ __forceinline__ C2 cmul_tw(C2 a, float2 w) {
+  if (DIR < 0) return {fma2(a.re, w.x, neg2(mul2(a.im, w.y))), fma2(a.re, w.y, mul2(a.im, w.x))};
+  return {fma2(a.re, w.x, mul2(a.im, w.y)), fma2(a.im, w.x, neg2(mul2(a.re, w.y)))};
+}
+// scalar version (one complex number)
+template <int DIR>
+__device__ __forceinline__ float2 cmul_tw1(float2 a, float2 w) {
   if (DIR < 0) return make_float2(a.x * w.x - a.y * w.y, a.x * w.y + a.y * w.x);
   return make_float2(a.x * w.x + a.y * w.y, a.y * w.x - a.x * w.y);
 }
 
-// multiply by exp(DIR * i * pi/2)
-template <int DIR>
-__device__ __forceinline__ float2 rot90(float2 a) {
-  return DIR < 0 ? make_float2(a.y, -a.x) : make_float2(-a.y, a.x);
-}
 // multiply by exp(DIR * i * pi/4)
 template <int DIR>
-__device__ __forceinline__ float2 rot45(float2 a) {
+__device__ __forceinline__ C2 rot45(C2 a) {
   const float h = 0.70710678118654752f;
-  return DIR < 0 ? make_float2(h * (a.x + a.y), h * (a.y - a.x)) : make_float2(h * (a.x - a.y), h * (a.x + a.y));
+  if (DIR < 0) return {mul2(add2(a.re, a.im), h), mul2(sub2(a.im, a.re), h)};
+  return {mul2(sub2(a.re, a.im), h), mul2(add2(a.re, a.im), h)};
+}
+// multiply by exp(DIR * i * pi/2): a register renaming plus a sign the consumer absorbs
+template <int DIR>
+__device__ __forceinline__ C2 rot90(C2 a) {
+  if (DIR < 0) return {a.im, neg2(a.re)};
+  return {neg2(a.im), a.re};
 }
 // multiply by exp(DIR * i * 3 pi/4)
 template <int DIR>
-__device__ __forceinline__ float2 rot135(float2 a) {
+__device__ __forceinline__ C2 rot135(C2 a) {
   const float h = 0.70710678118654752f;
-  return DIR < 0 ? make_float2(h * (a.y - a.x), -h * (a.x + a.y)) : make_float2(-h * (a.x + a.y), h * (a.x - a.y));
+  if (DIR < 0) return {mul2(sub2(a.im, a.re), h), mul2(add2(a.re, a.im), -h)};
+  return {mul2(add2(a.re, a.im), -h), mul2(sub2(a.re, a.im), h)};
 }
 // multiply by exp(DIR * i * phi) with cos(phi) = C, sin(phi) = S given as literals
 template <int DIR>
-__device__ __forceinline__ float2 rotcs(float2 a, const float C, const float S) {
-  return DIR < 0 ? make_float2(a.x * C + a.y * S, a.y * C - a.x * S) : make_float2(a.x * C - a.y * S, a.y * C + a.x * S);
+__device__ __forceinline__ C2 rotcs(C2 a, const float C, const float S) {
+  if (DIR < 0) return {fma2(a.re, C, mul2(a.im, S)), fma2(a.im, C, neg2(mul2(a.re, S)))};
+  return {fma2(a.re, C, neg2(mul2(a.im, S))), fma2(a.im, C, mul2(a.re, S))};
 }
 
 template <int R, int DIR>
@@ -55,8 +80,8 @@ struct Bfly;
 
 template <int DIR>
 struct Bfly<2, DIR> {
-  static __device__ __forceinline__ void run(float2* v) {
-    float2 a = v[0], b = v[1];
+  static __device__ __forceinline__ void run(C2* v) {
+    C2 a = v[0], b = v[1];
     v[0] = cadd(a, b);
     v[1] = csub(a, b);
   }
@@ -64,21 +89,26 @@ struct Bfly<2, DIR> {
 
 template <int DIR>
 struct Bfly<4, DIR> {
-  static __device__ __forceinline__ void run(float2& v0, float2& v1, float2& v2, float2& v3) {
-    float2 t0 = cadd(v0, v2), t1 = csub(v0, v2), t2 = cadd(v1, v3), t3 = rot90<DIR>(csub(v1, v3));
+  static __device__ __forceinline__ void run(C2& v0, C2& v1, C2& v2, C2& v3) {
+    const C2 t0 = cadd(v0, v2), t1 = csub(v0, v2), t2 = cadd(v1, v3), d = csub(v1, v3);
     v0 = cadd(t0, t2);
     v2 = csub(t0, t2);
-    v1 = cadd(t1, t3);
-    v3 = csub(t1, t3);
+    if (DIR < 0) {   // t3 = -i d = (d.im, -d.re)
+      v1 = {add2(t1.re, d.im), sub2(t1.im, d.re)};
+      v3 = {sub2(t1.re, d.im), add2(t1.im, d.re)};
+    } else {         // t3 = +i d = (-d.im, d.re)
+      v1 = {sub2(t1.re, d.im), add2(t1.im, d.re)};
+      v3 = {add2(t1.re, d.im), sub2(t1.im, d.re)};
+    }
   }
-  static __device__ __forceinline__ void run(float2* v) { run(v[0], v[1], v[2], v[3]); }
+  static __device__ __forceinline__ void run(C2* v) { run(v[0], v[1], v[2], v[3]); }
 };
 
 // 8 = 2 x 4: n = 4a + b, k = c + 2d
 template <int DIR>
 struct Bfly<8, DIR> {
-  static __device__ __forceinline__ void run(float2* v) {
-    float2 A0[4], A1[4];
+  static __device__ __forceinline__ void run(C2* v) {
+    C2 A0[4], A1[4];
 #pragma unroll
     for (int b = 0; b < 4; ++b) {
       A0[b] = cadd(v[b], v[b + 4]);
@@ -100,7 +130,7 @@ struct Bfly<8, DIR> {
 // 16 = 4 x 4: n = 4a + b, k = c + 4d; twiddles W16^{bc}
 template <int DIR>
 struct Bfly<16, DIR> {
-  static __device__ __forceinline__ void run(float2* v) {
+  static __device__ __forceinline__ void run(C2* v) {
     const float C1 = 0.92387953251128674f, S1 = 0.38268343236508977f;  // cos, sin of pi/8
 #pragma unroll
     for (int b = 0; b < 4; ++b) Bfly<4, DIR>::run(v[b], v[b + 4], v[b + 8], v[b + 12]);
@@ -122,7 +152,7 @@ struct Bfly<16, DIR> {
     for (int c = 0; c < 4; ++c)
 #pragma unroll
       for (int d = c + 1; d < 4; ++d) {
-        float2 tmp = v[4 * c + d];
+        C2 tmp = v[4 * c + d];
         v[4 * c + d] = v[4 * d + c];
         v[4 * d + c] = tmp;
       }
@@ -135,7 +165,7 @@ struct Plan {
   static constexpr int NPASS = RC_ > 1 ? 3 : 2;
   static constexpr int RLAST = RC_ > 1 ? RC_ : RB_;
   static constexpr int M1 = N_ / RA_, M2 = M1 / RB_;
-  static constexpr int XB = N_ + N_ / 16;                       // padded exchange buffer (float2)
+  static constexpr int XB = N_ + N_ / 16;                       // padded exchange buffer (float4 units)
   static constexpr int TW1 = (RA_ - 1) * (N_ / RA_);            // twiddle entries after pass 1
   static constexpr int TW2 = RC_ > 1 ? (RB_ - 1) * (N_ / RB_) : 0;
   static constexpr int TW = TW1 + TW2;
@@ -144,7 +174,13 @@ struct Plan {
   typedef Plan<N_, T_, (RC_ > 1 ? RC_ : RB_), (RC_ > 1 ? RB_ : RA_), (RC_ > 1 ? RA_ : 1)> Reversed;
 };
 
+// exchange-buffer index of point a: one 16-byte unit per point, one unit of padding per 16, so that
+// both the unit-stride writes and the stride-16 reads of the last pass hit 8 different 16-byte bank
+// groups per quarter-warp
 __device__ __forceinline__ int xpad(int a) { return a + (a >> 4); }
+
+__device__ __forceinline__ float4 pack(C2 a) { return make_float4(a.re.x, a.re.y, a.im.x, a.im.y); }
+__device__ __forceinline__ C2 unpack(float4 q) { return {make_float2(q.x, q.y), make_float2(q.z, q.w)}; }
 
 // synchronise the T threads of FFT group `gid` of a CTA with NT threads
 template <int T, int NT>
@@ -161,13 +197,13 @@ __device__ __forceinline__ int slot_index(int t, int e) {
 }
 
 template <class P, int R, int DIR>
-__device__ __forceinline__ void pass_butterflies(float2* v) {
+__device__ __forceinline__ void pass_butterflies(C2* v) {
 #pragma unroll
   for (int b = 0; b < P::E / R; ++b) Bfly<R, DIR>::run(v + b * R);
 }
 
 template <class P, int R, int DIR>
-__device__ __forceinline__ void pass_twiddle(float2* v, int t, const float2* __restrict__ tw) {
+__device__ __forceinline__ void pass_twiddle(C2* v, int t, const float2* __restrict__ tw) {
 #pragma unroll
   for (int b = 0; b < P::E / R; ++b) {
     const int bf = t + P::T * b;
@@ -179,28 +215,30 @@ __device__ __forceinline__ void pass_twiddle(float2* v, int t, const float2* __r
 // write the state after a radix-R pass, read the operands of the next radix-RN pass
 // (MP = rest size after the finished pass, MN = MP / RN)
 template <class P, int R, int RN, int MP, int NT>
-__device__ __forceinline__ void exchange(float2* v, float2* xb, int t, int gid) {
+__device__ __forceinline__ void exchange(C2* v, float4* xb, int t, int gid) {
   constexpr int MN = MP / RN;
   group_sync<P::T, NT>(gid);
 #pragma unroll
   for (int b = 0; b < P::E / R; ++b)
 #pragma unroll
-    for (int s = 0; s < R; ++s) xb[xpad(t + P::T * b + (P::N / R) * s)] = v[b * R + s];
+    for (int s = 0; s < R; ++s) xb[xpad(t + P::T * b + (P::N / R) * s)] = pack(v[b * R + s]);
   group_sync<P::T, NT>(gid);
 #pragma unroll
   for (int b = 0; b < P::E / RN; ++b) {
     const int bf = t + P::T * b;
     const int base = (bf / MN) * MP + (bf % MN);
 #pragma unroll
-    for (int s = 0; s < RN; ++s) v[b * RN + s] = xb[xpad(base + s * MN)];
+    for (int s = 0; s < RN; ++s) v[b * RN + s] = unpack(xb[xpad(base + s * MN)]);
   }
 }
 
-// In-register transform of the group's line: DIR = -1 forward exp(-i...), +1 inverse (unscaled).
-// v: E points in the RA-striped layout on entry, RLAST-striped on exit. xb: the group's exchange
-// buffer (P::XB float2). tw: P::TW forward twiddles of this plan. t: thread index inside the group.
+// In-register transform of the group's pair of lines: DIR = -1 forward exp(-i...), +1 inverse
+// (unscaled). v: E points in the RA-striped layout on entry, RLAST-striped on exit. xb: the group's
+// exchange buffer (P::XB float4). tw: P::TW forward twiddles of this plan. t: thread index inside
+// the group. The first exchange starts with a group barrier, so xb may still be read by the group
+// until then; after the call xb is only safe to reuse after another group barrier.
 template <class P, int DIR, int NT>
-__device__ __forceinline__ void fft(float2* v, float2* xb, int t, int gid, const float2* __restrict__ tw) {
+__device__ __forceinline__ void fft(C2* v, float4* xb, int t, int gid, const float2* __restrict__ tw) {
   pass_butterflies<P, P::RA, DIR>(v);
   pass_twiddle<P, P::RA, DIR>(v, t, tw);
   exchange<P, P::RA, P::RB, P::M1, NT>(v, xb, t, gid);
