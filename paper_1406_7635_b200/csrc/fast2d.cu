@@ -9,11 +9,12 @@ namespace {
 // per length: the radix plan (T threads and 16 points per thread for one pair of transforms) and
 // the CTA size NT; a CTA holds G = NT / T FFT groups and therefore 2G rows in the x kernels
 template <int N> struct PlanFor;
-template <> struct PlanFor<4096> { using P = rf::Plan<4096, 256, 16, 16, 16>; static constexpr int NT = 512; };
-template <> struct PlanFor<2048> { using P = rf::Plan<2048, 128, 16, 8, 16>; static constexpr int NT = 512; };
-template <> struct PlanFor<1024> { using P = rf::Plan<1024, 64, 16, 4, 16>; static constexpr int NT = 256; };
-template <> struct PlanFor<512> { using P = rf::Plan<512, 32, 16, 2, 16>; static constexpr int NT = 256; };
-template <> struct PlanFor<256> { using P = rf::Plan<256, 16, 16, 16, 1>; static constexpr int NT = 128; };
+// (NTF: the forward x kernel, whose transposed store wants at least 4 rows = 32-byte pieces)
+template <> struct PlanFor<4096> { using P = rf::Plan<4096, 256, 16, 16, 16>; static constexpr int NT = 256, NTF = 512; };
+template <> struct PlanFor<2048> { using P = rf::Plan<2048, 128, 16, 8, 16>; static constexpr int NT = 256, NTF = 256; };
+template <> struct PlanFor<1024> { using P = rf::Plan<1024, 64, 16, 4, 16>; static constexpr int NT = 256, NTF = 256; };
+template <> struct PlanFor<512> { using P = rf::Plan<512, 32, 16, 2, 16>; static constexpr int NT = 256, NTF = 256; };
+template <> struct PlanFor<256> { using P = rf::Plan<256, 16, 16, 16, 1>; static constexpr int NT = 128, NTF = 128; };
 
 // forward twiddles of a plan, laid out as fft_reg.cuh reads them
 template <class P>
@@ -68,38 +69,39 @@ int axis_tables(mm_sim* s, int N, float2** fwd, float2** rev, float2** half) {
 template <int N>
 int x_attrs(mm_sim* s) {
   using F = PlanFor<N>;
-  const int bytes = (int)k2_smem<typename F::P, F::NT>();
-  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd<typename F::P, F::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-  CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv<typename F::P, F::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd<typename F::P, F::NTF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)k2_smem<typename F::P, F::NTF>()));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv<typename F::P, F::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)k2_smem<typename F::P, F::NT>()));
   return MM_OK;
 }
 template <int N>
 int y_attrs(mm_sim* s) {
   using F = PlanFor<N>;
   CUDA_TRY(s, cudaFuncSetAttribute(k2_ycol<typename F::P, F::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   (int)k2_smem<typename F::P, F::NT>()));
+                                   (int)k2_y_smem<typename F::P, F::NT>()));
   return MM_OK;
 }
 
 template <int N>
 void launch_x(mm_sim* s, bool inverse, int role) {
   using F = PlanFor<N>;
-  constexpr int G = F::NT / F::P::T;
-  const dim3 grid(s->g.Ny / (2 * G), 3);
-  const size_t bytes = k2_smem<typename F::P, F::NT>();
-  if (!inverse) k2_xfwd<typename F::P, F::NT><<<grid, F::NT, bytes, s->stream>>>(s->f2, role);
-  else k2_xinv<typename F::P, F::NT><<<grid, F::NT, bytes, s->stream>>>(s->f2, role);
+  constexpr int GF = F::NTF / F::P::T, GI = F::NT / F::P::T;
+  if (!inverse)
+    k2_xfwd<typename F::P, F::NTF><<<dim3(s->g.Ny / (2 * GF), 3), F::NTF, k2_smem<typename F::P, F::NTF>(), s->stream>>>(s->f2, role);
+  else
+    k2_xinv<typename F::P, F::NT><<<dim3(s->g.Ny / (2 * GI), 3), F::NT, k2_smem<typename F::P, F::NT>(), s->stream>>>(s->f2, role);
 }
-// one launch: XY jobs (G/2 columns per CTA) followed by Z jobs (G columns per CTA)
+// one launch: XY jobs (one column per FFT group) followed by Z jobs (two columns per group)
 template <int N>
 void launch_y(mm_sim* s) {
   using F = PlanFor<N>;
   constexpr int G = F::NT / F::P::T;
-  const int nxy = (s->f2.Cx + G / 2 - 1) / (G / 2), nz = (s->f2.Cx + G - 1) / G;
-  k2_ycol<typename F::P, F::NT><<<nxy + nz, F::NT, k2_smem<typename F::P, F::NT>(), s->stream>>>(s->f2, nxy);
+  const int nxy = (s->f2.Cx + G - 1) / G, nz = ((s->f2.Cx + 1) / 2 + G - 1) / G;
+  k2_ycol<typename F::P, F::NT><<<nxy + nz, F::NT, k2_y_smem<typename F::P, F::NT>(), s->stream>>>(s->f2, nxy);
 }
 
-template <int N> constexpr int rows_of() { return 2 * (PlanFor<N>::NT / PlanFor<N>::P::T); }
+template <int N> constexpr int rows_of() { return 2 * (PlanFor<N>::NTF / PlanFor<N>::P::T); }   // NTF >= NT
 int rows_per_cta(int N) {
   switch (N) {
     case 4096: return rows_of<4096>();

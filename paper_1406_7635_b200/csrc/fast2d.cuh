@@ -10,11 +10,10 @@
 //   K_A  k2_xfwd : rows -> x spectrum. Two real rows a, b form one complex line z = a + i b (one
 //                  FFT group per row pair); the spectra of a and b are separated (Hermitian
 //                  symmetry) on the way out and written TRANSPOSED, spec[c][kx][y], kx = 0..Nx.
-//   K_B  k2_ycol : columns (kx fixed, all y; contiguous). XY job: two FFT groups take the x and the
-//                  y component of one column, transform forward, swap spectra through shared memory,
-//                  each forms its row of the 2x2 symmetric kernel product (K_xx K_xy; K_xy K_yy),
-//                  transforms back, stores in place. Z job: one group per column, K_zz only
-//                  (K_xz = K_yz = 0 for one layer).
+//   K_B  k2_ycol : columns (kx fixed, all y; contiguous), one FFT group per job. XY job: transform the
+//                  x component forward and stash it in shared memory, transform y, form the 2x2
+//                  symmetric kernel product (K_xx K_xy; K_xy K_yy), transform both back, store in
+//                  place. Z job: K_zz only (K_xz = K_yz = 0 for one layer), two columns.
 //   K_C  k2_xinv : x spectrum -> rows of B_demag (only the Nx physical outputs are formed).
 #pragma once
 #include "common.cuh"
@@ -79,18 +78,29 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd(Fast2DArgs a, int src_ro
   // separate the two real rows of every pair and store transposed: lane 0 holds bin kx = 2k,
   // lane 1 bin kx = 2k + 1 of the padded transform; stored kx = 0 .. N
   float2* __restrict__ out = a.spec + (size_t)c * a.cstride;
-  for (int w = tid; w < (N / 2 + 1) * G; w += NT) {
-    const int p = w % G, k = w / G;
+  // (N/2) G items (k, p) over NT = G N/16 threads: exactly 8 per thread; all shared-memory reads first
+  constexpr int IT = (N / 2) * G / NT;
+  static_assert(IT * NT == (N / 2) * G, "items must divide evenly");
+  float4 u[IT]; float2 zm0[IT], zm1[IT];
+#pragma unroll
+  for (int it = 0; it < IT; ++it) {
+    const int w = tid + it * NT, p = w % G, k = w / G;
     const float4* st = smem4 + (size_t)p * GP;
     const float2* st2 = reinterpret_cast<const float2*>(st);
-    const float4 u = st[k];
-    const float2 zm0 = st2[2 * ((N - k) & (N - 1))];
+    u[it] = st[k];
+    zm0[it] = st2[2 * ((N - k) & (N - 1))];
+    zm1[it] = st2[2 * (N - 1 - k) + 1];
+  }
+#pragma unroll
+  for (int it = 0; it < IT; ++it) {
+    const int w = tid + it * NT, p = w % G, k = w / G;
     float2* o = out + (size_t)(2 * k) * a.Ny + r0 + 2 * p;
-    *reinterpret_cast<float4*>(o) = separate(make_float2(u.x, u.y), zm0);
-    if (k < N / 2) {
-      const float2 zm1 = st2[2 * (N - 1 - k) + 1];
-      *reinterpret_cast<float4*>(o + a.Ny) = separate(make_float2(u.z, u.w), zm1);
-    }
+    *reinterpret_cast<float4*>(o) = separate(make_float2(u[it].x, u[it].y), zm0[it]);
+    *reinterpret_cast<float4*>(o + a.Ny) = separate(make_float2(u[it].z, u[it].w), zm1[it]);
+  }
+  if (tid < G) {   // bin kx = N (k = N/2 of the even half): its own partner
+    const float2 z = reinterpret_cast<const float2*>(smem4 + (size_t)tid * GP)[2 * (N / 2)];
+    *reinterpret_cast<float4*>(out + (size_t)N * a.Ny + r0 + 2 * tid) = separate(z, z);
   }
 }
 
@@ -106,22 +116,32 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xinv(Fast2DArgs a, int dst_ro
   const int c = blockIdx.y, r0 = blockIdx.x * 2 * G;
   float* __restrict__ dst = a.st->ptr[dst_role] + (size_t)c * a.ncell;
   const float2* __restrict__ in = a.spec + (size_t)c * a.cstride;
-  // gather bins of the 2G rows; rebuild Z = A + iB and its Hermitian partner for both halves
-  for (int w = tid; w < (N / 2 + 1) * G; w += NT) {
-    const int p = w % G, k = w / G;
-    float4* st = smem4 + (size_t)p * GP;
-    float2* st2 = reinterpret_cast<float2*>(st);
-    const float2* src = in + (size_t)(2 * k) * a.Ny + r0 + 2 * p;
-    const float4 e = *reinterpret_cast<const float4*>(src);
-    const float2 z0 = make_float2(e.x - e.w, e.y + e.z), zm0 = make_float2(e.x + e.w, e.z - e.y);
-    if (k < N / 2) {
-      const float4 o = *reinterpret_cast<const float4*>(src + a.Ny);
-      const float2 z1 = make_float2(o.x - o.w, o.y + o.z), zm1 = make_float2(o.x + o.w, o.z - o.y);
-      st[k] = make_float4(z0.x, z0.y, z1.x, z1.y);
-      if (k > 0) st2[2 * (N - k)] = zm0;
-      st2[2 * (N - 1 - k) + 1] = zm1;
-    } else {
-      st2[2 * k] = z0;            // k = N/2: its own partner; the odd half has no such bin
+  // gather bins of the 2G rows; rebuild Z = A + iB and its Hermitian partner for both halves.
+  // (N/2) G items (k, p) over NT threads: exactly 8 per thread, all 16 loads in flight at once
+  constexpr int IT = (N / 2) * G / NT;
+  static_assert(IT * NT == (N / 2) * G, "items must divide evenly");
+  {
+    float4 ev[IT], od[IT];
+#pragma unroll
+    for (int it = 0; it < IT; ++it) {
+      const int w = tid + it * NT, p = w % G, k = w / G;
+      const float2* src = in + (size_t)(2 * k) * a.Ny + r0 + 2 * p;
+      ev[it] = *reinterpret_cast<const float4*>(src);
+      od[it] = *reinterpret_cast<const float4*>(src + a.Ny);
+    }
+#pragma unroll
+    for (int it = 0; it < IT; ++it) {
+      const int w = tid + it * NT, p = w % G, k = w / G;
+      float4* st = smem4 + (size_t)p * GP;
+      float2* st2 = reinterpret_cast<float2*>(st);
+      const float4 e = ev[it], o = od[it];
+      st[k] = make_float4(e.x - e.w, e.y + e.z, o.x - o.w, o.y + o.z);
+      if (k > 0) st2[2 * (N - k)] = make_float2(e.x + e.w, e.z - e.y);
+      st2[2 * (N - 1 - k) + 1] = make_float2(o.x + o.w, o.z - o.y);
+    }
+    if (tid < G) {   // bin kx = N (k = N/2 of the even half): its own partner; the odd half has no such bin
+      const float4 e = *reinterpret_cast<const float4*>(in + (size_t)N * a.Ny + r0 + 2 * tid);
+      reinterpret_cast<float2*>(smem4 + (size_t)tid * GP)[2 * (N / 2)] = make_float2(e.x - e.w, e.y + e.z);
     }
   }
   __syncthreads();
@@ -151,70 +171,105 @@ __device__ __forceinline__ void k2_kidx(int j, int& i0, int& i1, float& s0, floa
   s1 = j >= N / 2 ? -1.f : 1.f;
 }
 
+// shared memory of one FFT group in k2_ycol: plane-wise exchange buffer (XB float2) + stash (N float4)
+template <class P>
+struct K2YShape {
+  static constexpr int GROUP_BYTES = P::XB * 8 + P::N * 16;
+};
+template <class P, int NT>
+constexpr size_t k2_y_smem() { return (size_t)(NT / P::T) * K2YShape<P>::GROUP_BYTES; }
+
+// Every FFT group works on its own: an XY job is one column (x and y components, coupled by the
+// kernel product), a Z job two columns of the z component - the same number of transforms, so
+// the CTAs of one launch (XY jobs first) take about the same time and several of them share an SM
+// out of phase with one another (butterflies of one over the exchanges and loads of the other).
+__device__ __forceinline__ void k2_prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 template <class P, int NT>
 __global__ void __launch_bounds__(NT, 512 / NT) k2_ycol(Fast2DArgs a, int nxy) {
   if (a.st->skip) return;
   using PI = typename P::Reversed;
-  constexpr int N = P::N, T = P::T, E = P::E, G = NT / T, GP = K2Shape<P, NT>::GP;
-  static_assert(G % 2 == 0, "XY jobs need an even number of FFT groups");
+  constexpr int N = P::N, T = P::T, E = P::E, G = NT / T;
   extern __shared__ float4 smem4[];
   const int tid = threadIdx.x, gid = tid / T, t = tid % T;
-  float4* xb = smem4 + (size_t)gid * GP;
+  char* mine = reinterpret_cast<char*>(smem4) + (size_t)gid * K2YShape<P>::GROUP_BYTES;
+  float4* stash = reinterpret_cast<float4*>(mine);
+  float2* xb = reinterpret_cast<float2*>(mine + (size_t)N * 16);
   const bool xy = (int)blockIdx.x < nxy;
-  const int role = gid & 1;
-  const int kx_raw = xy ? (int)blockIdx.x * (G / 2) + (gid >> 1) : ((int)blockIdx.x - nxy) * G + gid;
-  const bool active = kx_raw < a.Cx;
-  const int kx = active ? kx_raw : a.Cx - 1;       // idle groups shadow the last column, store nothing
-  const int comp = xy ? role : 2;
-  float2* __restrict__ s = a.spec + (size_t)comp * a.cstride + (size_t)kx * a.Ny;
-  const float* __restrict__ Kc = a.Kt + (size_t)kx * (N + 1);
-  rf::C2 v[E];
-#pragma unroll
-  for (int e = 0; e < E; ++e) {
-    const int n = rf::slot_index<P, P::RA>(t, e);
-    const float2 z = s[n];
-    const float2 zw = rf::cmul_tw1<-1>(z, __ldg(&a.twoy[n]));
-    v[e] = {make_float2(z.x, zw.x), make_float2(z.y, zw.y)};
-  }
-  rf::fft<P, -1, NT>(v, xb, t, gid, a.twy);
-  if (xy) {
-    // B~_x = K_xx M~_x + K_xy M~_y,  B~_y = K_xy M~_x + K_yy M~_y   (Eq. 3; K real, L145)
-    rf::group_sync<T, NT>(gid);
-#pragma unroll
-    for (int e = 0; e < E; ++e) xb[e * T + t] = rf::pack(v[e]);
-    __syncthreads();
-    const float4* other = smem4 + (size_t)(gid ^ 1) * GP;
-    const float* __restrict__ Kd = Kc + (size_t)role * a.kstride;
-    const float* __restrict__ Ko = Kc + (size_t)3 * a.kstride;
-#pragma unroll
-    for (int e = 0; e < E; ++e) {
-      int i0, i1; float s0, s1;
-      k2_kidx<N>(rf::slot_index<P, P::RLAST>(t, e), i0, i1, s0, s1);
-      const float2 kd = make_float2(__ldg(&Kd[i0]), __ldg(&Kd[i1]));
-      const float2 ko = make_float2(s0 * __ldg(&Ko[i0]), s1 * __ldg(&Ko[i1]));
-      const rf::C2 o = rf::unpack(other[e * T + t]);
-      v[e].re = __ffma2_rn(ko, o.re, __fmul2_rn(kd, v[e].re));
-      v[e].im = __ffma2_rn(ko, o.im, __fmul2_rn(kd, v[e].im));
+  const int job = xy ? (int)blockIdx.x * G + gid : ((int)blockIdx.x - nxy) * G + gid;
+  const int ncol = xy ? 1 : 2, nc = xy ? 2 : 1, cbase = xy ? 0 : 2;
+#pragma unroll 1
+  for (int q = 0; q < ncol; ++q) {
+    const int kx = xy ? job : 2 * job + q;
+    if (kx >= a.Cx) return;                      // the whole group leaves together
+    float2* __restrict__ col = a.spec + (size_t)kx * a.Ny;
+    const float* __restrict__ Kc = a.Kt + (size_t)kx * (N + 1);
+    // start the kernel-spectrum rows of this column on their way from DRAM to L2
+    for (int i = t * 32; i < N + 1; i += T * 32) {
+      if (xy) { k2_prefetch_l2(Kc + i); k2_prefetch_l2(Kc + a.kstride + i); k2_prefetch_l2(Kc + 3 * a.kstride + i); }
+      else k2_prefetch_l2(Kc + 2 * a.kstride + i);
     }
-    __syncthreads();
-  } else {
-    const float* __restrict__ Kz = Kc + (size_t)2 * a.kstride;
+    rf::C2 v[E];
+#pragma unroll 1
+    for (int c = 0; c < nc; ++c) {
+      const float2* __restrict__ s = col + (size_t)(cbase + c) * a.cstride;
 #pragma unroll
-    for (int e = 0; e < E; ++e) {
-      int i0, i1; float s0, s1;
-      k2_kidx<N>(rf::slot_index<P, P::RLAST>(t, e), i0, i1, s0, s1);
-      const float2 kz = make_float2(__ldg(&Kz[i0]), __ldg(&Kz[i1]));
-      v[e].re = __fmul2_rn(kz, v[e].re);
-      v[e].im = __fmul2_rn(kz, v[e].im);
+      for (int e = 0; e < E; ++e) {
+        const int n = rf::slot_index<P, P::RA>(t, e);
+        const float2 z = s[n];
+        const float2 zw = rf::cmul_tw1<-1>(z, __ldg(&a.twoy[n]));
+        v[e] = {make_float2(z.x, zw.x), make_float2(z.y, zw.y)};
+      }
+      rf::fft<P, -1, NT, true>(v, xb, t, gid, a.twy);
+      if (xy && c == 0) {
+#pragma unroll
+        for (int e = 0; e < E; ++e) stash[e * T + t] = rf::pack(v[e]);     // own slots: no barrier
+      }
     }
-  }
-  rf::fft<PI, +1, NT>(v, xb, t, gid, a.twy_r);
-  if (active) {
+    if (xy) {
+      // B~_x = K_xx M~_x + K_xy M~_y,  B~_y = K_xy M~_x + K_yy M~_y   (Eq. 3; K real, L145)
+      const float* __restrict__ Ky = Kc + a.kstride;
+      const float* __restrict__ Ko = Kc + (size_t)3 * a.kstride;
 #pragma unroll
-    for (int e = 0; e < E; ++e) {
-      const int n = rf::slot_index<PI, PI::RLAST>(t, e);
-      const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), __ldg(&a.twoy[n]));
-      s[n] = make_float2(v[e].re.x + u.x, v[e].im.x + u.y);
+      for (int e = 0; e < E; ++e) {
+        int i0, i1; float s0, s1;
+        k2_kidx<N>(rf::slot_index<P, P::RLAST>(t, e), i0, i1, s0, s1);
+        const float2 kxx = make_float2(__ldg(&Kc[i0]), __ldg(&Kc[i1]));
+        const float2 kyy = make_float2(__ldg(&Ky[i0]), __ldg(&Ky[i1]));
+        const float2 kxy = make_float2(s0 * __ldg(&Ko[i0]), s1 * __ldg(&Ko[i1]));
+        const rf::C2 X = rf::unpack(stash[e * T + t]), Y = v[e];
+        rf::C2 bx;
+        bx.re = __ffma2_rn(kxy, Y.re, __fmul2_rn(kxx, X.re));
+        bx.im = __ffma2_rn(kxy, Y.im, __fmul2_rn(kxx, X.im));
+        stash[e * T + t] = rf::pack(bx);
+        v[e].re = __ffma2_rn(kxy, X.re, __fmul2_rn(kyy, Y.re));
+        v[e].im = __ffma2_rn(kxy, X.im, __fmul2_rn(kyy, Y.im));
+      }
+    } else {
+      const float* __restrict__ Kz = Kc + (size_t)2 * a.kstride;
+#pragma unroll
+      for (int e = 0; e < E; ++e) {
+        int i0, i1; float s0, s1;
+        k2_kidx<N>(rf::slot_index<P, P::RLAST>(t, e), i0, i1, s0, s1);
+        const float2 kz = make_float2(__ldg(&Kz[i0]), __ldg(&Kz[i1]));
+        v[e].re = __fmul2_rn(kz, v[e].re);
+        v[e].im = __fmul2_rn(kz, v[e].im);
+      }
+    }
+#pragma unroll 1
+    for (int c = nc - 1; c >= 0; --c) {
+      if (xy && c == 0) {
+#pragma unroll
+        for (int e = 0; e < E; ++e) v[e] = rf::unpack(stash[e * T + t]);
+      }
+      rf::fft<PI, +1, NT, true>(v, xb, t, gid, a.twy_r);
+      float2* __restrict__ d = col + (size_t)(cbase + c) * a.cstride;
+#pragma unroll
+      for (int e = 0; e < E; ++e) {
+        const int n = rf::slot_index<PI, PI::RLAST>(t, e);
+        const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), __ldg(&a.twoy[n]));
+        d[n] = make_float2(v[e].re.x + u.x, v[e].im.x + u.y);
+      }
     }
   }
 }

@@ -202,51 +202,100 @@ __device__ __forceinline__ void pass_butterflies(C2* v) {
   for (int b = 0; b < P::E / R; ++b) Bfly<R, DIR>::run(v + b * R);
 }
 
-template <class P, int R, int DIR>
-__device__ __forceinline__ void pass_twiddle(C2* v, int t, const float2* __restrict__ tw) {
-#pragma unroll
-  for (int b = 0; b < P::E / R; ++b) {
-    const int bf = t + P::T * b;
-#pragma unroll
-    for (int s = 1; s < R; ++s) v[b * R + s] = cmul_tw<DIR>(v[b * R + s], __ldg(&tw[(s - 1) * (P::N / R) + bf]));
-  }
-}
-
-// write the state after a radix-R pass, read the operands of the next radix-RN pass
-// (MP = rest size after the finished pass, MN = MP / RN)
-template <class P, int R, int RN, int MP, int NT>
-__device__ __forceinline__ void exchange(C2* v, float4* xb, int t, int gid) {
-  constexpr int MN = MP / RN;
-  group_sync<P::T, NT>(gid);
+// twiddles of the pass that follows a radix-R butterfly: fetched early (before the butterflies or
+// before the preceding exchange) so that their latency hides behind that work
+template <class P, int R>
+__device__ __forceinline__ void load_twiddles(float2* w, int t, const float2* __restrict__ tw) {
 #pragma unroll
   for (int b = 0; b < P::E / R; ++b)
 #pragma unroll
-    for (int s = 0; s < R; ++s) xb[xpad(t + P::T * b + (P::N / R) * s)] = pack(v[b * R + s]);
-  group_sync<P::T, NT>(gid);
+    for (int s = 1; s < R; ++s) w[b * (R - 1) + s - 1] = __ldg(&tw[(s - 1) * (P::N / R) + t + P::T * b]);
+}
+
+template <class P, int R, int DIR>
+__device__ __forceinline__ void apply_twiddles(C2* v, const float2* w) {
 #pragma unroll
-  for (int b = 0; b < P::E / RN; ++b) {
-    const int bf = t + P::T * b;
-    const int base = (bf / MN) * MP + (bf % MN);
+  for (int b = 0; b < P::E / R; ++b)
 #pragma unroll
-    for (int s = 0; s < RN; ++s) v[b * RN + s] = unpack(xb[xpad(base + s * MN)]);
+    for (int s = 1; s < R; ++s) v[b * R + s] = cmul_tw<DIR>(v[b * R + s], w[b * (R - 1) + s - 1]);
+}
+
+__host__ __device__ constexpr int xpadc(int c) { return c + c / 16; }
+
+// Write the state after a radix-R pass, read the operands of the next radix-RN pass
+// (MP = rest size after the finished pass, MN = MP / RN). All indices are xpad(thread part) plus a
+// compile-time constant: the constant parts are multiples of 16 or stay inside one 16-block, so
+// xpad is additive over them and every access is base register + immediate.
+// PLANES = false: one 16-byte unit per point (xb = XB float4), two group barriers.
+// PLANES = true : the re pairs and then the im pairs go through a buffer of 8-byte units (xb = XB
+//                 float2, half the shared memory), four group barriers.
+template <class P, int R, int RN, int MP, int NT, bool PLANES>
+__device__ __forceinline__ void exchange(C2* v, void* xbuf, int t, int gid) {
+  constexpr int MN = MP / RN;
+  static_assert(MP % 16 == 0 && (MN % 16 == 0 || MP == 16) && P::T % 16 == 0 && P::T % MN == 0,
+                "exchange indices must be affine under xpad");
+  const int wbase = xpad(t);
+  const int rbase = xpad((t / MN) * MP + (t % MN));
+  constexpr int RB_STEP = (P::T / MN) * MP;      // read-base step per butterfly index b
+  if constexpr (!PLANES) {
+    float4* xb = reinterpret_cast<float4*>(xbuf);
+    group_sync<P::T, NT>(gid);
+#pragma unroll
+    for (int b = 0; b < P::E / R; ++b)
+#pragma unroll
+      for (int s = 0; s < R; ++s) xb[wbase + xpadc(P::T * b + (P::N / R) * s)] = pack(v[b * R + s]);
+    group_sync<P::T, NT>(gid);
+#pragma unroll
+    for (int b = 0; b < P::E / RN; ++b)
+#pragma unroll
+      for (int s = 0; s < RN; ++s) v[b * RN + s] = unpack(xb[rbase + xpadc(RB_STEP * b + s * MN)]);
+  } else {
+    float2* xb = reinterpret_cast<float2*>(xbuf);
+    group_sync<P::T, NT>(gid);
+#pragma unroll
+    for (int b = 0; b < P::E / R; ++b)
+#pragma unroll
+      for (int s = 0; s < R; ++s) xb[wbase + xpadc(P::T * b + (P::N / R) * s)] = v[b * R + s].re;
+    group_sync<P::T, NT>(gid);
+#pragma unroll
+    for (int b = 0; b < P::E / RN; ++b)
+#pragma unroll
+      for (int s = 0; s < RN; ++s) v[b * RN + s].re = xb[rbase + xpadc(RB_STEP * b + s * MN)];
+    group_sync<P::T, NT>(gid);
+#pragma unroll
+    for (int b = 0; b < P::E / R; ++b)
+#pragma unroll
+      for (int s = 0; s < R; ++s) xb[wbase + xpadc(P::T * b + (P::N / R) * s)] = v[b * R + s].im;
+    group_sync<P::T, NT>(gid);
+#pragma unroll
+    for (int b = 0; b < P::E / RN; ++b)
+#pragma unroll
+      for (int s = 0; s < RN; ++s) v[b * RN + s].im = xb[rbase + xpadc(RB_STEP * b + s * MN)];
   }
 }
 
 // In-register transform of the group's pair of lines: DIR = -1 forward exp(-i...), +1 inverse
 // (unscaled). v: E points in the RA-striped layout on entry, RLAST-striped on exit. xb: the group's
-// exchange buffer (P::XB float4). tw: P::TW forward twiddles of this plan. t: thread index inside
+// exchange buffer (P::XB float4, or P::XB float2 with PLANES). tw: P::TW forward twiddles of this plan. t: thread index inside
 // the group. The first exchange starts with a group barrier, so xb may still be read by the group
 // until then; after the call xb is only safe to reuse after another group barrier.
-template <class P, int DIR, int NT>
-__device__ __forceinline__ void fft(C2* v, float4* xb, int t, int gid, const float2* __restrict__ tw) {
+template <class P, int DIR, int NT, bool PLANES = false>
+__device__ __forceinline__ void fft(C2* v, void* xb, int t, int gid, const float2* __restrict__ tw) {
+  float2 w[(P::RA - 1) * (P::E / P::RA)];
+  load_twiddles<P, P::RA>(w, t, tw);
   pass_butterflies<P, P::RA, DIR>(v);
-  pass_twiddle<P, P::RA, DIR>(v, t, tw);
-  exchange<P, P::RA, P::RB, P::M1, NT>(v, xb, t, gid);
-  pass_butterflies<P, P::RB, DIR>(v);
+  apply_twiddles<P, P::RA, DIR>(v, w);
   if constexpr (P::NPASS == 3) {
-    pass_twiddle<P, P::RB, DIR>(v, t, tw + P::TW1);
-    exchange<P, P::RB, P::RC, P::M2, NT>(v, xb, t, gid);
+    float2 w2[(P::RB - 1) * (P::E / P::RB)];
+    load_twiddles<P, P::RB>(w2, t, tw + P::TW1);
+    exchange<P, P::RA, P::RB, P::M1, NT, PLANES>(v, xb, t, gid);
+    pass_butterflies<P, P::RB, DIR>(v);
+    apply_twiddles<P, P::RB, DIR>(v, w2);
+    exchange<P, P::RB, P::RC, P::M2, NT, PLANES>(v, xb, t, gid);
     pass_butterflies<P, P::RC, DIR>(v);
+  } else {
+    exchange<P, P::RA, P::RB, P::M1, NT, PLANES>(v, xb, t, gid);
+    pass_butterflies<P, P::RB, DIR>(v);
   }
 }
 

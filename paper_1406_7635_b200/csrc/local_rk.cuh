@@ -81,6 +81,132 @@ __global__ void k_local(Geometry g, const uint8_t* __restrict__ regions, const L
   dst[i] = bx; dst[N + i] = by; dst[2 * N + i] = bz;
 }
 
+// Same computation, four consecutive x cells per thread (Nx % 4 == 0): 16-byte loads of m, its y/z
+// neighbour rows, B_demag and the region bytes; only the two x-edge neighbours are scalar loads.
+// UNIFORM = one region: no region gathers, the exchange coefficient is a constant.
+// grid = (Nx/4 / blockDim.x, Ny, Nz)
+template <bool UNIFORM>
+__global__ void __launch_bounds__(128) k_local4(Geometry g, const uint8_t* __restrict__ regions, const Luts* __restrict__ lut,
+                                                DevState* st, int m_role, int bd_role, int dst_role, unsigned mask,
+                                                int out_torque) {
+  if (st->skip) return;
+  const int x4 = blockIdx.x * blockDim.x + threadIdx.x;
+  if (x4 * 4 >= g.Nx) return;
+  const int x = x4 * 4, y = blockIdx.y, z = blockIdx.z;
+  const long long N = g.N;
+  const long long row = ((long long)z * g.Ny + y) * g.Nx;
+  const long long i = row + x;
+  const float* __restrict__ m = st->ptr[m_role];
+  const float* __restrict__ bd = st->ptr[bd_role];
+  float* __restrict__ dst = st->ptr[dst_role];
+  float mc[3][4], b[3][4];
+  int r[4] = {0, 0, 0, 0};
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const float4 q = *reinterpret_cast<const float4*>(m + c * N + i);
+    mc[c][0] = q.x; mc[c][1] = q.y; mc[c][2] = q.z; mc[c][3] = q.w;
+    if (mask & MM_DEMAG) {
+      const float4 d = *reinterpret_cast<const float4*>(bd + c * N + i);
+      b[c][0] = d.x; b[c][1] = d.y; b[c][2] = d.z; b[c][3] = d.w;
+    } else {
+      b[c][0] = b[c][1] = b[c][2] = b[c][3] = 0.f;
+    }
+  }
+  if (!UNIFORM) {
+    const uchar4 q = *reinterpret_cast<const uchar4*>(regions + i);
+    r[0] = q.x; r[1] = q.y; r[2] = q.z; r[3] = q.w;
+  }
+  if (mask & MM_EXCH) {
+    const float a0 = lut->exch[0];
+    // a whole neighbour row segment (y or z direction): j = index of its first cell
+    auto nb_row = [&](long long j, float w) {
+      int rn[4] = {0, 0, 0, 0};
+      if (!UNIFORM) {
+        const uchar4 q = *reinterpret_cast<const uchar4*>(regions + j);
+        rn[0] = q.x; rn[1] = q.y; rn[2] = q.z; rn[3] = q.w;
+      }
+      float a[4];
+#pragma unroll
+      for (int l = 0; l < 4; ++l) a[l] = w * (UNIFORM ? a0 : __ldg(&lut->exch[tri_index(r[l], rn[l])]));
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        const float4 q = *reinterpret_cast<const float4*>(m + c * N + j);
+        b[c][0] += a[0] * (q.x - mc[c][0]); b[c][1] += a[1] * (q.y - mc[c][1]);
+        b[c][2] += a[2] * (q.z - mc[c][2]); b[c][3] += a[3] * (q.w - mc[c][3]);
+      }
+    };
+    // one neighbour cell j of lane l
+    auto nb_one = [&](int l, long long j, float w) {
+      const float a = w * (UNIFORM ? a0 : __ldg(&lut->exch[tri_index(r[l], regions[j])]));
+#pragma unroll
+      for (int c = 0; c < 3; ++c) b[c][l] += a * (m[c * N + j] - mc[c][l]);
+    };
+    if (g.Nx > 1) {
+      const float w = g.inv_dx2;
+      // interior x neighbours come from the registers
+#pragma unroll
+      for (int l = 0; l < 3; ++l) {
+        const float a = w * (UNIFORM ? a0 : __ldg(&lut->exch[tri_index(r[l], r[l + 1])]));
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          const float d = mc[c][l + 1] - mc[c][l];
+          b[c][l] += a * d; b[c][l + 1] -= a * d;
+        }
+      }
+      if (x > 0) nb_one(0, i - 1, w); else if (g.pbc[0]) nb_one(0, row + g.Nx - 1, w);
+      if (x + 4 < g.Nx) nb_one(3, i + 4, w); else if (g.pbc[0]) nb_one(3, row, w);
+    }
+    if (g.Ny > 1) {
+      const long long s = g.Nx;
+      if (y + 1 < g.Ny) nb_row(i + s, g.inv_dy2); else if (g.pbc[1]) nb_row(i + s - s * g.Ny, g.inv_dy2);
+      if (y > 0) nb_row(i - s, g.inv_dy2); else if (g.pbc[1]) nb_row(i - s + s * g.Ny, g.inv_dy2);
+    }
+    if (g.Nz > 1) {
+      const long long s = (long long)g.Nx * g.Ny;
+      if (z + 1 < g.Nz) nb_row(i + s, g.inv_dz2); else if (g.pbc[2]) nb_row(i + s - s * g.Nz, g.inv_dz2);
+      if (z > 0) nb_row(i - s, g.inv_dz2); else if (g.pbc[2]) nb_row(i - s + s * g.Nz, g.inv_dz2);
+    }
+  }
+  const bool uni = (mask & MM_ANIS) && lut->has_uniaxial, cub = (mask & MM_ANIS) && lut->has_cubic;
+#pragma unroll
+  for (int l = 0; l < 4; ++l) {
+    const int rr = r[l];
+    const float mx = mc[0][l], my = mc[1][l], mz = mc[2][l];
+    float bx = b[0][l], by = b[1][l], bz = b[2][l];
+    if (uni) {
+      float ux = lut->u[0][rr], uy = lut->u[1][rr], uz = lut->u[2][rr];
+      float um = ux * mx + uy * my + uz * mz;
+      float sc = lut->ku1[rr] * um + lut->ku2[rr] * um * um * um;
+      bx += sc * ux; by += sc * uy; bz += sc * uz;
+    }
+    if (cub) {
+      float c1x = lut->c1[0][rr], c1y = lut->c1[1][rr], c1z = lut->c1[2][rr];
+      float c2x = lut->c2[0][rr], c2y = lut->c2[1][rr], c2z = lut->c2[2][rr];
+      float c3x = lut->c3[0][rr], c3y = lut->c3[1][rr], c3z = lut->c3[2][rr];
+      float a1 = c1x * mx + c1y * my + c1z * mz, a2 = c2x * mx + c2y * my + c2z * mz, a3 = c3x * mx + c3y * my + c3z * mz;
+      float q1 = a1 * a1, q2 = a2 * a2, q3 = a3 * a3;
+      float k1 = lut->kc1[rr], k2 = lut->kc2[rr], k3 = lut->kc3[rr];
+      float f1 = (k1 * (q2 + q3) + k2 * (q2 * q3) + k3 * (q2 * q2 + q3 * q3) * q1) * a1;
+      float f2 = (k1 * (q1 + q3) + k2 * (q1 * q3) + k3 * (q1 * q1 + q3 * q3) * q2) * a2;
+      float f3 = (k1 * (q1 + q2) + k2 * (q1 * q2) + k3 * (q1 * q1 + q2 * q2) * q3) * a3;
+      bx += f1 * c1x + f2 * c2x + f3 * c3x;
+      by += f1 * c1y + f2 * c2y + f3 * c3y;
+      bz += f1 * c1z + f2 * c2z + f3 * c3z;
+    }
+    if (mask & MM_ZEEMAN) { bx += lut->bext[0]; by += lut->bext[1]; bz += lut->bext[2]; }
+    if (out_torque) {
+      const float al = lut->alpha[rr];
+      const float pre = -lut->live[rr] / (1.f + al * al);
+      float tx = my * bz - mz * by, ty = mz * bx - mx * bz, tz = mx * by - my * bx;   // m x B
+      float dx = my * tz - mz * ty, dy = mz * tx - mx * tz, dz = mx * ty - my * tx;   // m x (m x B)
+      bx = pre * (tx + al * dx); by = pre * (ty + al * dy); bz = pre * (tz + al * dz);
+    }
+    b[0][l] = bx; b[1][l] = by; b[2][l] = bz;
+  }
+#pragma unroll
+  for (int c = 0; c < 3; ++c) *reinterpret_cast<float4*>(dst + c * N + i) = make_float4(b[c][0], b[c][1], b[c][2], b[c][3]);
+}
+
 // Dormand-Prince stage input y_i = normalise(m0 + h sum_j a_ij k_j) (L365; every stage input is
 // renormalised, reading #9). k_j are torques over gamma [T], hg = gamma * h.
 struct StageCoef { float a[6]; int n; };

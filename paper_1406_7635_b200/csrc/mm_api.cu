@@ -170,8 +170,18 @@ void launch_demag(mm_sim* s, int src_role) {
 void launch_eval(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_torque) {
   if (mask & MM_DEMAG) launch_demag(s, src_role);
   Launch l(s, KK_LOCAL);
-  k_local<<<blocks_for(s->g.N, 256), 256, 0, s->stream>>>(s->g, s->regions, s->luts, s->dstate, src_role, R_B, dst_role,
-                                                         mask, out_torque);
+  const Geometry& g = s->g;
+  if (g.Nx % 4 == 0 && g.Ny <= 65535 && g.Nz <= 65535) {
+    const int q = g.Nx / 4, bt = q >= 128 ? 128 : (q >= 64 ? 64 : 32);
+    const dim3 grid((q + bt - 1) / bt, g.Ny, g.Nz);
+    if (s->nregions == 1)
+      k_local4<true><<<grid, bt, 0, s->stream>>>(g, s->regions, s->luts, s->dstate, src_role, R_B, dst_role, mask, out_torque);
+    else
+      k_local4<false><<<grid, bt, 0, s->stream>>>(g, s->regions, s->luts, s->dstate, src_role, R_B, dst_role, mask, out_torque);
+    return;
+  }
+  k_local<<<blocks_for(g.N, 256), 256, 0, s->stream>>>(g, s->regions, s->luts, s->dstate, src_role, R_B, dst_role, mask,
+                                                       out_torque);
 }
 
 void enqueue_step(mm_sim* s) {
