@@ -92,12 +92,12 @@ void launch_x(mm_sim* s, bool inverse, int role) {
   else
     k2_xinv<typename F::P, F::NT><<<dim3(s->g.Ny / (2 * GI), 3), F::NT, k2_smem<typename F::P, F::NT>(), s->stream>>>(s->f2, role);
 }
-// one launch: XY jobs (one column per FFT group) followed by Z jobs (two columns per group)
+// one launch: XY jobs (one column per FFT group) followed by Z jobs (one column per group)
 template <int N>
 void launch_y(mm_sim* s) {
   using F = PlanFor<N>;
   constexpr int G = F::NT / F::P::T;
-  const int nxy = (s->f2.Cx + G - 1) / G, nz = ((s->f2.Cx + 1) / 2 + G - 1) / G;
+  const int nxy = (s->f2.Cx + G - 1) / G, nz = nxy;
   k2_ycol<typename F::P, F::NT><<<nxy + nz, F::NT, k2_y_smem<typename F::P, F::NT>(), s->stream>>>(s->f2, nxy);
 }
 

@@ -179,16 +179,47 @@ struct K2YShape {
 template <class P, int NT>
 constexpr size_t k2_y_smem() { return (size_t)(NT / P::T) * K2YShape<P>::GROUP_BYTES; }
 
-// Every FFT group works on its own: an XY job is one column (x and y components, coupled by the
-// kernel product), a Z job two columns of the z component - the same number of transforms, so
-// the CTAs of one launch (XY jobs first) take about the same time and several of them share an SM
-// out of phase with one another (butterflies of one over the exchanges and loads of the other).
 __device__ __forceinline__ void k2_prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
+// Every FFT group works on its own: an XY job is one column of the x and y components (coupled by
+// the kernel product), a Z job one column of the z component. All code is straight-line (a rolled
+// loop over components would carry the 64-register point array around its back edge, which costs
+// a register permutation through local memory). Several CTAs share an SM out of phase with one
+// another: butterflies of one over the exchanges and loads of the other.
+template <class P, int NT>
+struct K2Col {
+  using PI = typename P::Reversed;
+  static constexpr int N = P::N, T = P::T, E = P::E;
+
+  // column -> lanes (z[n], z[n] w^n) -> forward transforms of the even and the odd bins
+  static __device__ __forceinline__ void load_fwd(const Fast2DArgs& a, const float2* __restrict__ s, rf::C2* v, float2* xb,
+                                                  int t, int gid) {
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+      const int n = rf::slot_index<P, P::RA>(t, e);
+      const float2 z = s[n];
+      const float2 zw = rf::cmul_tw1<-1>(z, __ldg(&a.twoy[n]));
+      v[e] = {make_float2(z.x, zw.x), make_float2(z.y, zw.y)};
+    }
+    rf::fft<P, -1, NT, true>(v, xb, t, gid, a.twy);
+  }
+  // inverse transforms -> first N samples: even part + conj(w)^n odd part -> column (in place)
+  static __device__ __forceinline__ void inv_store(const Fast2DArgs& a, float2* __restrict__ d, rf::C2* v, float2* xb, int t,
+                                                   int gid) {
+    rf::fft<PI, +1, NT, true>(v, xb, t, gid, a.twy_r);
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+      const int n = rf::slot_index<PI, PI::RLAST>(t, e);
+      const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), __ldg(&a.twoy[n]));
+      d[n] = make_float2(v[e].re.x + u.x, v[e].im.x + u.y);
+    }
+  }
+};
 
 template <class P, int NT>
 __global__ void __launch_bounds__(NT, 512 / NT) k2_ycol(Fast2DArgs a, int nxy) {
   if (a.st->skip) return;
-  using PI = typename P::Reversed;
+  using C = K2Col<P, NT>;
   constexpr int N = P::N, T = P::T, E = P::E, G = NT / T;
   extern __shared__ float4 smem4[];
   const int tid = threadIdx.x, gid = tid / T, t = tid % T;
@@ -196,80 +227,55 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_ycol(Fast2DArgs a, int nxy) {
   float4* stash = reinterpret_cast<float4*>(mine);
   float2* xb = reinterpret_cast<float2*>(mine + (size_t)N * 16);
   const bool xy = (int)blockIdx.x < nxy;
-  const int job = xy ? (int)blockIdx.x * G + gid : ((int)blockIdx.x - nxy) * G + gid;
-  const int ncol = xy ? 1 : 2, nc = xy ? 2 : 1, cbase = xy ? 0 : 2;
-#pragma unroll 1
-  for (int q = 0; q < ncol; ++q) {
-    const int kx = xy ? job : 2 * job + q;
-    if (kx >= a.Cx) return;                      // the whole group leaves together
-    float2* __restrict__ col = a.spec + (size_t)kx * a.Ny;
-    const float* __restrict__ Kc = a.Kt + (size_t)kx * (N + 1);
-    // start the kernel-spectrum rows of this column on their way from DRAM to L2
-    for (int i = t * 32; i < N + 1; i += T * 32) {
-      if (xy) { k2_prefetch_l2(Kc + i); k2_prefetch_l2(Kc + a.kstride + i); k2_prefetch_l2(Kc + 3 * a.kstride + i); }
-      else k2_prefetch_l2(Kc + 2 * a.kstride + i);
+  const int kx = xy ? (int)blockIdx.x * G + gid : ((int)blockIdx.x - nxy) * G + gid;
+  if (kx >= a.Cx) return;                      // the whole group leaves together
+  float2* __restrict__ col = a.spec + (size_t)kx * a.Ny;
+  const float* __restrict__ Kc = a.Kt + (size_t)kx * (N + 1);
+  // start the kernel-spectrum rows of this column on their way from DRAM to L2
+  for (int i = t * 32; i < N + 1; i += T * 32) {
+    if (xy) { k2_prefetch_l2(Kc + i); k2_prefetch_l2(Kc + a.kstride + i); k2_prefetch_l2(Kc + 3 * a.kstride + i); }
+    else k2_prefetch_l2(Kc + 2 * a.kstride + i);
+  }
+  rf::C2 v[E];
+  if (xy) {
+    C::load_fwd(a, col, v, xb, t, gid);
+#pragma unroll
+    for (int e = 0; e < E; ++e) stash[e * T + t] = rf::pack(v[e]);     // own slots: no barrier
+    C::load_fwd(a, col + a.cstride, v, xb, t, gid);
+    // B~_x = K_xx M~_x + K_xy M~_y,  B~_y = K_xy M~_x + K_yy M~_y   (Eq. 3; K real, L145)
+    const float* __restrict__ Ky = Kc + a.kstride;
+    const float* __restrict__ Ko = Kc + (size_t)3 * a.kstride;
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+      int i0, i1; float s0, s1;
+      k2_kidx<N>(rf::slot_index<P, P::RLAST>(t, e), i0, i1, s0, s1);
+      const float2 kxx = make_float2(__ldg(&Kc[i0]), __ldg(&Kc[i1]));
+      const float2 kyy = make_float2(__ldg(&Ky[i0]), __ldg(&Ky[i1]));
+      const float2 kxy = make_float2(s0 * __ldg(&Ko[i0]), s1 * __ldg(&Ko[i1]));
+      const rf::C2 X = rf::unpack(stash[e * T + t]), Y = v[e];
+      rf::C2 bx;
+      bx.re = __ffma2_rn(kxy, Y.re, __fmul2_rn(kxx, X.re));
+      bx.im = __ffma2_rn(kxy, Y.im, __fmul2_rn(kxx, X.im));
+      stash[e * T + t] = rf::pack(bx);
+      v[e].re = __ffma2_rn(kxy, X.re, __fmul2_rn(kyy, Y.re));
+      v[e].im = __ffma2_rn(kxy, X.im, __fmul2_rn(kyy, Y.im));
     }
-    rf::C2 v[E];
-#pragma unroll 1
-    for (int c = 0; c < nc; ++c) {
-      const float2* __restrict__ s = col + (size_t)(cbase + c) * a.cstride;
+    C::inv_store(a, col + a.cstride, v, xb, t, gid);
 #pragma unroll
-      for (int e = 0; e < E; ++e) {
-        const int n = rf::slot_index<P, P::RA>(t, e);
-        const float2 z = s[n];
-        const float2 zw = rf::cmul_tw1<-1>(z, __ldg(&a.twoy[n]));
-        v[e] = {make_float2(z.x, zw.x), make_float2(z.y, zw.y)};
-      }
-      rf::fft<P, -1, NT, true>(v, xb, t, gid, a.twy);
-      if (xy && c == 0) {
+    for (int e = 0; e < E; ++e) v[e] = rf::unpack(stash[e * T + t]);
+    C::inv_store(a, col, v, xb, t, gid);
+  } else {
+    float2* __restrict__ cz = col + 2 * a.cstride;
+    C::load_fwd(a, cz, v, xb, t, gid);
+    const float* __restrict__ Kz = Kc + (size_t)2 * a.kstride;
 #pragma unroll
-        for (int e = 0; e < E; ++e) stash[e * T + t] = rf::pack(v[e]);     // own slots: no barrier
-      }
+    for (int e = 0; e < E; ++e) {
+      int i0, i1; float s0, s1;
+      k2_kidx<N>(rf::slot_index<P, P::RLAST>(t, e), i0, i1, s0, s1);
+      const float2 kz = make_float2(__ldg(&Kz[i0]), __ldg(&Kz[i1]));
+      v[e].re = __fmul2_rn(kz, v[e].re);
+      v[e].im = __fmul2_rn(kz, v[e].im);
     }
-    if (xy) {
-      // B~_x = K_xx M~_x + K_xy M~_y,  B~_y = K_xy M~_x + K_yy M~_y   (Eq. 3; K real, L145)
-      const float* __restrict__ Ky = Kc + a.kstride;
-      const float* __restrict__ Ko = Kc + (size_t)3 * a.kstride;
-#pragma unroll
-      for (int e = 0; e < E; ++e) {
-        int i0, i1; float s0, s1;
-        k2_kidx<N>(rf::slot_index<P, P::RLAST>(t, e), i0, i1, s0, s1);
-        const float2 kxx = make_float2(__ldg(&Kc[i0]), __ldg(&Kc[i1]));
-        const float2 kyy = make_float2(__ldg(&Ky[i0]), __ldg(&Ky[i1]));
-        const float2 kxy = make_float2(s0 * __ldg(&Ko[i0]), s1 * __ldg(&Ko[i1]));
-        const rf::C2 X = rf::unpack(stash[e * T + t]), Y = v[e];
-        rf::C2 bx;
-        bx.re = __ffma2_rn(kxy, Y.re, __fmul2_rn(kxx, X.re));
-        bx.im = __ffma2_rn(kxy, Y.im, __fmul2_rn(kxx, X.im));
-        stash[e * T + t] = rf::pack(bx);
-        v[e].re = __ffma2_rn(kxy, X.re, __fmul2_rn(kyy, Y.re));
-        v[e].im = __ffma2_rn(kxy, X.im, __fmul2_rn(kyy, Y.im));
-      }
-    } else {
-      const float* __restrict__ Kz = Kc + (size_t)2 * a.kstride;
-#pragma unroll
-      for (int e = 0; e < E; ++e) {
-        int i0, i1; float s0, s1;
-        k2_kidx<N>(rf::slot_index<P, P::RLAST>(t, e), i0, i1, s0, s1);
-        const float2 kz = make_float2(__ldg(&Kz[i0]), __ldg(&Kz[i1]));
-        v[e].re = __fmul2_rn(kz, v[e].re);
-        v[e].im = __fmul2_rn(kz, v[e].im);
-      }
-    }
-#pragma unroll 1
-    for (int c = nc - 1; c >= 0; --c) {
-      if (xy && c == 0) {
-#pragma unroll
-        for (int e = 0; e < E; ++e) v[e] = rf::unpack(stash[e * T + t]);
-      }
-      rf::fft<PI, +1, NT, true>(v, xb, t, gid, a.twy_r);
-      float2* __restrict__ d = col + (size_t)(cbase + c) * a.cstride;
-#pragma unroll
-      for (int e = 0; e < E; ++e) {
-        const int n = rf::slot_index<PI, PI::RLAST>(t, e);
-        const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), __ldg(&a.twoy[n]));
-        d[n] = make_float2(v[e].re.x + u.x, v[e].im.x + u.y);
-      }
-    }
+    C::inv_store(a, cz, v, xb, t, gid);
   }
 }

@@ -281,21 +281,22 @@ __device__ __forceinline__ void exchange(C2* v, void* xbuf, int t, int gid) {
 // until then; after the call xb is only safe to reuse after another group barrier.
 template <class P, int DIR, int NT, bool PLANES = false>
 __device__ __forceinline__ void fft(C2* v, void* xb, int t, int gid, const float2* __restrict__ tw) {
-  float2 w[(P::RA - 1) * (P::E / P::RA)];
-  load_twiddles<P, P::RA>(w, t, tw);
   pass_butterflies<P, P::RA, DIR>(v);
-  apply_twiddles<P, P::RA, DIR>(v, w);
+  {
+    float2 w[(P::RA - 1) * (P::E / P::RA)];
+    load_twiddles<P, P::RA>(w, t, tw);
+    apply_twiddles<P, P::RA, DIR>(v, w);
+  }
+  exchange<P, P::RA, P::RB, P::M1, NT, PLANES>(v, xb, t, gid);
+  pass_butterflies<P, P::RB, DIR>(v);
   if constexpr (P::NPASS == 3) {
-    float2 w2[(P::RB - 1) * (P::E / P::RB)];
-    load_twiddles<P, P::RB>(w2, t, tw + P::TW1);
-    exchange<P, P::RA, P::RB, P::M1, NT, PLANES>(v, xb, t, gid);
-    pass_butterflies<P, P::RB, DIR>(v);
-    apply_twiddles<P, P::RB, DIR>(v, w2);
+    {
+      float2 w[(P::RB - 1) * (P::E / P::RB)];
+      load_twiddles<P, P::RB>(w, t, tw + P::TW1);
+      apply_twiddles<P, P::RB, DIR>(v, w);
+    }
     exchange<P, P::RB, P::RC, P::M2, NT, PLANES>(v, xb, t, gid);
     pass_butterflies<P, P::RC, DIR>(v);
-  } else {
-    exchange<P, P::RA, P::RB, P::M1, NT, PLANES>(v, xb, t, gid);
-    pass_butterflies<P, P::RB, DIR>(v);
   }
 }
 
