@@ -188,10 +188,11 @@ def main():
     if world > 1:
         dist.barrier()
     import paper_1406_7635_b200 as mm
+    from paper_1406_7635_b200 import replicas
     from synth import config_c4
 
     n = args.size
-    cfg = config_c4(n)
+    cfg = config_c4(n, seed_offset=replicas.replica_seed(0, rank))     # one independent replica per rank
     sim = mm.from_config(cfg)
     sim.set_solver(fix_dt=cfg["fix_dt"])
     P = sim.fft_size()[0]
@@ -216,11 +217,7 @@ def main():
     ms = e0.elapsed_time(e1)
     launches = sim.launch_count() - l0
     clocks = sampler.stop() if sampler else None
-    if world > 1:
-        t = torch.tensor([ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * cells * args.steps / (ms * 1e-3)
+    value, ms = replicas.aggregate_throughput(cells * args.steps, ms, device="cuda")   # all ranks' units / max time
 
     # ---- per-kernel CUDA-event timing of the same K steps (separate pass: events bracket every launch)
     sim.profile(True)
@@ -266,12 +263,10 @@ def main():
         host_in, host_out = host_out, host_in
     barrier()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_value, e2e_ms = replicas.aggregate_throughput(cells * ke, 1e3 * e2e_s, device="cuda")
+    e2e_s = 1e-3 * e2e_ms
     nbytes = int(host_in.numel() * 4)
-    e2e = {"value": world * cells * ke / e2e_s, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+    e2e = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
            "steps": ke, "ms_per_step": 1e3 * e2e_s / ke}
 
     if rank == 0:

@@ -87,12 +87,13 @@ def config_c3(grid=(128, 128, 32), ngrains=64):
                 params=p, m0=_random_m(seed, grid), max_err=1e-5, nsteps=100)
 
 
-def config_c4(n=4096):
-    """Large 2D film of the throughput sweep: Permalloy, random m, B_ext 10 mT along x."""
+def config_c4(n=4096, seed_offset=0):
+    """Large 2D film of the throughput sweep: Permalloy, random m, B_ext 10 mT along x.
+    seed_offset selects an independent replica (bench.py --gpus N: one per rank)."""
     grid = (n, n, 1)
     return dict(name="C4-%d" % n, grid=grid, cell=(4e-9, 4e-9, 2e-9), pbc=(0, 0, 0), regions=None,
                 params=Params.uniform(1, Msat=8.6e5, Aex=1.3e-11, alpha=0.01, B_ext=(10e-3, 0, 0)),
-                m0=_random_m(SEED0 + 4, grid), fix_dt=1e-13, nsteps=1000)
+                m0=_random_m(SEED0 + 4 + 1000 * seed_offset, grid), fix_dt=1e-13, nsteps=1000)
 
 
 def config_c5(n=128, pbc=False):

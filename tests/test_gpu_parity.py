@@ -125,6 +125,72 @@ def test_fast2d_path_fields(mm, grid):
     assert np.abs(Bf - Bg).max() <= 2e-5 * np.abs(Bg).max()
 
 
+def test_fast2d_one_region_and_steps(mm):
+    # one region (the bench workload's shape): B_sat is a constant and the region gathers are skipped
+    cfg = config_c4(512)
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    _field_check(sim, ref, (MM_DEMAG, MM_EXCH, MM_ALL))
+    sim.set_solver(fix_dt=cfg["fix_dt"]); ref.set_solver(fix_dt=cfg["fix_dt"])
+    sim.steps(3)
+    for _ in range(3):
+        ref.step()
+    assert np.abs(sim.get_m() - ref.m).max() < 2e-5
+    assert abs(np.linalg.norm(sim.get_m().reshape(3, -1), axis=0) - 1).max() < 1e-6
+
+
+def _direct_sum_at(cells, M, cell):
+    """Eq. 3 (L121-L123) written out for single destination cells of a one-layer film: the sum over
+    ALL source cells with the oracle's tensor K = -N on the (|dx|, |dy|) quadrant."""
+    from oracle.demag_tensor import tensor
+    _, ny, nx = M.shape[1:]
+    K = {k: np.empty((ny, nx)) for k in ("xx", "yy", "zz", "xy")}
+    X = np.arange(nx) * cell[0]
+    for y0 in range(0, ny, 256):                      # in slabs: bounded temporaries
+        Y = np.arange(y0, min(ny, y0 + 256)) * cell[1]
+        XX, YY = np.meshgrid(X, Y, indexing="xy")
+        T = tensor(XX, YY, np.zeros_like(XX), cell)
+        for k in K:
+            K[k][y0:y0 + len(Y)] = -T[k]
+    out = []
+    for (ix, iy) in cells:
+        ax = np.abs(ix - np.arange(nx)); ay = np.abs(iy - np.arange(ny))
+        sx = np.sign(ix - np.arange(nx)); sy = np.sign(iy - np.arange(ny))
+        sel = np.ix_(ay, ax)
+        kxy = K["xy"][sel] * np.outer(sy, sx)         # odd in X and in Y
+        Mx, My, Mz = M[0, 0], M[1, 0], M[2, 0]
+        out.append(((K["xx"][sel] * Mx).sum() + (kxy * My).sum(),
+                    (kxy * Mx).sum() + (K["yy"][sel] * My).sum(),
+                    (K["zz"][sel] * Mz).sum()))
+    return np.array(out)
+
+
+def test_c4_full_size_sampled_cells(mm):
+    # the bench workload and launch configuration (4096 x 4096 x 1, fast 2D kernels): sampled cells
+    # against the plain double sum; corners, edges, tile seams and interior points
+    n = 4096
+    cfg = config_c4(n)
+    sim = mm.from_config(cfg)
+    sim.profile(True)
+    B = sim.b_eff(MM_DEMAG).astype(np.float64).reshape(3, n, n)
+    assert "f2_ycol" in sim.profile_read()
+    sim.profile(False)
+    p = cfg["params"]
+    M = (4e-7 * np.pi * float(np.atleast_1d(p.Msat)[0])) * cfg["m0"].astype(np.float64)
+    cells = [(0, 0), (n - 1, n - 1), (0, n - 1), (2047, 2048), (255, 256), (1000, 3), (4095, 1777), (3071, 513)]
+    Br = _direct_sum_at(cells, M, cfg["cell"])
+    scale = np.abs(B).max()
+    for (ix, iy), br in zip(cells, Br):
+        err = np.abs(B[:, iy, ix] - br).max() / scale
+        assert err <= FIELD_TOL, ((ix, iy), err)
+    # properties that hold at any size: the full field (exchange of random m ~ 10 T dominates) stays
+    # finite everywhere and the step keeps |m| = 1
+    sim.set_solver(fix_dt=cfg["fix_dt"])
+    sim.steps(2)
+    m = sim.get_m().reshape(3, -1)
+    assert np.isfinite(m).all() and abs(np.linalg.norm(m, axis=0) - 1).max() < 1e-6
+
+
 def test_uniform_m_has_no_exchange_field_and_film_limit(mm):
     cfg = _rand_cfg((64, 64, 1), (5e-9, 5e-9, 1e-9), pbc=(32, 32, 0), nreg=1)
     cfg["m0"][:] = 0; cfg["m0"][2] = 1.0
