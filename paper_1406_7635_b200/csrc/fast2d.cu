@@ -10,11 +10,11 @@ namespace {
 // the CTA size NT; a CTA holds G = NT / T FFT groups and therefore 2G rows in the x kernels
 template <int N> struct PlanFor;
 // (NTF: the forward x kernel, whose transposed store wants at least 4 rows = 32-byte pieces)
-template <> struct PlanFor<4096> { using P = rf::Plan<4096, 256, 16, 16, 16>; static constexpr int NT = 256, NTF = 512; };
-template <> struct PlanFor<2048> { using P = rf::Plan<2048, 128, 16, 8, 16>; static constexpr int NT = 256, NTF = 256; };
-template <> struct PlanFor<1024> { using P = rf::Plan<1024, 64, 16, 4, 16>; static constexpr int NT = 256, NTF = 256; };
-template <> struct PlanFor<512> { using P = rf::Plan<512, 32, 16, 2, 16>; static constexpr int NT = 256, NTF = 256; };
-template <> struct PlanFor<256> { using P = rf::Plan<256, 16, 16, 16, 1>; static constexpr int NT = 128, NTF = 128; };
+template <> struct PlanFor<4096> { using P = rf::Plan<4096, 256, 16, 16, 16>; static constexpr int NT = 256, NTF = 512, NTI = 512; };
+template <> struct PlanFor<2048> { using P = rf::Plan<2048, 128, 16, 8, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
+template <> struct PlanFor<1024> { using P = rf::Plan<1024, 64, 16, 4, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
+template <> struct PlanFor<512> { using P = rf::Plan<512, 32, 16, 2, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
+template <> struct PlanFor<256> { using P = rf::Plan<256, 16, 16, 16, 1>; static constexpr int NT = 128, NTF = 128, NTI = 128; };
 
 // forward twiddles of a plan, laid out as fft_reg.cuh reads them
 template <class P>
@@ -71,8 +71,8 @@ int x_attrs(mm_sim* s) {
   using F = PlanFor<N>;
   CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd<typename F::P, F::NTF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    (int)k2_smem<typename F::P, F::NTF>()));
-  CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv<typename F::P, F::NT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   (int)k2_smem<typename F::P, F::NT>()));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv<typename F::P, F::NTI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)k2_smem<typename F::P, F::NTI>()));
   return MM_OK;
 }
 template <int N>
@@ -86,11 +86,11 @@ int y_attrs(mm_sim* s) {
 template <int N>
 void launch_x(mm_sim* s, bool inverse, int role) {
   using F = PlanFor<N>;
-  constexpr int GF = F::NTF / F::P::T, GI = F::NT / F::P::T;
+  constexpr int GF = F::NTF / F::P::T, GI = F::NTI / F::P::T;
   if (!inverse)
     k2_xfwd<typename F::P, F::NTF><<<dim3(s->g.Ny / (2 * GF), 3), F::NTF, k2_smem<typename F::P, F::NTF>(), s->stream>>>(s->f2, role);
   else
-    k2_xinv<typename F::P, F::NT><<<dim3(s->g.Ny / (2 * GI), 3), F::NT, k2_smem<typename F::P, F::NT>(), s->stream>>>(s->f2, role);
+    k2_xinv<typename F::P, F::NTI><<<dim3(s->g.Ny / (2 * GI), 3), F::NTI, k2_smem<typename F::P, F::NTI>(), s->stream>>>(s->f2, role);
 }
 // one launch: XY jobs (one column per FFT group) followed by Z jobs (one column per group)
 template <int N>

@@ -192,6 +192,7 @@ struct K2Col {
   static constexpr int N = P::N, T = P::T, E = P::E;
 
   // column -> lanes (z[n], z[n] w^n) -> forward transforms of the even and the odd bins
+  template <bool PLANES>
   static __device__ __forceinline__ void load_fwd(const Fast2DArgs& a, const float2* __restrict__ s, rf::C2* v, float2* xb,
                                                   int t, int gid) {
 #pragma unroll
@@ -201,12 +202,13 @@ struct K2Col {
       const float2 zw = rf::cmul_tw1<-1>(z, __ldg(&a.twoy[n]));
       v[e] = {make_float2(z.x, zw.x), make_float2(z.y, zw.y)};
     }
-    rf::fft<P, -1, NT, true>(v, xb, t, gid, a.twy);
+    rf::fft<P, -1, NT, PLANES>(v, xb, t, gid, a.twy);
   }
   // inverse transforms -> first N samples: even part + conj(w)^n odd part -> column (in place)
+  template <bool PLANES>
   static __device__ __forceinline__ void inv_store(const Fast2DArgs& a, float2* __restrict__ d, rf::C2* v, float2* xb, int t,
                                                    int gid) {
-    rf::fft<PI, +1, NT, true>(v, xb, t, gid, a.twy_r);
+    rf::fft<PI, +1, NT, PLANES>(v, xb, t, gid, a.twy_r);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       const int n = rf::slot_index<PI, PI::RLAST>(t, e);
@@ -238,10 +240,10 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_ycol(Fast2DArgs a, int nxy) {
   }
   rf::C2 v[E];
   if (xy) {
-    C::load_fwd(a, col, v, xb, t, gid);
+    C::template load_fwd<true>(a, col, v, xb, t, gid);
 #pragma unroll
     for (int e = 0; e < E; ++e) stash[e * T + t] = rf::pack(v[e]);     // own slots: no barrier
-    C::load_fwd(a, col + a.cstride, v, xb, t, gid);
+    C::template load_fwd<true>(a, col + a.cstride, v, xb, t, gid);
     // B~_x = K_xx M~_x + K_xy M~_y,  B~_y = K_xy M~_x + K_yy M~_y   (Eq. 3; K real, L145)
     const float* __restrict__ Ky = Kc + a.kstride;
     const float* __restrict__ Ko = Kc + (size_t)3 * a.kstride;
@@ -260,13 +262,14 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_ycol(Fast2DArgs a, int nxy) {
       v[e].re = __ffma2_rn(kxy, X.re, __fmul2_rn(kyy, Y.re));
       v[e].im = __ffma2_rn(kxy, X.im, __fmul2_rn(kyy, Y.im));
     }
-    C::inv_store(a, col + a.cstride, v, xb, t, gid);
+    C::template inv_store<true>(a, col + a.cstride, v, xb, t, gid);
 #pragma unroll
     for (int e = 0; e < E; ++e) v[e] = rf::unpack(stash[e * T + t]);
-    C::inv_store(a, col, v, xb, t, gid);
+    C::template inv_store<true>(a, col, v, xb, t, gid);
   } else {
     float2* __restrict__ cz = col + 2 * a.cstride;
-    C::load_fwd(a, cz, v, xb, t, gid);
+    float2* xz = reinterpret_cast<float2*>(mine);      // no stash needed: 16-byte units, half the barriers
+    C::template load_fwd<false>(a, cz, v, xz, t, gid);
     const float* __restrict__ Kz = Kc + (size_t)2 * a.kstride;
 #pragma unroll
     for (int e = 0; e < E; ++e) {
@@ -276,6 +279,6 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_ycol(Fast2DArgs a, int nxy) {
       v[e].re = __fmul2_rn(kz, v[e].re);
       v[e].im = __fmul2_rn(kz, v[e].im);
     }
-    C::inv_store(a, cz, v, xb, t, gid);
+    C::template inv_store<false>(a, cz, v, xz, t, gid);
   }
 }
