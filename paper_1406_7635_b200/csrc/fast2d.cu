@@ -10,7 +10,7 @@ namespace {
 // the CTA size NT; a CTA holds G = NT / T FFT groups and therefore 2G rows in the x kernels
 template <int N> struct PlanFor;
 // (NTF: the forward x kernel, whose transposed store wants at least 4 rows = 32-byte pieces)
-template <> struct PlanFor<4096> { using P = rf::Plan<4096, 256, 16, 16, 16>; static constexpr int NT = 256, NTF = 512, NTI = 512; };
+template <> struct PlanFor<4096> { using P = rf::Plan<4096, 256, 16, 16, 16>; static constexpr int NT = 256, NTF = 512, NTI = 256; };
 template <> struct PlanFor<2048> { using P = rf::Plan<2048, 128, 16, 8, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
 template <> struct PlanFor<1024> { using P = rf::Plan<1024, 64, 16, 4, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
 template <> struct PlanFor<512> { using P = rf::Plan<512, 32, 16, 2, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
@@ -32,6 +32,29 @@ std::vector<float2> plan_table() {
       for (int bf = 0; bf < N / P::RB; ++bf)
         put((size_t)P::TW1 + (size_t)(s - 1) * (N / P::RB) + bf, (double)((long long)s * P::RA * (bf % P::M2) % N) / N);
   return tw;
+}
+
+// 3-D TMA view of spec: floats along y innermost (2 per bin), then kx, then component; one box =
+// {rows * 2 floats, K2_KB bins, 1}. Returns false if the driver entry point is unavailable.
+bool make_spec_map(mm_sim* s, int rows, CUtensorMap* out) {
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+      qres != cudaDriverEntryPointSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  const Fast2DArgs& a = s->f2;
+  const cuuint64_t dims[3] = {(cuuint64_t)2 * a.Ny, (cuuint64_t)a.Cx, 3};
+  const cuuint64_t strides[2] = {(cuuint64_t)a.Ny * sizeof(float2), (cuuint64_t)a.cstride * sizeof(float2)};
+  const cuuint32_t box[3] = {(cuuint32_t)(2 * rows), (cuuint32_t)K2_KB, 1};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  return ((EncodeFn)fn)(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)a.spec, dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 int upload(mm_sim* s, const std::vector<float2>& h, float2** out) {
@@ -73,6 +96,8 @@ int x_attrs(mm_sim* s) {
                                    (int)k2_smem<typename F::P, F::NTF>()));
   CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv<typename F::P, F::NTI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    (int)k2_smem<typename F::P, F::NTI>()));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv_tma<typename F::P, F::NTI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)k2_tma_smem<typename F::P, F::NTI>()));
   return MM_OK;
 }
 template <int N>
@@ -89,6 +114,8 @@ void launch_x(mm_sim* s, bool inverse, int role) {
   constexpr int GF = F::NTF / F::P::T, GI = F::NTI / F::P::T;
   if (!inverse)
     k2_xfwd<typename F::P, F::NTF><<<dim3(s->g.Ny / (2 * GF), 3), F::NTF, k2_smem<typename F::P, F::NTF>(), s->stream>>>(s->f2, role);
+  else if (s->f2_tma)
+    k2_xinv_tma<typename F::P, F::NTI><<<dim3(s->g.Ny / (2 * GI), 3), F::NTI, k2_tma_smem<typename F::P, F::NTI>(), s->stream>>>(s->f2, role, s->f2_map_inv);
   else
     k2_xinv<typename F::P, F::NTI><<<dim3(s->g.Ny / (2 * GI), 3), F::NTI, k2_smem<typename F::P, F::NTI>(), s->stream>>>(s->f2, role);
 }
@@ -101,6 +128,7 @@ void launch_y(mm_sim* s) {
   k2_ycol<typename F::P, F::NT><<<nxy + nz, F::NT, k2_y_smem<typename F::P, F::NT>(), s->stream>>>(s->f2, nxy);
 }
 
+template <int N> constexpr int rows_inv_of() { return 2 * (PlanFor<N>::NTI / PlanFor<N>::P::T); }
 template <int N> constexpr int rows_of() { return 2 * (PlanFor<N>::NTF / PlanFor<N>::P::T); }   // NTF >= NT
 int rows_per_cta(int N) {
   switch (N) {
@@ -151,6 +179,11 @@ int mm_fast2d_init(mm_sim* s) {
   F2_SWITCH(g.Ny, YA)
 #undef XA
 #undef YA
+  int rows_inv = 0;
+#define RI(N) rows_inv = rows_inv_of<N>()
+  F2_SWITCH(g.Nx, RI)
+#undef RI
+  s->f2_tma = make_spec_map(s, rows_inv, &s->f2_map_inv);
   return MM_OK;
 }
 

@@ -19,6 +19,7 @@
 #include "common.cuh"
 #include "fft_reg.cuh"
 #include "demag_conv_args.cuh"
+#include "tma_util.cuh"
 
 // pitch (float4 units) between the exchange buffers of consecutive FFT groups: XB plus a skew that
 // spreads the G groups over the 8 16-byte bank groups when one quarter-warp touches several buffers
@@ -280,5 +281,83 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_ycol(Fast2DArgs a, int nxy) {
       v[e].im = __fmul2_rn(kz, v[e].im);
     }
     C::template inv_store<false>(a, cz, v, xz, t, gid);
+  }
+}
+
+// ---------------------------------------------------------------------------------- K_C with TMA
+// Same computation as k2_xinv, but the transposed 16G-byte pieces of the CTA's 2G rows arrive as
+// TMA boxes {2G rows, KB bins} of a 3-D tensor map over spec (y innermost, then kx, then component):
+// a ring of NBUF boxes is in flight while the threads turn the previous box into Z = A + iB and
+// its mirror, so the gather costs no LSU global-load wavefronts and no registers.
+constexpr int K2_KB = 256;      // kx bins per box
+template <int G> struct K2Ring { static constexpr int NBUF = G >= 4 ? 2 : 8 / G; };   // boxes in flight (32-64 KB)
+
+template <class P, int NT>
+constexpr size_t k2_tma_smem() {
+  return k2_smem<P, NT>() + (size_t)K2Ring<K2Shape<P, NT>::G>::NBUF * K2_KB * K2Shape<P, NT>::G * sizeof(float4) + 128;
+}
+
+template <class P, int NT>
+__global__ void __launch_bounds__(NT, 512 / NT) k2_xinv_tma(Fast2DArgs a, int dst_role, const __grid_constant__ CUtensorMap map) {
+  if (a.st->skip) return;
+  using PI = typename P::Reversed;
+  constexpr int N = P::N, T = P::T, E = P::E, G = NT / T, GP = K2Shape<P, NT>::GP;
+  constexpr int NB = (N + 1 + K2_KB - 1) / K2_KB;            // boxes covering kx = 0 .. N
+  constexpr int K2_NBUF = K2Ring<G>::NBUF;
+  constexpr uint32_t BOX_BYTES = K2_KB * G * sizeof(float4);
+  extern __shared__ __align__(128) float4 smem4[];
+  __shared__ __align__(8) uint64_t full[K2_NBUF];
+  float4* tiles = smem4 + (size_t)G * GP + ((128 - ((size_t)G * GP * 16) % 128) % 128) / 16;   // 128-byte aligned
+  const int tid = threadIdx.x, gid = tid / T, t = tid % T;
+  float4* xb = smem4 + (size_t)gid * GP;
+  const int c = blockIdx.y, r0 = blockIdx.x * 2 * G;
+  float* __restrict__ dst = a.st->ptr[dst_role] + (size_t)c * a.ncell;
+  if (tid == 0) {
+#pragma unroll
+    for (int b = 0; b < K2_NBUF; ++b) tma::mbar_init(&full[b], 1);
+    tma::fence_barrier_init();
+    tma::fence_proxy_async();
+#pragma unroll
+    for (int b = 0; b < K2_NBUF && b < NB; ++b) {
+      tma::mbar_expect_tx(&full[b], BOX_BYTES);
+      tma::load_3d(tiles + (size_t)b * K2_KB * G, &map, 2 * r0, b * K2_KB, c, &full[b]);
+    }
+  }
+  __syncthreads();
+#pragma unroll 1
+  for (int j = 0; j < NB; ++j) {
+    const int b = j % K2_NBUF;
+    tma::mbar_wait(&full[b], (j / K2_NBUF) & 1);
+    const float4* tile = tiles + (size_t)b * K2_KB * G;
+    for (int i = tid; i < K2_KB * G; i += NT) {
+      const int p = i % G, kx = j * K2_KB + i / G;
+      if (kx > N) continue;
+      const float4 e = tile[i];
+      float2* st2 = reinterpret_cast<float2*>(smem4 + (size_t)p * GP);
+      const int k = kx >> 1, h = kx & 1;
+      const float2 z = make_float2(e.x - e.w, e.y + e.z), zm = make_float2(e.x + e.w, e.z - e.y);
+      st2[2 * k + h] = z;
+      if (h) st2[2 * (N - 1 - k) + 1] = zm;
+      else if (k > 0 && k < N / 2) st2[2 * (N - k)] = zm;
+    }
+    __syncthreads();                       // everyone is done with this box: refill it
+    if (tid == 0 && j + K2_NBUF < NB) {
+      tma::mbar_expect_tx(&full[b], BOX_BYTES);
+      tma::load_3d(tiles + (size_t)b * K2_KB * G, &map, 2 * r0, (j + K2_NBUF) * K2_KB, c, &full[b]);
+    }
+  }
+  {
+    rf::C2 v[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) v[e] = stage_unpack(xb[rf::slot_index<PI, PI::RA>(t, e)]);
+    rf::fft<PI, +1, NT>(v, xb, t, gid, a.twx_r);
+    const size_t rowA = (size_t)(r0 + 2 * gid) * N;
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+      const int n = rf::slot_index<PI, PI::RLAST>(t, e);
+      const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), __ldg(&a.twox[n]));
+      dst[rowA + n] = v[e].re.x + u.x;
+      dst[rowA + N + n] = v[e].im.x + u.y;
+    }
   }
 }

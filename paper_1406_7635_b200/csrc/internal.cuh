@@ -1,5 +1,6 @@
 // internal.cuh - handle layout and host helpers shared by the translation units of libmm_b200.so
 #pragma once
+#include <cuda.h>
 #include <string>
 #include <utility>
 #include <vector>
@@ -37,6 +38,8 @@ struct mm_sim {
   ConvArgs conv;
   float* Kt = nullptr;         // kernel spectrum in the fast 2D layout
   Fast2DArgs f2;
+  CUtensorMap f2_map_inv, f2_map_fwd;   // TMA views of spec for the x kernels (boxes of 2G rows x 256 bins)
+  bool f2_tma = false;         // tensor maps valid: the x kernels move their transposed pieces with TMA
   bool fast2d = false;         // fast 2D path available for this box
   bool force_generic = false;  // mm_set_option(MM_OPT_GENERIC_FFT)
   // host state
