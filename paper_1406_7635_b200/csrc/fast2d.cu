@@ -94,6 +94,8 @@ int x_attrs(mm_sim* s) {
   using F = PlanFor<N>;
   CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd<typename F::P, F::NTF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    (int)k2_smem<typename F::P, F::NTF>()));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd_tma<typename F::P, F::NTF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)k2_tma_store_smem<typename F::P, F::NTF>()));
   CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv<typename F::P, F::NTI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    (int)k2_smem<typename F::P, F::NTI>()));
   CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv_tma<typename F::P, F::NTI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -112,7 +114,9 @@ template <int N>
 void launch_x(mm_sim* s, bool inverse, int role) {
   using F = PlanFor<N>;
   constexpr int GF = F::NTF / F::P::T, GI = F::NTI / F::P::T;
-  if (!inverse)
+  if (!inverse && s->f2_tma)
+    k2_xfwd_tma<typename F::P, F::NTF><<<dim3(s->g.Ny / (2 * GF), 3), F::NTF, k2_tma_store_smem<typename F::P, F::NTF>(), s->stream>>>(s->f2, role, s->f2_map_fwd);
+  else if (!inverse)
     k2_xfwd<typename F::P, F::NTF><<<dim3(s->g.Ny / (2 * GF), 3), F::NTF, k2_smem<typename F::P, F::NTF>(), s->stream>>>(s->f2, role);
   else if (s->f2_tma)
     k2_xinv_tma<typename F::P, F::NTI><<<dim3(s->g.Ny / (2 * GI), 3), F::NTI, k2_tma_smem<typename F::P, F::NTI>(), s->stream>>>(s->f2, role, s->f2_map_inv);
@@ -183,7 +187,7 @@ int mm_fast2d_init(mm_sim* s) {
 #define RI(N) rows_inv = rows_inv_of<N>()
   F2_SWITCH(g.Nx, RI)
 #undef RI
-  s->f2_tma = make_spec_map(s, rows_inv, &s->f2_map_inv);
+  s->f2_tma = make_spec_map(s, rows_inv, &s->f2_map_inv) && make_spec_map(s, rows_per_cta(g.Nx), &s->f2_map_fwd);
   return MM_OK;
 }
 

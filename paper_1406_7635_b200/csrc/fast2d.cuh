@@ -361,3 +361,75 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xinv_tma(Fast2DArgs a, int ds
     }
   }
 }
+
+// ---------------------------------------------------------------------------------- K_A with TMA
+// Same computation as k2_xfwd; the separated spectra of the CTA's 2G rows leave as TMA boxes
+// {2G rows, KB bins}: the threads fill a ring of tiles in shared memory, one thread issues the tensor
+// stores, so the transposed 16G-byte pieces cost no LSU store wavefronts and the CTA does not wait
+// for them to drain.
+template <int G> struct K2StoreRing { static constexpr int NBUF = G >= 4 ? 3 : 4; };
+template <class P, int NT>
+constexpr size_t k2_tma_store_smem() {
+  return k2_smem<P, NT>() + (size_t)K2StoreRing<K2Shape<P, NT>::G>::NBUF * K2_KB * K2Shape<P, NT>::G * sizeof(float4) + 128;
+}
+
+template <class P, int NT>
+__global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd_tma(Fast2DArgs a, int src_role, const __grid_constant__ CUtensorMap map) {
+  if (a.st->skip) return;
+  constexpr int N = P::N, T = P::T, E = P::E, G = NT / T, GP = K2Shape<P, NT>::GP;
+  constexpr int NB = (N + 1 + K2_KB - 1) / K2_KB, NBUF = K2StoreRing<G>::NBUF;
+  extern __shared__ __align__(128) float4 smem4[];
+  __shared__ float bsat_s[MM_MAX_REGIONS];
+  float4* tiles = smem4 + (size_t)G * GP + ((128 - ((size_t)G * GP * 16) % 128) % 128) / 16;   // 128-byte aligned
+  const int tid = threadIdx.x, gid = tid / T, t = tid % T;
+  float4* xb = smem4 + (size_t)gid * GP;
+  const int c = blockIdx.y, r0 = blockIdx.x * 2 * G;
+  const float* __restrict__ src = a.st->ptr[src_role] + (size_t)c * a.ncell;
+  const uint8_t* __restrict__ reg = a.regions;
+  const bool uniform = a.luts->nregions == 1;       // one region: B_sat is a constant
+  const float b0 = a.luts->Bsat[0];
+  if (!uniform) {
+    for (int i = tid; i < MM_MAX_REGIONS; i += NT) bsat_s[i] = a.luts->Bsat[i];
+    __syncthreads();
+  }
+  {
+    const size_t rowA = (size_t)(r0 + 2 * gid) * N;
+    rf::C2 v[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+      const int n = rf::slot_index<P, P::RA>(t, e);
+      const size_t iA = rowA + n, iB = iA + N;
+      const float sa = uniform ? b0 : bsat_s[reg[iA]], sb = uniform ? b0 : bsat_s[reg[iB]];
+      const float2 z = make_float2(__ldg(src + iA) * sa, __ldg(src + iB) * sb);            // M = B_sat m (L121)
+      const float2 zw = rf::cmul_tw1<-1>(z, __ldg(&a.twox[n]));
+      v[e] = {make_float2(z.x, zw.x), make_float2(z.y, zw.y)};
+    }
+    rf::fft<P, -1, NT>(v, xb, t, gid, a.twx);
+    rf::group_sync<T, NT>(gid);
+#pragma unroll
+    for (int e = 0; e < E; ++e) xb[rf::slot_index<P, P::RLAST>(t, e)] = stage_pack(v[e]);
+  }
+  __syncthreads();
+  // separate the two real rows of every pair (lane 0 of unit k = bin kx = 2k, lane 1 = bin 2k + 1)
+  // into tiles [bin][pair] and hand them to TMA; stored bins kx = 0 .. N (rows beyond are clipped)
+#pragma unroll 1
+  for (int j = 0; j < NB; ++j) {
+    float4* tile = tiles + (size_t)(j % NBUF) * K2_KB * G;
+    for (int i = tid; i < K2_KB * G; i += NT) {
+      const int p = i % G, kx = j * K2_KB + i / G;
+      if (kx > N) continue;
+      const float2* st2 = reinterpret_cast<const float2*>(smem4 + (size_t)p * GP);
+      const int k = kx >> 1, h = kx & 1;
+      const int km = h ? N - 1 - k : (N - k) & (N - 1);
+      tile[i] = separate(st2[2 * k + h], st2[2 * km + h]);
+    }
+    tma::fence_proxy_async();
+    if (tid == 0) tma::store_wait_read<NBUF - 2>();     // the tile of iteration j + 1 is free again
+    __syncthreads();
+    if (tid == 0) {
+      tma::store_3d(&map, 2 * r0, j * K2_KB, c, tile);
+      tma::store_commit();
+    }
+  }
+  if (tid == 0) tma::store_wait_read<0>();               // shared memory must outlive the reads
+}
