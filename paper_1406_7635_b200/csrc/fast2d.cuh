@@ -25,6 +25,8 @@
 // spreads the G groups over the 8 16-byte bank groups when one quarter-warp touches several buffers
 template <class P, int NT>
 struct K2Shape {
+  static_assert(P::E == 16 && P::RA == 16 && P::Reversed::RLAST == 16 && P::T * 16 == P::N,
+                "the kernels assume 16 points per thread at stride N/16 on input and output");
   static constexpr int G = NT / P::T;
   static constexpr int GP = P::XB + (G >= 8 ? 1 : 8 / G);
 };
@@ -61,13 +63,14 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd(Fast2DArgs a, int src_ro
   {
     const size_t rowA = (size_t)(r0 + 2 * gid) * N;
     rf::C2 v[E];
+    const float2 wt = __ldg(&a.twox[t]);      // w_2N^t; the other points follow from constants
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       const int n = rf::slot_index<P, P::RA>(t, e);
       const size_t iA = rowA + n, iB = iA + N;
       const float sa = uniform ? b0 : bsat_s[reg[iA]], sb = uniform ? b0 : bsat_s[reg[iB]];
       const float2 z = make_float2(src[iA] * sa, src[iB] * sb);            // M = B_sat m (L121)
-      const float2 zw = rf::cmul_tw1<-1>(z, __ldg(&a.twox[n]));
+      const float2 zw = rf::cmul_tw1<-1>(z, rf::half_twiddle(wt, e));
       v[e] = {make_float2(z.x, zw.x), make_float2(z.y, zw.y)};
     }
     rf::fft<P, -1, NT>(v, xb, t, gid, a.twx);
@@ -150,12 +153,13 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xinv(Fast2DArgs a, int dst_ro
     rf::C2 v[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) v[e] = stage_unpack(xb[rf::slot_index<PI, PI::RA>(t, e)]);
+    const float2 wt = __ldg(&a.twox[t]);      // w_2N^t; the other points follow from constants
     rf::fft<PI, +1, NT>(v, xb, t, gid, a.twx_r);
     const size_t rowA = (size_t)(r0 + 2 * gid) * N;
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       const int n = rf::slot_index<PI, PI::RLAST>(t, e);
-      const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), __ldg(&a.twox[n]));
+      const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), rf::half_twiddle(wt, e));
       dst[rowA + n] = v[e].re.x + u.x;
       dst[rowA + N + n] = v[e].im.x + u.y;
     }
@@ -196,11 +200,12 @@ struct K2Col {
   template <bool PLANES>
   static __device__ __forceinline__ void load_fwd(const Fast2DArgs& a, const float2* __restrict__ s, rf::C2* v, float2* xb,
                                                   int t, int gid) {
+    const float2 wt = __ldg(&a.twoy[t]);      // w_2N^t; the other points follow from constants
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       const int n = rf::slot_index<P, P::RA>(t, e);
       const float2 z = s[n];
-      const float2 zw = rf::cmul_tw1<-1>(z, __ldg(&a.twoy[n]));
+      const float2 zw = rf::cmul_tw1<-1>(z, rf::half_twiddle(wt, e));
       v[e] = {make_float2(z.x, zw.x), make_float2(z.y, zw.y)};
     }
     rf::fft<P, -1, NT, PLANES>(v, xb, t, gid, a.twy);
@@ -209,11 +214,12 @@ struct K2Col {
   template <bool PLANES>
   static __device__ __forceinline__ void inv_store(const Fast2DArgs& a, float2* __restrict__ d, rf::C2* v, float2* xb, int t,
                                                    int gid) {
+    const float2 wt = __ldg(&a.twoy[t]);      // w_2N^t; the other points follow from constants
     rf::fft<PI, +1, NT, PLANES>(v, xb, t, gid, a.twy_r);
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       const int n = rf::slot_index<PI, PI::RLAST>(t, e);
-      const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), __ldg(&a.twoy[n]));
+      const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), rf::half_twiddle(wt, e));
       d[n] = make_float2(v[e].re.x + u.x, v[e].im.x + u.y);
     }
   }
@@ -350,12 +356,13 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xinv_tma(Fast2DArgs a, int ds
     rf::C2 v[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) v[e] = stage_unpack(xb[rf::slot_index<PI, PI::RA>(t, e)]);
+    const float2 wt = __ldg(&a.twox[t]);      // w_2N^t; the other points follow from constants
     rf::fft<PI, +1, NT>(v, xb, t, gid, a.twx_r);
     const size_t rowA = (size_t)(r0 + 2 * gid) * N;
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       const int n = rf::slot_index<PI, PI::RLAST>(t, e);
-      const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), __ldg(&a.twox[n]));
+      const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), rf::half_twiddle(wt, e));
       dst[rowA + n] = v[e].re.x + u.x;
       dst[rowA + N + n] = v[e].im.x + u.y;
     }
@@ -395,13 +402,14 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd_tma(Fast2DArgs a, int sr
   {
     const size_t rowA = (size_t)(r0 + 2 * gid) * N;
     rf::C2 v[E];
+    const float2 wt = __ldg(&a.twox[t]);      // w_2N^t; the other points follow from constants
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       const int n = rf::slot_index<P, P::RA>(t, e);
       const size_t iA = rowA + n, iB = iA + N;
       const float sa = uniform ? b0 : bsat_s[reg[iA]], sb = uniform ? b0 : bsat_s[reg[iB]];
       const float2 z = make_float2(__ldg(src + iA) * sa, __ldg(src + iB) * sb);            // M = B_sat m (L121)
-      const float2 zw = rf::cmul_tw1<-1>(z, __ldg(&a.twox[n]));
+      const float2 zw = rf::cmul_tw1<-1>(z, rf::half_twiddle(wt, e));
       v[e] = {make_float2(z.x, zw.x), make_float2(z.y, zw.y)};
     }
     rf::fft<P, -1, NT>(v, xb, t, gid, a.twx);

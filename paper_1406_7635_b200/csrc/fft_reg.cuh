@@ -202,14 +202,48 @@ __device__ __forceinline__ void pass_butterflies(C2* v) {
   for (int b = 0; b < P::E / R; ++b) Bfly<R, DIR>::run(v + b * R);
 }
 
-// twiddles of the pass that follows a radix-R butterfly: fetched early (before the butterflies or
-// before the preceding exchange) so that their latency hides behind that work
+// Twiddles of the pass that follows a radix-R butterfly: w^s, s = 1 .. R-1, of the per-thread base
+// w = table entry of s = 1. Only the base is loaded; the powers are formed in registers by a product
+// tree of depth <= 4 (about 4 ulp), so the butterfly phases of a warp do not queue behind the
+// shared-memory traffic of the other warps in the LSU pipe.
+__device__ __forceinline__ float2 csqr(float2 a) { return make_float2(a.x * a.x - a.y * a.y, 2.f * a.x * a.y); }
+__device__ __forceinline__ float2 cmul1(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+
+// exp(-i pi e / 16), e = 0 .. 15: with 16 points per thread at stride N/16 the half-bin twiddle
+// w_2N^n of point n = t + (N/16) e is w_2N^t times this constant, so one table load per thread serves
+// all 16 points
+__device__ __forceinline__ float2 half_twiddle(float2 wt, int e) {
+  constexpr float C[16] = {1.f, 0.98078528040323043f, 0.92387953251128674f, 0.83146961230254524f, 0.70710678118654752f,
+                           0.55557023301960218f, 0.38268343236508977f, 0.19509032201612825f, 0.f, -0.19509032201612825f,
+                           -0.38268343236508977f, -0.55557023301960218f, -0.70710678118654752f, -0.83146961230254524f,
+                           -0.92387953251128674f, -0.98078528040323043f};
+  constexpr float S[16] = {0.f, 0.19509032201612825f, 0.38268343236508977f, 0.55557023301960218f, 0.70710678118654752f,
+                           0.83146961230254524f, 0.92387953251128674f, 0.98078528040323043f, 1.f, 0.98078528040323043f,
+                           0.92387953251128674f, 0.83146961230254524f, 0.70710678118654752f, 0.55557023301960218f,
+                           0.38268343236508977f, 0.19509032201612825f};
+  if (e == 0) return wt;
+  if (e == 8) return make_float2(wt.y, -wt.x);                 // times -i
+  return make_float2(wt.x * C[e] + wt.y * S[e], wt.y * C[e] - wt.x * S[e]);   // wt * (C - i S)
+}
+
 template <class P, int R>
 __device__ __forceinline__ void load_twiddles(float2* w, int t, const float2* __restrict__ tw) {
 #pragma unroll
-  for (int b = 0; b < P::E / R; ++b)
+  for (int b = 0; b < P::E / R; ++b) {
+    float2* p = w + b * (R - 1);                      // p[s - 1] = base^s
+    p[0] = __ldg(&tw[t + P::T * b]);
+    if (R > 2) { p[1] = csqr(p[0]); p[2] = cmul1(p[1], p[0]); }
+    if (R > 4) {
+      p[3] = csqr(p[1]);
 #pragma unroll
-    for (int s = 1; s < R; ++s) w[b * (R - 1) + s - 1] = __ldg(&tw[(s - 1) * (P::N / R) + t + P::T * b]);
+      for (int s = 1; s <= 3; ++s) p[3 + s] = cmul1(p[3], p[s - 1]);
+    }
+    if (R > 8) {
+      p[7] = csqr(p[3]);
+#pragma unroll
+      for (int s = 1; s <= 7; ++s) p[7 + s] = cmul1(p[7], p[s - 1]);
+    }
+  }
 }
 
 template <class P, int R, int DIR>
