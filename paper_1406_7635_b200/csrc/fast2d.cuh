@@ -33,6 +33,9 @@ struct K2Shape {
 template <class P, int NT>
 constexpr size_t k2_smem() { return sizeof(float4) * (size_t)K2Shape<P, NT>::G * K2Shape<P, NT>::GP; }
 
+__device__ __forceinline__ void k2_prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+__device__ __forceinline__ void k2_prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
 // stage unit = (z0.re, z0.im, z1.re, z1.im): each lane's complex number is one 8-byte half
 __device__ __forceinline__ float4 stage_pack(rf::C2 a) { return make_float4(a.re.x, a.im.x, a.re.y, a.im.y); }
 __device__ __forceinline__ rf::C2 stage_unpack(float4 q) { return {make_float2(q.x, q.z), make_float2(q.y, q.w)}; }
@@ -184,7 +187,6 @@ struct K2YShape {
 template <class P, int NT>
 constexpr size_t k2_y_smem() { return (size_t)(NT / P::T) * K2YShape<P>::GROUP_BYTES; }
 
-__device__ __forceinline__ void k2_prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 // Every FFT group works on its own: an XY job is one column of the x and y components (coupled by
 // the kernel product), a Z job one column of the z component. All code is straight-line (a rolled
@@ -245,11 +247,25 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_ycol(Fast2DArgs a, int nxy) {
     if (xy) { k2_prefetch_l2(Kc + i); k2_prefetch_l2(Kc + a.kstride + i); k2_prefetch_l2(Kc + 3 * a.kstride + i); }
     else k2_prefetch_l2(Kc + 2 * a.kstride + i);
   }
+  {
+    // columns that will be wanted soon, on their way from DRAM to L2: this job's second component and
+    // the first component of the job that follows on this SM (CTAs are dispatched in order, two per SM)
+    const int ahead = kx + 2 * 148 * G;
+    const float2* nxt = a.spec + (size_t)(xy ? 0 : 2) * a.cstride + (size_t)ahead * a.Ny;
+    for (int i = t * 16; i < N; i += T * 16) {
+      if (xy) k2_prefetch_l2(col + a.cstride + i);
+      if (ahead < a.Cx) k2_prefetch_l2(nxt + i);
+    }
+  }
   rf::C2 v[E];
   if (xy) {
     C::template load_fwd<true>(a, col, v, xb, t, gid);
 #pragma unroll
     for (int e = 0; e < E; ++e) stash[e * T + t] = rf::pack(v[e]);     // own slots: no barrier
+    // the kernel rows are needed right after this transform: pull them from L2 into L1 now
+    for (int i = t * 32; i < N + 1; i += T * 32) {
+      k2_prefetch_l1(Kc + i); k2_prefetch_l1(Kc + a.kstride + i); k2_prefetch_l1(Kc + 3 * a.kstride + i);
+    }
     C::template load_fwd<true>(a, col + a.cstride, v, xb, t, gid);
     // B~_x = K_xx M~_x + K_xy M~_y,  B~_y = K_xy M~_x + K_yy M~_y   (Eq. 3; K real, L145)
     const float* __restrict__ Ky = Kc + a.kstride;
@@ -398,6 +414,15 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd_tma(Fast2DArgs a, int sr
   if (!uniform) {
     for (int i = tid; i < MM_MAX_REGIONS; i += NT) bsat_s[i] = a.luts->Bsat[i];
     __syncthreads();
+  }
+  {
+    // rows of the CTA that follows on this SM (dispatch is in order, 512 / NT CTAs per SM): DRAM -> L2
+    int nb = (int)blockIdx.x + 148 * (512 / NT), nc = c;
+    if (nb >= (int)gridDim.x) { nb -= gridDim.x; ++nc; }
+    if (nc < 3 && nb < (int)gridDim.x) {
+      const float* nxt = a.st->ptr[src_role] + (size_t)nc * a.ncell + (size_t)nb * 2 * G * N;
+      for (int i = tid * 32; i < 2 * G * N; i += NT * 32) k2_prefetch_l2(nxt + i);
+    }
   }
   {
     const size_t rowA = (size_t)(r0 + 2 * gid) * N;
