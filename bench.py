@@ -159,6 +159,8 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--size", type=int, default=4096)
+    ap.add_argument("--workload", default="c4", choices=["c4", "c5", "c5pbc"],
+                    help="c4: size x size x 1 film (default, the metric's workload); c5 / c5pbc: size^3 cube, open / PBC(4,4,0)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-size", type=int, default=256)
     ap.add_argument("--cpu-steps", type=int, default=12)
@@ -192,11 +194,19 @@ def main():
     from synth import config_c4
 
     n = args.size
-    cfg = config_c4(n, seed_offset=replicas.replica_seed(0, rank))     # one independent replica per rank
+    if args.workload == "c4":
+        cfg = config_c4(n, seed_offset=replicas.replica_seed(0, rank))     # one independent replica per rank
+        cells, step_bytes = n * n, STEP_BYTES_PER_CELL
+        wname = "C4 film %dx%dx1, 4x4x2 nm, Permalloy, random m, B_ext 10 mT, fix_dt 1e-13 s" % (n, n)
+    else:
+        from synth import config_c5
+        cfg = config_c5(n, pbc=args.workload == "c5pbc")
+        cells = n ** 3
+        step_bytes = 6 * 140.0 + 372.0 if args.workload == "c5pbc" else 2472.0
+        wname = "C5 cube %d^3, 2 nm, Kc1 -5e3, random m, %s, fix_dt 1e-13 s" % (n, "PBC (4,4,0)" if args.workload == "c5pbc" else "open")
     sim = mm.from_config(cfg)
     sim.set_solver(fix_dt=cfg["fix_dt"])
     P = sim.fft_size()[0]
-    cells = n * n
 
     def barrier():
         if world > 1:
@@ -229,10 +239,10 @@ def main():
     roofline, kernels = None, {}
     tot_ms = sum(v[0] for v in prof.values()) or 1.0
     for name, (kms, cnt) in prof.items():
-        b = kernel_bytes(name, n, P)
+        b = kernel_bytes(name, n, P) if args.workload == "c4" else 0.0     # byte table is for the 2D path
         kernels[name] = {"ms_per_launch": kms / cnt, "launches_per_step": cnt / args.steps, "share": kms / tot_ms,
                          "GBps": (b / (kms / cnt * 1e-3) / 1e9) if b else None}
-    if prof:
+    if prof and args.workload == "c4":
         top = max(prof, key=lambda k: prof[k][0])
         b = kernel_bytes(top, n, P)
         ach = b / (prof[top][0] / prof[top][1] * 1e-3) / 1e9
@@ -245,9 +255,9 @@ def main():
         roofline = {"bound": "hbm", "kernel": top, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                     "traffic": traffic, "peak_source": peak_src, "algorithmic_bytes_per_launch": b,
                     "share_of_step": prof[top][0] / tot_ms}
-    step_gbs = STEP_BYTES_PER_CELL * cells * args.steps / (ms * 1e-3) / 1e9
+    step_gbs = step_bytes * cells * args.steps / (ms * 1e-3) / 1e9
     step_roofline = {"achieved": step_gbs, "peak": peak, "unit": "GB/s", "frac": step_gbs / peak,
-                     "frac_of_8TBps": step_gbs / 8000.0, "bytes_per_cell_step": STEP_BYTES_PER_CELL}
+                     "frac_of_8TBps": step_gbs / 8000.0, "bytes_per_cell_step": step_bytes}
 
     # ---- end to end through the C ABI with HOST buffers: per step H2D of m, one RK45 step, D2H of m
     host_in = torch.from_numpy(cfg["m0"].copy()).pin_memory()
@@ -273,7 +283,7 @@ def main():
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": {"workload": "C4 film %dx%dx1, 4x4x2 nm, Permalloy, random m, B_ext 10 mT, fix_dt 1e-13 s" % (n, n),
+                "config": {"workload": wname,
                            "cells": cells, "fft": list(sim.fft_size()), "parallelism": "replicas x%d" % world,
                            "l2": "working set %.1f GB >> 126 MB L2 (no flush needed)" % (sim.stats()["peak_device_bytes"] / 1e9),
                            "evals_per_step": 6},

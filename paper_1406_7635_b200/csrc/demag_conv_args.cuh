@@ -20,8 +20,10 @@ struct ConvArgs {
 
 // argument block of the fast 2D path (fast2d.cuh)
 struct Fast2DArgs {
-  int Nx, Ny, Cx;        // Cx = Nx + 1 stored kx (0 .. Nx)
-  long long ncell;       // Nx * Ny
+  int Nx, Ny, Cx;        // transform lengths (powers of two >= the physical sizes); Cx = Nx + 1 stored kx
+  int nxp, nyp;          // physical cells along x and y (rows/columns beyond are implicit zeros)
+  int nsm;               // SMs of the device (look-ahead distance of the L2 prefetches)
+  long long ncell;       // nxp * nyp
   float2* spec;          // [3][Cx][Ny]
   long long cstride;     // Cx * Ny
   const float* Kt;       // [4][Cx][Ny + 1]: per (component, kx) the even-ky entries ky = 0,2,..,Ny

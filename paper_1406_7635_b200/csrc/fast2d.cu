@@ -156,38 +156,55 @@ int rows_per_cta(int N) {
     case 256: { CALL(256); break; }           \
   }
 
+int mm_fast2d_length(int N) {
+  int L = 256;
+  while (L < N) L *= 2;
+  return L;
+}
+
+// open one-layer films up to 4096 cells per side; sizes that are not powers of two are zero-filled
+// to the next one (any padded length >= 2N - 1 gives the same linear convolution, #4)
 bool mm_fast2d_supported(int Nx, int Ny, int Nz, const int* pbc) {
-  if (Nz != 1 || pbc[0] || pbc[1] || pbc[2]) return false;
-  const int rg = rows_per_cta(Nx);
-  return rg > 0 && rows_per_cta(Ny) > 0 && Ny % rg == 0;
+  if (Nz != 1 || pbc[0] || pbc[1] || pbc[2] || Nx > 4096 || Ny > 4096 || Nx < 64 || Ny < 64) return false;
+  const int rg = rows_per_cta(mm_fast2d_length(Nx));
+  return rg > 0 && Ny % rg == 0 && Nx % 2 == 0;
 }
 
 int mm_fast2d_init(mm_sim* s) {
   const Geometry& g = s->g;
   Fast2DArgs& a = s->f2;
-  a.Nx = g.Nx; a.Ny = g.Ny; a.Cx = g.Nx + 1;
+  a.Nx = g.Px / 2; a.Ny = g.Py / 2; a.Cx = a.Nx + 1;
+  a.nxp = g.Nx; a.nyp = g.Ny;
+  {
+    int dev = 0, nsm = 148;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+      cudaGetLastError();
+      nsm = 148;
+    }
+    a.nsm = nsm;
+  }
   a.ncell = g.N;
   a.spec = s->spec;
-  a.cstride = (long long)a.Cx * g.Ny;
+  a.cstride = (long long)a.Cx * a.Ny;
   a.Kt = s->Kt;
-  a.kstride = (long long)a.Cx * (g.Ny + 1);
+  a.kstride = (long long)a.Cx * (a.Ny + 1);
   a.regions = s->regions; a.luts = s->luts; a.st = s->dstate;
   float2 *fx, *rx, *hx, *fy, *ry, *hy;
   int rc;
-  if ((rc = axis_tables(s, g.Nx, &fx, &rx, &hx))) return rc;
-  if ((rc = axis_tables(s, g.Ny, &fy, &ry, &hy))) return rc;
+  if ((rc = axis_tables(s, a.Nx, &fx, &rx, &hx))) return rc;
+  if ((rc = axis_tables(s, a.Ny, &fy, &ry, &hy))) return rc;
   a.twx = fx; a.twx_r = rx; a.twox = hx; a.twy = fy; a.twy_r = ry; a.twoy = hy;
 #define XA(N) if ((rc = x_attrs<N>(s))) return rc
 #define YA(N) if ((rc = y_attrs<N>(s))) return rc
-  F2_SWITCH(g.Nx, XA)
-  F2_SWITCH(g.Ny, YA)
+  F2_SWITCH(a.Nx, XA)
+  F2_SWITCH(a.Ny, YA)
 #undef XA
 #undef YA
   int rows_inv = 0;
 #define RI(N) rows_inv = rows_inv_of<N>()
-  F2_SWITCH(g.Nx, RI)
+  F2_SWITCH(a.Nx, RI)
 #undef RI
-  s->f2_tma = make_spec_map(s, rows_inv, &s->f2_map_inv) && make_spec_map(s, rows_per_cta(g.Nx), &s->f2_map_fwd);
+  s->f2_tma = make_spec_map(s, rows_inv, &s->f2_map_inv) && make_spec_map(s, rows_per_cta(a.Nx), &s->f2_map_fwd);
   return MM_OK;
 }
 
@@ -196,9 +213,9 @@ void mm_fast2d_demag(mm_sim* s, int src_role) {
 #define XF(N) launch_x<N>(s, false, src_role)
 #define XI(N) launch_x<N>(s, true, R_B)
 #define YC(N) launch_y<N>(s)
-  { Launch l(s, KK_F2_XFWD); F2_SWITCH(s->g.Nx, XF) }
-  { Launch l(s, KK_F2_YCOL); F2_SWITCH(s->g.Ny, YC) }
-  { Launch l(s, KK_F2_XINV); F2_SWITCH(s->g.Nx, XI) }
+  { Launch l(s, KK_F2_XFWD); F2_SWITCH(s->f2.Nx, XF) }
+  { Launch l(s, KK_F2_YCOL); F2_SWITCH(s->f2.Ny, YC) }
+  { Launch l(s, KK_F2_XINV); F2_SWITCH(s->f2.Nx, XI) }
 #undef XF
 #undef XI
 #undef YC

@@ -64,15 +64,16 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd(Fast2DArgs a, int src_ro
     __syncthreads();
   }
   {
-    const size_t rowA = (size_t)(r0 + 2 * gid) * N;
+    const size_t rowA = (size_t)(r0 + 2 * gid) * a.nxp;      // physical row pitch; n >= nxp is zero fill
     rf::C2 v[E];
     const float2 wt = __ldg(&a.twox[t]);      // w_2N^t; the other points follow from constants
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       const int n = rf::slot_index<P, P::RA>(t, e);
-      const size_t iA = rowA + n, iB = iA + N;
+      const bool in = n < a.nxp;
+      const size_t iA = in ? rowA + n : rowA, iB = iA + a.nxp;
       const float sa = uniform ? b0 : bsat_s[reg[iA]], sb = uniform ? b0 : bsat_s[reg[iB]];
-      const float2 z = make_float2(src[iA] * sa, src[iB] * sb);            // M = B_sat m (L121)
+      const float2 z = in ? make_float2(__ldg(src + iA) * sa, __ldg(src + iB) * sb) : make_float2(0.f, 0.f);   // M = B_sat m (L121)
       const float2 zw = rf::cmul_tw1<-1>(z, rf::half_twiddle(wt, e));
       v[e] = {make_float2(z.x, zw.x), make_float2(z.y, zw.y)};
     }
@@ -158,13 +159,15 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xinv(Fast2DArgs a, int dst_ro
     for (int e = 0; e < E; ++e) v[e] = stage_unpack(xb[rf::slot_index<PI, PI::RA>(t, e)]);
     const float2 wt = __ldg(&a.twox[t]);      // w_2N^t; the other points follow from constants
     rf::fft<PI, +1, NT>(v, xb, t, gid, a.twx_r);
-    const size_t rowA = (size_t)(r0 + 2 * gid) * N;
+    const size_t rowA = (size_t)(r0 + 2 * gid) * a.nxp;      // physical row pitch; n >= nxp is zero fill
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       const int n = rf::slot_index<PI, PI::RLAST>(t, e);
       const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), rf::half_twiddle(wt, e));
-      dst[rowA + n] = v[e].re.x + u.x;
-      dst[rowA + N + n] = v[e].im.x + u.y;
+      if (n < a.nxp) {
+        dst[rowA + n] = v[e].re.x + u.x;
+        dst[rowA + a.nxp + n] = v[e].im.x + u.y;
+      }
     }
   }
 }
@@ -206,7 +209,7 @@ struct K2Col {
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       const int n = rf::slot_index<P, P::RA>(t, e);
-      const float2 z = s[n];
+      const float2 z = n < a.nyp ? s[n] : make_float2(0.f, 0.f);          // rows beyond the film: zero fill
       const float2 zw = rf::cmul_tw1<-1>(z, rf::half_twiddle(wt, e));
       v[e] = {make_float2(z.x, zw.x), make_float2(z.y, zw.y)};
     }
@@ -222,7 +225,7 @@ struct K2Col {
     for (int e = 0; e < E; ++e) {
       const int n = rf::slot_index<PI, PI::RLAST>(t, e);
       const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), rf::half_twiddle(wt, e));
-      d[n] = make_float2(v[e].re.x + u.x, v[e].im.x + u.y);
+      if (n < a.nyp) d[n] = make_float2(v[e].re.x + u.x, v[e].im.x + u.y);
     }
   }
 };
@@ -250,7 +253,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_ycol(Fast2DArgs a, int nxy) {
   {
     // columns that will be wanted soon, on their way from DRAM to L2: this job's second component and
     // the first component of the job that follows on this SM (CTAs are dispatched in order, two per SM)
-    const int ahead = kx + 2 * 148 * G;
+    const int ahead = kx + 2 * a.nsm * G;
     const float2* nxt = a.spec + (size_t)(xy ? 0 : 2) * a.cstride + (size_t)ahead * a.Ny;
     for (int i = t * 16; i < N; i += T * 16) {
       if (xy) k2_prefetch_l2(col + a.cstride + i);
@@ -374,13 +377,15 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xinv_tma(Fast2DArgs a, int ds
     for (int e = 0; e < E; ++e) v[e] = stage_unpack(xb[rf::slot_index<PI, PI::RA>(t, e)]);
     const float2 wt = __ldg(&a.twox[t]);      // w_2N^t; the other points follow from constants
     rf::fft<PI, +1, NT>(v, xb, t, gid, a.twx_r);
-    const size_t rowA = (size_t)(r0 + 2 * gid) * N;
+    const size_t rowA = (size_t)(r0 + 2 * gid) * a.nxp;      // physical row pitch; n >= nxp is zero fill
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       const int n = rf::slot_index<PI, PI::RLAST>(t, e);
       const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), rf::half_twiddle(wt, e));
-      dst[rowA + n] = v[e].re.x + u.x;
-      dst[rowA + N + n] = v[e].im.x + u.y;
+      if (n < a.nxp) {
+        dst[rowA + n] = v[e].re.x + u.x;
+        dst[rowA + a.nxp + n] = v[e].im.x + u.y;
+      }
     }
   }
 }
@@ -417,23 +422,24 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd_tma(Fast2DArgs a, int sr
   }
   {
     // rows of the CTA that follows on this SM (dispatch is in order, 512 / NT CTAs per SM): DRAM -> L2
-    int nb = (int)blockIdx.x + 148 * (512 / NT), nc = c;
+    int nb = (int)blockIdx.x + a.nsm * (512 / NT), nc = c;
     if (nb >= (int)gridDim.x) { nb -= gridDim.x; ++nc; }
     if (nc < 3 && nb < (int)gridDim.x) {
-      const float* nxt = a.st->ptr[src_role] + (size_t)nc * a.ncell + (size_t)nb * 2 * G * N;
-      for (int i = tid * 32; i < 2 * G * N; i += NT * 32) k2_prefetch_l2(nxt + i);
+      const float* nxt = a.st->ptr[src_role] + (size_t)nc * a.ncell + (size_t)nb * 2 * G * a.nxp;
+      for (int i = tid * 32; i < 2 * G * a.nxp; i += NT * 32) k2_prefetch_l2(nxt + i);
     }
   }
   {
-    const size_t rowA = (size_t)(r0 + 2 * gid) * N;
+    const size_t rowA = (size_t)(r0 + 2 * gid) * a.nxp;      // physical row pitch; n >= nxp is zero fill
     rf::C2 v[E];
     const float2 wt = __ldg(&a.twox[t]);      // w_2N^t; the other points follow from constants
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       const int n = rf::slot_index<P, P::RA>(t, e);
-      const size_t iA = rowA + n, iB = iA + N;
+      const bool in = n < a.nxp;
+      const size_t iA = in ? rowA + n : rowA, iB = iA + a.nxp;
       const float sa = uniform ? b0 : bsat_s[reg[iA]], sb = uniform ? b0 : bsat_s[reg[iB]];
-      const float2 z = make_float2(__ldg(src + iA) * sa, __ldg(src + iB) * sb);            // M = B_sat m (L121)
+      const float2 z = in ? make_float2(__ldg(src + iA) * sa, __ldg(src + iB) * sb) : make_float2(0.f, 0.f);   // M = B_sat m (L121)
       const float2 zw = rf::cmul_tw1<-1>(z, rf::half_twiddle(wt, e));
       v[e] = {make_float2(z.x, zw.x), make_float2(z.y, zw.y)};
     }

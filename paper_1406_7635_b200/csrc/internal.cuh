@@ -66,6 +66,7 @@ void* mm_dev_alloc(mm_sim* s, size_t bytes);
 void mm_dev_free(mm_sim* s, void* p);
 int mm_build_kernel_spectrum(mm_sim* s);   // setup.cu
 bool mm_fast2d_supported(int Nx, int Ny, int Nz, const int* pbc);   // fast2d.cu
+int mm_fast2d_length(int N);      // transform length of the fast path for N physical cells (power of two)
 int mm_fast2d_init(mm_sim* s);
 void mm_fast2d_demag(mm_sim* s, int src_role);
 

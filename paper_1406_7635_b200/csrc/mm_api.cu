@@ -280,6 +280,11 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
   g.Nx = Nx; g.Ny = Ny; g.Nz = Nz;
   g.N = (long long)Nx * Ny * Nz;
   g.Px = padded_length(Nx, pbc_x); g.Py = padded_length(Ny, pbc_y); g.Pz = padded_length(Nz, pbc_z);
+  s->fast2d = mm_fast2d_supported(Nx, Ny, Nz, s->rep);
+  if (s->fast2d) {   // fast 2D path: transform length = next power of two, padded length exactly twice that
+    g.Px = 2 * mm_fast2d_length(Nx);
+    g.Py = 2 * mm_fast2d_length(Ny);
+  }
   g.pbc[0] = pbc_x > 0; g.pbc[1] = pbc_y > 0; g.pbc[2] = pbc_z > 0;
   g.inv_dx2 = (float)(1.0 / (dx * dx)); g.inv_dy2 = (float)(1.0 / (dy * dy)); g.inv_dz2 = (float)(1.0 / (dz * dz));
   auto bail = [&](int code, const char* msg) {
@@ -306,14 +311,14 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
   s->dstate = (DevState*)mm_dev_alloc(s, sizeof(DevState));
   s->scratch3 = (double*)mm_dev_alloc(s, 3 * sizeof(double));
   const int rowsS = (g.Pz == 1) ? g.Ny : g.Nz * g.Py;
-  s->spec = (float2*)mm_dev_alloc(s, sizeof(float2) * 3 * (size_t)rowsS * g.pitch);
+  const size_t spec_rows = s->fast2d ? (size_t)g.Py / 2 : (size_t)rowsS;      // fast layout: [Cx][Py / 2]
+  s->spec = (float2*)mm_dev_alloc(s, sizeof(float2) * 3 * spec_rows * g.pitch);
   if (!s->regions || !s->luts || !s->dstate || !s->spec || !s->scratch3) return bail(MM_ENOMEM, "device buffers");
   if (cudaMemsetAsync(s->regions, 0, (size_t)g.N, s->stream) != cudaSuccess) return bail(MM_ECUDA, "memset");
   for (int r = 0; r < R_COUNT; ++r) cudaMemsetAsync(s->field[r], 0, fbytes, s->stream);
   if ((rc = upload_twiddles(s, g.Px, &s->twx)) || (rc = upload_twiddles(s, g.Py, &s->twy)) ||
       (rc = upload_twiddles(s, g.Pz, &s->twz)))
     return bail(rc, "twiddles");
-  s->fast2d = mm_fast2d_supported(Nx, Ny, Nz, s->rep);
   if ((rc = mm_build_kernel_spectrum(s))) { std::string m = s->err; return bail(rc, m.c_str()); }
   // convolution arguments
   ConvArgs& c = s->conv;

@@ -20,7 +20,8 @@ int mm_build_kernel_spectrum(mm_sim* s) {
   const long long nk = (long long)g.Cx * g.Hy * g.Hz;
   s->K = (float*)mm_dev_alloc(s, sizeof(float) * nk * ncomp);
   if (!s->K) return mm_fail(s, MM_ENOMEM, "kernel spectrum");
-  const long long nkt = (long long)g.Cx * (g.Ny + 1);
+  const int fNy = g.Py / 2;      // transform length along y of the fast path
+  const long long nkt = (long long)g.Cx * (fNy + 1);
   if (s->fast2d) {
     s->Kt = (float*)mm_dev_alloc(s, sizeof(float) * nkt * 4);
     if (!s->Kt) return mm_fail(s, MM_ENOMEM, "kernel spectrum (fast layout)");
@@ -60,7 +61,7 @@ int mm_build_kernel_spectrum(mm_sim* s) {
     s->launches++;
     if (s->fast2d) {
       setup::k_pack_spectrum_2dfast<<<blocks_for(nkt, 256), 256, 0, s->stream>>>(tg, src, s->Kt + (size_t)comp * nkt, g.Cx,
-                                                                                 g.Ny, scale);
+                                                                                 fNy, scale);
       s->launches++;
     }
     CUDA_TRY(s, cudaGetLastError());

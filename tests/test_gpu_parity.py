@@ -106,10 +106,11 @@ def test_multi_tile_2d_and_3d_fields(mm):
 
 
 @pytest.mark.parametrize("grid", [(256, 256, 1), (512, 256, 1), (256, 1024, 1), (2048, 256, 1), (256, 4096, 1),
-                                  (4096, 256, 1), (1024, 1024, 1)])
+                                  (4096, 256, 1), (1024, 1024, 1), (384, 320, 1), (1000, 600, 1), (66, 1536, 1)])
 def test_fast2d_path_fields(mm, grid):
-    # power-of-two open 2D films take the register-FFT kernels (fast2d.cuh); several CTAs per kernel,
-    # rectangular shapes exercise every plan on either axis; regions exercise the B_sat gather
+    # open 2D films take the register-FFT kernels (fast2d.cuh); several CTAs per kernel, rectangular
+    # shapes exercise every plan on either axis; regions exercise the B_sat gather; sizes that are not
+    # powers of two are zero-filled to the next one (ragged tails inside the transforms)
     cfg = _rand_cfg(grid, (4e-9, 4e-9, 2e-9), nreg=5, anis=True, seed=21)
     sim = mm.from_config(cfg)
     ref = _ref_from(cfg, "fft")
