@@ -92,9 +92,13 @@ int axis_tables(mm_sim* s, int N, float2** fwd, float2** rev, float2** half) {
 template <int N>
 int x_attrs(mm_sim* s) {
   using F = PlanFor<N>;
-  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd<typename F::P, F::NTF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd<typename F::P, F::NTF, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    (int)k2_smem<typename F::P, F::NTF>()));
-  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd_tma<typename F::P, F::NTF>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd<typename F::P, F::NTF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)k2_smem<typename F::P, F::NTF>()));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd_tma<typename F::P, F::NTF, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)k2_tma_store_smem<typename F::P, F::NTF>()));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd_tma<typename F::P, F::NTF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    (int)k2_tma_store_smem<typename F::P, F::NTF>()));
   CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv<typename F::P, F::NTI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    (int)k2_smem<typename F::P, F::NTI>()));
@@ -114,10 +118,17 @@ template <int N>
 void launch_x(mm_sim* s, bool inverse, int role) {
   using F = PlanFor<N>;
   constexpr int GF = F::NTF / F::P::T, GI = F::NTI / F::P::T;
-  if (!inverse && s->f2_tma)
-    k2_xfwd_tma<typename F::P, F::NTF><<<dim3(s->g.Ny / (2 * GF), 3), F::NTF, k2_tma_store_smem<typename F::P, F::NTF>(), s->stream>>>(s->f2, role, s->f2_map_fwd);
-  else if (!inverse)
-    k2_xfwd<typename F::P, F::NTF><<<dim3(s->g.Ny / (2 * GF), 3), F::NTF, k2_smem<typename F::P, F::NTF>(), s->stream>>>(s->f2, role);
+  const dim3 gf(s->g.Ny / (2 * GF), 3);
+  const bool ragged = s->f2.nxp < s->f2.Nx;
+  if (!inverse && s->f2_tma) {
+    const size_t b = k2_tma_store_smem<typename F::P, F::NTF>();
+    if (ragged) k2_xfwd_tma<typename F::P, F::NTF, true><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd);
+    else k2_xfwd_tma<typename F::P, F::NTF, false><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd);
+  } else if (!inverse) {
+    const size_t b = k2_smem<typename F::P, F::NTF>();
+    if (ragged) k2_xfwd<typename F::P, F::NTF, true><<<gf, F::NTF, b, s->stream>>>(s->f2, role);
+    else k2_xfwd<typename F::P, F::NTF, false><<<gf, F::NTF, b, s->stream>>>(s->f2, role);
+  }
   else if (s->f2_tma)
     k2_xinv_tma<typename F::P, F::NTI><<<dim3(s->g.Ny / (2 * GI), 3), F::NTI, k2_tma_smem<typename F::P, F::NTI>(), s->stream>>>(s->f2, role, s->f2_map_inv);
   else

@@ -46,7 +46,8 @@ __device__ __forceinline__ float4 separate(float2 z, float2 zm) {
 }
 
 // ---------------------------------------------------------------------------------- K_A
-template <class P, int NT>
+// RAGGED: the film is narrower than the transform (nxp < N): columns beyond are zero fill
+template <class P, int NT, bool RAGGED>
 __global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd(Fast2DArgs a, int src_role) {
   if (a.st->skip) return;
   constexpr int N = P::N, T = P::T, E = P::E, G = NT / T, GP = K2Shape<P, NT>::GP;
@@ -70,10 +71,12 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd(Fast2DArgs a, int src_ro
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       const int n = rf::slot_index<P, P::RA>(t, e);
-      const bool in = n < a.nxp;
-      const size_t iA = in ? rowA + n : rowA, iB = iA + a.nxp;
-      const float sa = uniform ? b0 : bsat_s[reg[iA]], sb = uniform ? b0 : bsat_s[reg[iB]];
-      const float2 z = in ? make_float2(__ldg(src + iA) * sa, __ldg(src + iB) * sb) : make_float2(0.f, 0.f);   // M = B_sat m (L121)
+      float2 z = make_float2(0.f, 0.f);
+      if (!RAGGED || n < a.nxp) {
+        const size_t iA = rowA + n, iB = iA + a.nxp;
+        const float sa = uniform ? b0 : bsat_s[reg[iA]], sb = uniform ? b0 : bsat_s[reg[iB]];
+        z = make_float2(src[iA] * sa, src[iB] * sb);            // M = B_sat m (L121)
+      }
       const float2 zw = rf::cmul_tw1<-1>(z, rf::half_twiddle(wt, e));
       v[e] = {make_float2(z.x, zw.x), make_float2(z.y, zw.y)};
     }
@@ -401,7 +404,7 @@ constexpr size_t k2_tma_store_smem() {
   return k2_smem<P, NT>() + (size_t)K2StoreRing<K2Shape<P, NT>::G>::NBUF * K2_KB * K2Shape<P, NT>::G * sizeof(float4) + 128;
 }
 
-template <class P, int NT>
+template <class P, int NT, bool RAGGED>
 __global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd_tma(Fast2DArgs a, int src_role, const __grid_constant__ CUtensorMap map) {
   if (a.st->skip) return;
   constexpr int N = P::N, T = P::T, E = P::E, G = NT / T, GP = K2Shape<P, NT>::GP;
@@ -436,10 +439,12 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd_tma(Fast2DArgs a, int sr
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       const int n = rf::slot_index<P, P::RA>(t, e);
-      const bool in = n < a.nxp;
-      const size_t iA = in ? rowA + n : rowA, iB = iA + a.nxp;
-      const float sa = uniform ? b0 : bsat_s[reg[iA]], sb = uniform ? b0 : bsat_s[reg[iB]];
-      const float2 z = in ? make_float2(__ldg(src + iA) * sa, __ldg(src + iB) * sb) : make_float2(0.f, 0.f);   // M = B_sat m (L121)
+      float2 z = make_float2(0.f, 0.f);
+      if (!RAGGED || n < a.nxp) {
+        const size_t iA = rowA + n, iB = iA + a.nxp;
+        const float sa = uniform ? b0 : bsat_s[reg[iA]], sb = uniform ? b0 : bsat_s[reg[iB]];
+        z = make_float2(src[iA] * sa, src[iB] * sb);            // M = B_sat m (L121)
+      }
       const float2 zw = rf::cmul_tw1<-1>(z, rf::half_twiddle(wt, e));
       v[e] = {make_float2(z.x, zw.x), make_float2(z.y, zw.y)};
     }
