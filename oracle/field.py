@@ -156,8 +156,10 @@ def cross(a, b):
     return np.stack([a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]])
 
 
-def ll_torque_over_gamma(m, B, alpha_cell):
+def ll_torque_over_gamma(m, B, alpha_cell, precession=True):
     """tau / gamma_LL = -1/(1+alpha^2) [ m x B + alpha m x (m x B) ]  (Eq. 2 with the sign of
-    SURVEY.md 8(c) #5: damping must move m towards B)."""
+    SURVEY.md 8(c) #5: damping must move m towards B).  precession=False drops the m x B term
+    ("disables the precession term", relax())."""
     mxB = cross(m, B)
-    return -(mxB + alpha_cell[None] * cross(m, mxB)) / (1.0 + alpha_cell[None] ** 2)
+    damp = alpha_cell[None] * cross(m, mxB)
+    return -((mxB if precession else 0.0) + damp) / (1.0 + alpha_cell[None] ** 2)

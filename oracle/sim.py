@@ -26,6 +26,16 @@ DP_B5 = (35 / 384, 0.0, 500 / 1113, 125 / 192, -2187 / 6784, 11 / 84, 0.0)
 DP_B4 = (5179 / 57600, 0.0, 7571 / 16695, 393 / 640, -92097 / 339200, 187 / 2100, 1 / 40)
 DP_E = tuple(b5 - b4 for b5, b4 in zip(DP_B5, DP_B4))
 
+# Bogacki-Shampine 3(2), 4 stages with FSAL ("RK32, the Bogacki-Shampine method, 3-th order convergence
+# and a 2nd order error estimate"; the paper prints no tableau: textbook coefficients)
+BS_A = ((), (1 / 2,), (0.0, 3 / 4), (2 / 9, 1 / 3, 4 / 9))
+BS_B3 = (2 / 9, 1 / 3, 4 / 9, 0.0)
+BS_B2 = (7 / 24, 1 / 4, 1 / 3, 1 / 8)
+BS_E = tuple(b3 - b2 for b3, b2 in zip(BS_B3, BS_B2))
+
+# solver -> (a rows, error weights, exponent of the step-size rule = 1 / order of the solution)
+SOLVERS = {"rk45": (DP_A, DP_E, 1 / 5), "rk23": (BS_A, BS_E, 1 / 3)}
+
 DIRECT_SUM_MAX_CELLS = 2048
 
 
@@ -54,6 +64,14 @@ class RefSim:
         self._K = None
         self._Kp = None
         self.terms = MM_ALL
+        self.solver = "rk45"
+        self.precession = True
+
+    def set_solver_kind(self, name):
+        """"rk45" (default) or "rk23" (L366). Invalidates the FSAL slope."""
+        assert name in SOLVERS
+        self.solver = name
+        self.k1 = None
 
     # ---- setup
     def set_terms(self, mask):
@@ -112,7 +130,7 @@ class RefSim:
         """dm/dt [1/s] (Eq. 1-2)."""
         self.n_eval += 1
         alpha = self.p.alpha[self.regions]
-        return self.p.gamma_LL * fld.ll_torque_over_gamma(m, self.b_eff(self.terms, m), alpha)
+        return self.p.gamma_LL * fld.ll_torque_over_gamma(m, self.b_eff(self.terms, m), alpha, self.precession)
 
     # ---- energies (Eq. 4, 8, 20, 23; Zeeman -M.B_ext), joules
     def energy(self, m=None):
@@ -129,29 +147,31 @@ class RefSim:
         e += -(M * np.asarray(self.p.B_ext)[:, None, None, None]).sum()
         return e * self.cell[0] * self.cell[1] * self.cell[2]
 
-    # ---- one attempted Dormand-Prince step
+    # ---- one attempted Runge-Kutta step of the selected embedded pair
     def step(self, dt_force=None):
+        A, E, expo = SOLVERS[self.solver]
+        ns = len(A)
         if self.k1 is None:
             self.k1 = self.torque(self.m)
         h = self.dt if dt_force is None else dt_force
         m0 = self.m
         k = [self.k1]
         y = None
-        for i in range(1, 7):
-            y = _normalise(m0 + h * sum(a * kj for a, kj in zip(DP_A[i], k)))   # every stage input
+        for i in range(1, ns):
+            y = _normalise(m0 + h * sum(a * kj for a, kj in zip(A[i], k)))       # every stage input
             k.append(self.torque(y))                                              # is renormalised (#9)
-        err_vec = sum(e * kj for e, kj in zip(DP_E, k))
+        err_vec = sum(e * kj for e, kj in zip(E, k))
         err = h * np.sqrt((err_vec * err_vec).sum(axis=0)).max()
         fixed = self.fix_dt > 0
         accepted = fixed or (err <= self.max_err)
         if accepted:
-            self.m, self.k1 = y, k[6]            # y_7 is the 5th-order result; FSAL: k7 -> k1
+            self.m, self.k1 = y, k[ns - 1]       # last stage input = the high-order result; FSAL
             self.t += h
             self.n_steps += 1
         else:
             self.n_rejected += 1
         if not fixed:
-            fac = 2.0 if err == 0 else min(2.0, max(0.5, (self.max_err / err) ** 0.2))
+            fac = 2.0 if err == 0 else min(2.0, max(0.5, (self.max_err / err) ** expo))
             self.dt = min(self.dt_max, max(self.dt_min, h * self.headroom * fac))
         return dict(t=self.t, dt_taken=h, dt_next=self.dt, err=err, accepted=accepted)
 

@@ -210,6 +210,51 @@ def test_dormand_prince_tableau_conditions():
     assert abs(sum(osim.DP_E)) < 1e-15
 
 
+def test_bogacki_shampine_tableau_conditions_and_third_order_convergence():
+    # RK23 (L366): 3rd-order solution, 2nd-order embedded estimate, FSAL; Fig. 10 shows its 3rd-order slope
+    A, b3, b2 = osim.BS_A, np.array(osim.BS_B3), np.array(osim.BS_B2)
+    c = np.array([sum(r) for r in A])
+    assert np.allclose(c, [0, 1 / 2, 3 / 4, 1]) and tuple(A[3]) == tuple(b3[:3])      # FSAL
+    for q in range(3):
+        assert abs((b3 * c ** q).sum() - 1 / (q + 1)) < 1e-15
+    for q in range(2):
+        assert abs((b2 * c ** q).sum() - 1 / (q + 1)) < 1e-15
+    Am = np.zeros((4, 4))
+    for i in range(4):
+        Am[i, :len(A[i])] = A[i]
+    assert abs(b3 @ Am @ c - 1 / 6) < 1e-15 and abs(b2 @ Am @ c - 1 / 6) > 1e-3    # order 3 vs only order 2
+    assert abs(sum(osim.BS_E)) < 1e-15
+    period = 2 * np.pi / (0.1 * GAMMA)
+    errs = []
+    for n in (40, 80, 160):
+        sim = _macrospin(m0=(1, 0, 1))
+        sim.set_solver_kind("rk23")
+        sim.set_solver(fix_dt=period / n)
+        for _ in range(n):
+            sim.step()
+        errs.append(np.linalg.norm(sim.m[:, 0, 0, 0] - np.array([1, 0, 1]) / np.sqrt(2)))
+    assert 6.5 < errs[0] / errs[1] < 10 and 7 < errs[1] / errs[2] < 9.5          # 2^3 = 8 asymptotically
+    # adaptive: lands on time, error scales with MaxErr (Fig. 11), three evaluations per step
+    sim = _macrospin(m0=(1, 0, 1))
+    sim.set_solver_kind("rk23")
+    sim.set_solver(max_err=1e-6, dt_init=1e-13)
+    sim.run(period)
+    assert abs(sim.t - period) < 1e-24
+    assert np.linalg.norm(sim.m[:, 0, 0, 0] - np.array([1, 0, 1]) / np.sqrt(2)) < 1e-3
+    assert sim.n_eval == 1 + 3 * (sim.n_steps + sim.n_rejected)
+
+
+def test_no_precession_torque_only_lowers_the_energy():
+    # relax() "disables the precession term" (L388): m then moves straight towards B_eff
+    sim = _macrospin(alpha=0.5, m0=(1, 0, 0.2))
+    sim.precession = False
+    sim.set_solver(max_err=1e-6)
+    e0 = sim.energy()
+    sim.run(0.05e-9)
+    mx, my, mz = sim.m[:, 0, 0, 0]
+    assert abs(my) < 1e-12 and mz > 0.2 and sim.energy() < e0      # stays in the x-z plane: no precession
+
+
 def _small_film(alpha, seed=21, grid=(12, 6, 1), fix_dt=0.0):
     sim = RefSim(grid, (4e-9, 4e-9, 3e-9))
     sim.set_params(Params.uniform(1, Msat=8e5, Aex=1.3e-11, alpha=alpha))
