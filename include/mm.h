@@ -116,6 +116,17 @@ int mm_set_option(mm_sim* sim, int option, int value);
 int mm_set_solver(mm_sim* sim, double max_err, double headroom, double fix_dt, double dt_init, double dt_min,
                   double dt_max);
 
+/* Which embedded Runge-Kutta pair mm_step_rk45 / mm_steps / mm_run advance with (the paper's SetSolver,
+ * L805, L853): MM_RK45 = Dormand-Prince 5(4), 7 stages, the default for dynamics (L365); MM_RK23 =
+ * Bogacki-Shampine 3(2), 4 stages, used when relaxing (L366, L392). Both are FSAL; the step-size rule
+ * uses the exponent 1/5 resp. 1/3. Invalidates the FSAL slope. */
+enum { MM_RK45 = 0, MM_RK23 = 1 };
+int mm_set_solver_kind(mm_sim* sim, int kind);
+
+/* Precession term of Eq. 2 on (default) or off: off leaves tau = -gamma alpha/(1+alpha^2) m x (m x B),
+ * "so that the effective field points towards decreasing energy" (relax(), L388). */
+int mm_set_precession(mm_sim* sim, int on);
+
 /* Reduced magnetisation: 3N floats; normalised to unit length on entry (L85). Cells with
  * Msat = 0 keep m = 0. Invalidates the FSAL slope. mm_get_m copies the current m out. */
 int mm_set_m(mm_sim* sim, const float* m);
@@ -131,6 +142,8 @@ int mm_torque(mm_sim* sim, float* tau_over_gamma_out);
  * synchronisation); otherwise the stream is synchronised and *info filled.
  * MM_ESTATE before mm_set_params + mm_set_m; MM_ENAN if the error estimate is not finite. */
 int mm_step_rk45(mm_sim* sim, mm_step_info* info_or_null);
+/* The same call under a solver-neutral name: one attempted step of the selected pair. */
+int mm_step(mm_sim* sim, mm_step_info* info_or_null);
 
 /* n attempted steps, enqueued back to back without host synchronisation (the paper's steps(n),
  * L1072, counting rejected attempts too). Synchronises once at the end. */

@@ -14,6 +14,7 @@ MM_OK, MM_EINVAL, MM_ENOMEM, MM_ECUDA, MM_ESTATE, MM_ENAN, MM_EDT = 0, -1, -2, -
 MM_DEMAG, MM_EXCH, MM_ANIS, MM_ZEEMAN, MM_ALL = 1, 2, 4, 8, 15
 MM_MAX_REGIONS = 256
 MM_OPT_GENERIC_FFT = 1
+MM_RK45, MM_RK23 = 0, 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmm_b200.so")
@@ -65,7 +66,10 @@ _SIGNATURES = {
     "mm_get_m": (C.c_int, [C.c_void_p, C.c_void_p]),
     "mm_b_eff": (C.c_int, [C.c_void_p, C.c_uint, C.c_void_p]),
     "mm_torque": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "mm_set_solver_kind": (C.c_int, [C.c_void_p, C.c_int]),
+    "mm_set_precession": (C.c_int, [C.c_void_p, C.c_int]),
     "mm_step_rk45": (C.c_int, [C.c_void_p, C.POINTER(mm_step_info)]),
+    "mm_step": (C.c_int, [C.c_void_p, C.POINTER(mm_step_info)]),
     "mm_steps": (C.c_int, [C.c_void_p, C.c_int]),
     "mm_run": (C.c_int, [C.c_void_p, C.c_double]),
     "mm_get_time": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
@@ -207,6 +211,13 @@ class Sim:
 
     def set_solver(self, max_err=0.0, headroom=0.0, fix_dt=0.0, dt_init=0.0, dt_min=0.0, dt_max=0.0):
         _check(lib().mm_set_solver(self._h, max_err, headroom, fix_dt, dt_init, dt_min, dt_max), self._h)
+
+    def set_solver_kind(self, kind):
+        """MM_RK45 (default) or MM_RK23."""
+        _check(lib().mm_set_solver_kind(self._h, int(kind)), self._h)
+
+    def set_precession(self, on):
+        _check(lib().mm_set_precession(self._h, 1 if on else 0), self._h)
 
     def set_m(self, m):
         if isinstance(m, np.ndarray):

@@ -23,6 +23,8 @@ struct DevState {
   float hg;          // gamma * h as float (torque slopes are kept in tesla)
   unsigned err_bits; // float bits of max || sum_j e_j k_j ||  (atomicMax; non-negative floats order as uints)
   float last_err;
+  int nstage;        // stages of the embedded pair: 7 (Dormand-Prince) or 4 (Bogacki-Shampine)
+  double expo;       // exponent of the step-size rule: 1/5 or 1/3
   int run_mode;      // 1: stop at t_end
   int clipped;       // current attempt was clipped to land on t_end
   int skip;          // 1: t_end reached (or failure) -> every kernel of the step returns at once

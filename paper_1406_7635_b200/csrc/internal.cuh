@@ -46,6 +46,8 @@ struct mm_sim {
   DevState hst;
   bool have_params = false, have_m = false, have_k1 = false;
   unsigned terms = MM_ALL;
+  int solver = MM_RK45;
+  bool precession = true;
   int nregions = 1;
   long launches = 0;
   long extra_evals = 0;

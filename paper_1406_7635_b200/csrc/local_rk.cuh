@@ -76,7 +76,8 @@ __global__ void k_local(Geometry g, const uint8_t* __restrict__ regions, const L
     const float pre = -lut->live[r] / (1.f + al * al);
     float tx = my * bz - mz * by, ty = mz * bx - mx * bz, tz = mx * by - my * bx;   // m x B
     float dx = my * tz - mz * ty, dy = mz * tx - mx * tz, dz = mx * ty - my * tx;   // m x (m x B)
-    bx = pre * (tx + al * dx); by = pre * (ty + al * dy); bz = pre * (tz + al * dz);
+    const float pr = out_torque == 1 ? 1.f : 0.f;      // out_torque == 2: precession term off (relax, L388)
+      bx = pre * (pr * tx + al * dx); by = pre * (pr * ty + al * dy); bz = pre * (pr * tz + al * dz);
   }
   dst[i] = bx; dst[N + i] = by; dst[2 * N + i] = bz;
 }
@@ -199,7 +200,8 @@ __global__ void __launch_bounds__(128) k_local4(Geometry g, const uint8_t* __res
       const float pre = -lut->live[rr] / (1.f + al * al);
       float tx = my * bz - mz * by, ty = mz * bx - mx * bz, tz = mx * by - my * bx;   // m x B
       float dx = my * tz - mz * ty, dy = mz * tx - mx * tz, dz = mx * ty - my * tx;   // m x (m x B)
-      bx = pre * (tx + al * dx); by = pre * (ty + al * dy); bz = pre * (tz + al * dz);
+      const float pr = out_torque == 1 ? 1.f : 0.f;      // out_torque == 2: precession term off (relax, L388)
+      bx = pre * (pr * tx + al * dx); by = pre * (pr * ty + al * dy); bz = pre * (pr * tz + al * dz);
     }
     b[0][l] = bx; b[1][l] = by; b[2][l] = bz;
   }
@@ -288,14 +290,15 @@ __global__ void k_ctrl_end(DevState* st) {
   const double h = st->h;
   const double err = (double)emax * st->gamma * h;
   st->last_err = (float)err;
-  st->evals += 6;
+  st->evals += st->nstage - 1;
   if (!(err == err) || isinf(err)) { st->status = MM_ENAN; st->last_accepted = 0; st->skip = 1; return; }
   const bool fixed = st->fix_dt > 0;
   const bool accept = fixed || err <= st->max_err;
   st->last_accepted = accept ? 1 : 0;
   if (accept) {
     float* p = st->ptr[R_M]; st->ptr[R_M] = st->ptr[R_MNEW]; st->ptr[R_MNEW] = p;
-    p = st->ptr[R_K0]; st->ptr[R_K0] = st->ptr[R_K6]; st->ptr[R_K6] = p;
+    const int last = R_K0 + st->nstage - 1;          // FSAL: the last stage slope is the next first one
+    p = st->ptr[R_K0]; st->ptr[R_K0] = st->ptr[last]; st->ptr[last] = p;
     st->t = st->clipped ? st->t_end : st->t + h;
     st->steps += 1;
   } else {
@@ -305,7 +308,7 @@ __global__ void k_ctrl_end(DevState* st) {
     if (accept && st->clipped) {
       st->dt = st->keep_dt;
     } else {
-      double fac = (err == 0.0) ? 2.0 : fmin(2.0, fmax(0.5, pow(st->max_err / err, 0.2)));
+      double fac = (err == 0.0) ? 2.0 : fmin(2.0, fmax(0.5, pow(st->max_err / err, st->expo)));
       double dt = h * st->headroom * fac;
       dt = fmin(st->dt_max, fmax(st->dt_min, dt));
       if (!accept && h <= st->dt_min) { st->status = MM_EDT; st->skip = 1; }

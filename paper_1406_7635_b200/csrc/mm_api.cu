@@ -30,6 +30,10 @@ const double DP_E[7] = {35.0 / 384 - 5179.0 / 57600, 0.0, 500.0 / 1113 - 7571.0 
                         -2187.0 / 6784 + 92097.0 / 339200, 11.0 / 84 - 187.0 / 2100, -1.0 / 40};
 
 
+// Bogacki-Shampine 3(2) tableau (PAPER.md L366 names the method; textbook coefficients)
+const double BS_A[4][6] = {{0, 0, 0, 0, 0, 0}, {1.0 / 2, 0, 0, 0, 0, 0}, {0, 3.0 / 4, 0, 0, 0, 0}, {2.0 / 9, 1.0 / 3, 4.0 / 9, 0, 0, 0}};
+const double BS_E[7] = {2.0 / 9 - 7.0 / 24, 1.0 / 3 - 1.0 / 4, 4.0 / 9 - 1.0 / 3, -1.0 / 8, 0, 0, 0};
+
 bool smooth5(int n) {
   for (int f : {2, 3, 5}) while (n % f == 0) n /= f;
   return n == 1;
@@ -186,22 +190,25 @@ void launch_eval(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_t
 
 void enqueue_step(mm_sim* s) {
   const long long N = s->g.N;
+  const bool bs = s->solver == MM_RK23;
+  const int ns = bs ? 4 : 7;                                  // stages; the last one is the FSAL evaluation
+  const int tq = s->precession ? 1 : 2;                       // torque with / without the precession term
   if (!s->have_k1) {
-    launch_eval(s, R_M, R_K0, s->terms, 1);
+    launch_eval(s, R_M, R_K0, s->terms, tq);
     s->have_k1 = true;
     s->extra_evals++;
   }
   { Launch l(s, KK_CTRL); k_ctrl_begin<<<1, 1, 0, s->stream>>>(s->dstate); }
-  for (int i = 1; i < 7; ++i) {
+  for (int i = 1; i < ns; ++i) {
     StageCoef sc;
     sc.n = i;
-    for (int j = 0; j < 6; ++j) sc.a[j] = (float)DP_A[i][j];
-    const int yrole = (i == 6) ? R_MNEW : R_Y;
+    for (int j = 0; j < 6; ++j) sc.a[j] = (float)(bs ? BS_A[i][j] : DP_A[i][j]);
+    const int yrole = (i == ns - 1) ? R_MNEW : R_Y;
     { Launch l(s, KK_STAGE); k_stage<<<blocks_for(N, 256), 256, 0, s->stream>>>(N, s->dstate, sc, yrole); }
-    launch_eval(s, yrole, R_K0 + i, s->terms, 1);
+    launch_eval(s, yrole, R_K0 + i, s->terms, tq);
   }
   ErrCoef ec;
-  for (int j = 0; j < 7; ++j) ec.e[j] = (float)DP_E[j];
+  for (int j = 0; j < 7; ++j) ec.e[j] = (float)(bs ? BS_E[j] : DP_E[j]);
   { Launch l(s, KK_ERROR); k_error<<<148 * 8, 256, 0, s->stream>>>(N, s->dstate, ec); }
   { Launch l(s, KK_CTRL); k_ctrl_end<<<1, 1, 0, s->stream>>>(s->dstate); }
 }
@@ -334,6 +341,7 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
   for (int r = 0; r < R_COUNT; ++r) h.ptr[r] = s->field[r];
   h.max_err = 1e-5; h.headroom = 0.8; h.fix_dt = 0.0; h.dt = 1e-14; h.dt_min = 1e-18; h.dt_max = 1e-9;
   h.gamma = 1.7595e11;
+  h.nstage = 7; h.expo = 0.2;
   h.status = MM_OK;
   if ((rc = push_state(s))) { std::string m = s->err; return bail(rc, m.c_str()); }
   *out = s;
@@ -443,6 +451,27 @@ int mm_set_terms(mm_sim* s, unsigned mask) {
   return MM_OK;
 }
 
+int mm_set_solver_kind(mm_sim* s, int kind) {
+  if (!s) return MM_EINVAL;
+  if (kind != MM_RK45 && kind != MM_RK23) return mm_fail(s, MM_EINVAL, "unknown solver");
+  int rc;
+  if ((rc = pull_state(s))) return rc;
+  s->solver = kind;
+  s->hst.nstage = kind == MM_RK23 ? 4 : 7;
+  s->hst.expo = kind == MM_RK23 ? 1.0 / 3.0 : 0.2;
+  s->have_k1 = false;
+  return push_state(s);
+}
+
+int mm_set_precession(mm_sim* s, int on) {
+  if (!s) return MM_EINVAL;
+  s->precession = on != 0;
+  s->have_k1 = false;
+  return MM_OK;
+}
+
+int mm_step(mm_sim* s, mm_step_info* info) { return mm_step_rk45(s, info); }
+
 int mm_set_option(mm_sim* s, int option, int value) {
   if (!s) return MM_EINVAL;
   switch (option) {
@@ -505,7 +534,7 @@ int mm_torque(mm_sim* s, float* out) {
   int rc;
   if ((rc = check_ready(s))) return rc;
   if (!out) return mm_fail(s, MM_EINVAL, "null argument");
-  launch_eval(s, R_M, R_Y, s->terms, 1);
+  launch_eval(s, R_M, R_Y, s->terms, s->precession ? 1 : 2);
   CUDA_TRY(s, cudaGetLastError());
   if ((rc = pull_state(s))) return rc;
   return copy_out(s, out, s->hst.ptr[R_Y], sizeof(float) * 3 * (size_t)s->g.N);

@@ -339,3 +339,53 @@ def test_device_pointers_and_vacuum_cells(mm):
     assert np.all(m[:, cfg["regions"] == 1] == 0)
     sim.steps(3)
     assert np.all(sim.get_m()[:, cfg["regions"] == 1] == 0)
+
+
+# --------------------------------------------------------------------------- RK23 and relax building blocks
+def test_rk23_fixed_step_trajectory_and_adaptive_run(mm):
+    # Bogacki-Shampine pair (L366): same kernels, 3 new evaluations per step, exponent 1/3
+    cfg = config_c1()
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg)
+    sim.set_solver_kind(mm.MM_RK23); ref.set_solver_kind("rk23")
+    sim.set_solver(fix_dt=1e-13); ref.set_solver(fix_dt=1e-13)
+    e0 = sim.stats()["evals"]
+    sim.steps(50)
+    for _ in range(50):
+        ref.step()
+    assert np.abs(sim.get_m() - ref.m).max() < 1e-4
+    assert sim.stats()["evals"] - e0 == 1 + 3 * 50
+    # adaptive: both sides to the same physical time; every attempt costs three evaluations
+    sim.set_solver(max_err=1e-5, dt_init=1e-14); ref.set_solver(max_err=1e-5, dt_init=1e-14)
+    t0 = sim.t
+    sim.run(20e-12); ref.run(20e-12)
+    assert abs((sim.t - t0) - 20e-12) < 1e-24
+    assert np.abs(sim.avg_m() - ref.avg_m()).max() < 1e-3
+    st = sim.stats()
+    assert st["steps"] > 50 and st["rejected"] >= 0
+    info = sim.step()
+    assert info["accepted"] in (0, 1) and info["err"] >= 0
+    # back to RK45: the FSAL slope is recomputed, trajectories still agree
+    sim.set_solver_kind(mm.MM_RK45); ref.set_solver_kind("rk45")
+
+
+def test_precession_off_descends_in_energy(mm):
+    # relax()'s right-hand side (L388): tau = -gamma alpha/(1+alpha^2) m x (m x B); parity of the
+    # torque itself and of a short trajectory; the oracle's energy of the GPU state must fall
+    cfg = _rand_cfg((64, 32, 1), (4e-9, 4e-9, 3e-9), nreg=3, anis=True, seed=4)
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    sim.set_precession(False); ref.precession = False
+    tq = sim.torque().astype(np.float64)
+    tr = ref.torque(ref.m) / ref.p.gamma_LL
+    assert np.abs(tq - tr).max() <= FIELD_TOL * np.abs(tr).max()
+    m = ref.m
+    assert np.abs((tq * m).sum(axis=0)).max() < 1e-4 * np.abs(tq).max()        # tau is perpendicular to m
+    sim.set_solver_kind(mm.MM_RK23); ref.set_solver_kind("rk23")
+    sim.set_solver(fix_dt=2e-14); ref.set_solver(fix_dt=2e-14)
+    e0 = ref.energy()
+    sim.steps(40)
+    for _ in range(40):
+        ref.step()
+    assert np.abs(sim.get_m() - ref.m).max() < 1e-4
+    assert ref.energy(sim.get_m().astype(np.float64)) < e0
