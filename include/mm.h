@@ -155,6 +155,13 @@ int mm_steps(mm_sim* sim, int n);
  * MM_EDT if the step size falls below dt_min; MM_ENAN on a non-finite error estimate. */
 int mm_run(mm_sim* sim, double duration);
 
+/* Total energy of the current m for the selected terms, joules: demag Eq. 4 (L125), exchange Eq. 8
+ * (L202), anisotropy Eq. 20 / 23 (L278, L297), Zeeman -M.B_ext; fp32 per cell, fp64 sum. */
+int mm_energy(mm_sim* sim, unsigned term_mask, double* joules);
+/* max over cells of |torque| / gamma_LL [T] of the current m (enabled terms, precession switch as
+ * set): the quantity relax() monitors near equilibrium (L388-L390). */
+int mm_max_torque(mm_sim* sim, double* tesla);
+
 int mm_get_time(mm_sim* sim, double* t);
 int mm_set_time(mm_sim* sim, double t);
 /* Plain mean of m over all cells (fp64 accumulation), the paper's m.average() (L861). */

@@ -133,18 +133,23 @@ class RefSim:
         return self.p.gamma_LL * fld.ll_torque_over_gamma(m, self.b_eff(self.terms, m), alpha, self.precession)
 
     # ---- energies (Eq. 4, 8, 20, 23; Zeeman -M.B_ext), joules
-    def energy(self, m=None):
+    def energy(self, m=None, terms=MM_ALL):
         m = self.m if m is None else m
         Ms = self.p.Msat[self.regions][None]
         M = Ms * m
-        e = -0.5 * (M * self.b_demag(m)).sum()
-        e += -0.5 * (M * fld.b_exchange(m, self.regions, self.L, self.cell, self.pbc)).sum()
-        e += -0.5 * (M * fld.b_anis_uniaxial(m, self.regions, self.p, only=1)).sum()
-        e += -0.25 * (M * fld.b_anis_uniaxial(m, self.regions, self.p, only=2)).sum()
-        e += -(1 / 4) * (M * fld.b_anis_cubic(m, self.regions, self.p, only=1)).sum()
-        e += -(1 / 6) * (M * fld.b_anis_cubic(m, self.regions, self.p, only=2)).sum()
-        e += -(1 / 8) * (M * fld.b_anis_cubic(m, self.regions, self.p, only=3)).sum()
-        e += -(M * np.asarray(self.p.B_ext)[:, None, None, None]).sum()
+        e = 0.0
+        if terms & MM_DEMAG:
+            e += -0.5 * (M * self.b_demag(m)).sum()                                            # Eq. 4
+        if terms & MM_EXCH:
+            e += -0.5 * (M * fld.b_exchange(m, self.regions, self.L, self.cell, self.pbc)).sum()   # Eq. 8
+        if terms & MM_ANIS:
+            e += -0.5 * (M * fld.b_anis_uniaxial(m, self.regions, self.p, only=1)).sum()       # Eq. 20
+            e += -0.25 * (M * fld.b_anis_uniaxial(m, self.regions, self.p, only=2)).sum()
+            e += -(1 / 4) * (M * fld.b_anis_cubic(m, self.regions, self.p, only=1)).sum()      # Eq. 23
+            e += -(1 / 6) * (M * fld.b_anis_cubic(m, self.regions, self.p, only=2)).sum()
+            e += -(1 / 8) * (M * fld.b_anis_cubic(m, self.regions, self.p, only=3)).sum()
+        if terms & MM_ZEEMAN:
+            e += -(M * np.asarray(self.p.B_ext)[:, None, None, None]).sum()
         return e * self.cell[0] * self.cell[1] * self.cell[2]
 
     # ---- one attempted Runge-Kutta step of the selected embedded pair

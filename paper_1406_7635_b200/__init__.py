@@ -72,6 +72,8 @@ _SIGNATURES = {
     "mm_step": (C.c_int, [C.c_void_p, C.POINTER(mm_step_info)]),
     "mm_steps": (C.c_int, [C.c_void_p, C.c_int]),
     "mm_run": (C.c_int, [C.c_void_p, C.c_double]),
+    "mm_energy": (C.c_int, [C.c_void_p, C.c_uint, C.POINTER(C.c_double)]),
+    "mm_max_torque": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
     "mm_get_time": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
     "mm_set_time": (C.c_int, [C.c_void_p, C.c_double]),
     "mm_get_avg_m": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
@@ -263,6 +265,16 @@ class Sim:
     def t(self):
         v = C.c_double()
         _check(lib().mm_get_time(self._h, C.byref(v)), self._h)
+        return v.value
+
+    def energy(self, term_mask=MM_ALL):
+        v = C.c_double()
+        _check(lib().mm_energy(self._h, int(term_mask), C.byref(v)), self._h)
+        return v.value
+
+    def max_torque(self):
+        v = C.c_double()
+        _check(lib().mm_max_torque(self._h, C.byref(v)), self._h)
         return v.value
 
     def set_time(self, t):

@@ -341,3 +341,81 @@ __global__ void k_sum3(long long N, const float* __restrict__ m, double* __restr
     if ((threadIdx.x & 31) == 0) atomicAdd(&out[c], s[c]);
   }
 }
+
+// Energy of the selected terms, joules / cell volume summed over cells (fp64 accumulation):
+//   E/V = - sum_cells M . [ 1/2 B_demag (Eq. 4) + 1/2 B_exch (Eq. 8) + 1/2 B_anis(Ku1) + 1/4 B_anis(Ku2) (Eq. 20)
+//                           + 1/4 B(Kc1) + 1/6 B(Kc2) + 1/8 B(Kc3) (Eq. 23) + B_ext ],   M = Msat m.
+// B_demag of m must already be in role bd_role. out[0] must be zeroed first.
+__global__ void k_energy(Geometry g, const uint8_t* __restrict__ regions, const Luts* __restrict__ lut, DevState* st,
+                         int m_role, int bd_role, unsigned mask, double* __restrict__ out) {
+  const float* __restrict__ m = st->ptr[m_role];
+  const float* __restrict__ bd = st->ptr[bd_role];
+  const long long N = g.N;
+  double acc = 0.0;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+    const int x = (int)(i % g.Nx);
+    const long long t = i / g.Nx;
+    const int y = (int)(t % g.Ny), z = (int)(t / g.Ny);
+    const int r = regions[i];
+    const float mx = m[i], my = m[N + i], mz = m[2 * N + i];
+    float e = 0.f;                                      // sum of weight * m . B  [T]
+    if (mask & MM_DEMAG) e += 0.5f * (mx * bd[i] + my * bd[N + i] + mz * bd[2 * N + i]);
+    if (mask & MM_EXCH) {
+      float ex = 0.f, ey = 0.f, ez = 0.f;
+      auto nb = [&](long long j, float w) {
+        float a = w * __ldg(&lut->exch[tri_index(r, regions[j])]);
+        ex += a * (m[j] - mx); ey += a * (m[N + j] - my); ez += a * (m[2 * N + j] - mz);
+      };
+      if (g.Nx > 1) {
+        if (x + 1 < g.Nx) nb(i + 1, g.inv_dx2); else if (g.pbc[0]) nb(i + 1 - g.Nx, g.inv_dx2);
+        if (x > 0) nb(i - 1, g.inv_dx2); else if (g.pbc[0]) nb(i - 1 + g.Nx, g.inv_dx2);
+      }
+      if (g.Ny > 1) {
+        const long long s = g.Nx;
+        if (y + 1 < g.Ny) nb(i + s, g.inv_dy2); else if (g.pbc[1]) nb(i + s - s * g.Ny, g.inv_dy2);
+        if (y > 0) nb(i - s, g.inv_dy2); else if (g.pbc[1]) nb(i - s + s * g.Ny, g.inv_dy2);
+      }
+      if (g.Nz > 1) {
+        const long long s = (long long)g.Nx * g.Ny;
+        if (z + 1 < g.Nz) nb(i + s, g.inv_dz2); else if (g.pbc[2]) nb(i + s - s * g.Nz, g.inv_dz2);
+        if (z > 0) nb(i - s, g.inv_dz2); else if (g.pbc[2]) nb(i - s + s * g.Nz, g.inv_dz2);
+      }
+      e += 0.5f * (mx * ex + my * ey + mz * ez);
+    }
+    if (mask & MM_ANIS) {
+      if (lut->has_uniaxial) {
+        const float um = lut->u[0][r] * mx + lut->u[1][r] * my + lut->u[2][r] * mz, u2 = um * um;
+        e += 0.5f * lut->ku1[r] * u2 + 0.25f * lut->ku2[r] * u2 * u2;
+      }
+      if (lut->has_cubic) {
+        const float a1 = lut->c1[0][r] * mx + lut->c1[1][r] * my + lut->c1[2][r] * mz;
+        const float a2 = lut->c2[0][r] * mx + lut->c2[1][r] * my + lut->c2[2][r] * mz;
+        const float a3 = lut->c3[0][r] * mx + lut->c3[1][r] * my + lut->c3[2][r] * mz;
+        const float q1 = a1 * a1, q2 = a2 * a2, q3 = a3 * a3;
+        e += 0.25f * lut->kc1[r] * 2.f * (q1 * q2 + q1 * q3 + q2 * q3) + (1.f / 6.f) * lut->kc2[r] * 3.f * q1 * q2 * q3 +
+             0.125f * lut->kc3[r] * 2.f * (q1 * q1 * q2 * q2 + q1 * q1 * q3 * q3 + q2 * q2 * q3 * q3);
+      }
+    }
+    if (mask & MM_ZEEMAN) e += mx * lut->bext[0] + my * lut->bext[1] + mz * lut->bext[2];
+    acc -= (double)lut->Bsat[r] * (double)e;           // times mu0 Msat; divided by mu0 on the host
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if ((threadIdx.x & 31) == 0) atomicAdd(out, acc);
+}
+
+// max over cells of the Euclidean norm of a 3N vector field (float bits; non-negative floats order as uints)
+__global__ void k_maxnorm(long long N, const float* __restrict__ v, unsigned* __restrict__ out) {
+  float best = 0.f;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+    const float x = v[i], y = v[N + i], z = v[2 * N + i];
+    const float n = sqrtf(x * x + y * y + z * z);
+    best = (n > best || n != n) ? n : best;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const float other = __shfl_xor_sync(0xffffffffu, best, o);
+    best = (other > best || other != other) ? other : best;
+  }
+  if ((threadIdx.x & 31) == 0) atomicMax(out, (best != best) ? 0x7fc00000u : __float_as_uint(best));
+}

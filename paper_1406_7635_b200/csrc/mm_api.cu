@@ -621,6 +621,39 @@ int mm_get_avg_m(mm_sim* s, double avg[3]) {
   return MM_OK;
 }
 
+int mm_energy(mm_sim* s, unsigned mask, double* joules) {
+  int rc;
+  if ((rc = check_ready(s))) return rc;
+  if (!joules) return mm_fail(s, MM_EINVAL, "null argument");
+  mask &= MM_ALL;
+  if (mask & MM_DEMAG) launch_demag(s, R_M);
+  CUDA_TRY(s, cudaMemsetAsync(s->scratch3, 0, 3 * sizeof(double), s->stream));
+  { Launch l(s, KK_OTHER); k_energy<<<148 * 8, 256, 0, s->stream>>>(s->g, s->regions, s->luts, s->dstate, R_M, R_B, mask, s->scratch3); }
+  CUDA_TRY(s, cudaGetLastError());
+  double e = 0.0;
+  if ((rc = copy_out(s, &e, s->scratch3, sizeof(double)))) return rc;
+  *joules = e / (4e-7 * M_PI) * s->cell[0] * s->cell[1] * s->cell[2];
+  return MM_OK;
+}
+
+int mm_max_torque(mm_sim* s, double* tesla) {
+  int rc;
+  if ((rc = check_ready(s))) return rc;
+  if (!tesla) return mm_fail(s, MM_EINVAL, "null argument");
+  if ((rc = pull_state(s))) return rc;
+  launch_eval(s, R_M, R_Y, s->terms, s->precession ? 1 : 2);
+  unsigned* bits = reinterpret_cast<unsigned*>(s->scratch3);
+  CUDA_TRY(s, cudaMemsetAsync(bits, 0, sizeof(unsigned), s->stream));
+  { Launch l(s, KK_OTHER); k_maxnorm<<<148 * 8, 256, 0, s->stream>>>(s->g.N, s->hst.ptr[R_Y], bits); }
+  CUDA_TRY(s, cudaGetLastError());
+  unsigned b = 0;
+  if ((rc = copy_out(s, &b, bits, sizeof(unsigned)))) return rc;
+  float f;
+  memcpy(&f, &b, sizeof(f));
+  *tesla = (double)f;
+  return f == f ? MM_OK : mm_fail(s, MM_ENAN, "non-finite torque");
+}
+
 int mm_get_stats(mm_sim* s, long* steps, long* rejected, long* evals, size_t* peak) {
   if (!s) return MM_EINVAL;
   int rc;

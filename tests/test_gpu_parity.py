@@ -389,3 +389,17 @@ def test_precession_off_descends_in_energy(mm):
         ref.step()
     assert np.abs(sim.get_m() - ref.m).max() < 1e-4
     assert ref.energy(sim.get_m().astype(np.float64)) < e0
+
+
+def test_energy_and_max_torque(mm):
+    # Eq. 4, 8, 20, 23 and the Zeeman energy per term and in total; max |tau|/gamma (relax monitors both)
+    for grid, cell, pbc in (((64, 32, 1), (4e-9, 4e-9, 3e-9), (0, 0, 0)), ((24, 20, 6), (2e-9, 3e-9, 2e-9), (2, 0, 0))):
+        cfg = _rand_cfg(grid, cell, pbc=pbc, nreg=4, anis=True, seed=13)
+        sim = mm.from_config(cfg)
+        ref = _ref_from(cfg, "fft")
+        scale = sum(abs(ref.energy(terms=t)) for t in (MM_DEMAG, MM_EXCH, MM_ANIS, MM_ZEEMAN))
+        for mask in (MM_DEMAG, MM_EXCH, MM_ANIS, MM_ZEEMAN, MM_ALL):
+            assert abs(sim.energy(mask) - ref.energy(terms=mask)) <= 2e-6 * scale, mask
+        tr = ref.torque(ref.m) / ref.p.gamma_LL
+        tmax = np.sqrt((tr * tr).sum(axis=0)).max()
+        assert abs(sim.max_torque() - tmax) <= FIELD_TOL * tmax
