@@ -162,6 +162,13 @@ int mm_energy(mm_sim* sim, unsigned term_mask, double* joules);
  * set): the quantity relax() monitors near equilibrium (L388-L390). */
 int mm_max_torque(mm_sim* sim, double* tesla);
 
+/* The paper's relax() (L388-L392): with the precession term off and the RK23 pair, advance while the
+ * total energy keeps falling, then while the maximum torque keeps falling, decreasing MaxErr each time
+ * it stops until MaxErr = 1e-9 (sampled every 3 steps, MaxErr divided by sqrt 2: DESIGN.md #15).
+ * Solver kind, precession switch, MaxErr and fixed step are restored; time advances. Host-driven:
+ * one scalar crosses to the host per sample. */
+int mm_relax(mm_sim* sim);
+
 int mm_get_time(mm_sim* sim, double* t);
 int mm_set_time(mm_sim* sim, double t);
 /* Plain mean of m over all cells (fp64 accumulation), the paper's m.average() (L861). */

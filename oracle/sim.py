@@ -194,5 +194,44 @@ class RefSim:
             else:
                 self.step()
 
+    def max_torque(self):
+        """max over cells of |tau| / gamma_LL [T] (what relax() monitors near equilibrium)."""
+        tq = self.torque(self.m) / self.p.gamma_LL
+        return float(np.sqrt((tq * tq).sum(axis=0)).max())
+
+    def relax(self, max_batches=20000):
+        """relax() as the paper describes it (L388-L392): precession term off, RK23, adaptive step.
+        Advance while the total energy keeps falling; then monitor the maximum torque instead and
+        advance while it keeps falling; each time it stops falling decrease MaxErr, until MaxErr = 1e-9.
+        Readings (the paper gives no numbers; #15): quantities are sampled every 3 steps,
+        MaxErr is divided by sqrt(2) each time. Solver settings are restored afterwards."""
+        saved = (self.solver, self.precession, self.max_err, self.fix_dt)
+        self.set_solver_kind("rk23")
+        self.precession, self.fix_dt = False, 0.0
+        n = 3
+
+        def advance():
+            for _ in range(n):
+                self.step()
+
+        batches = 0
+        advance(); e0 = self.energy(terms=self.terms)
+        advance(); e1 = self.energy(terms=self.terms)
+        while e1 < e0 and batches < max_batches:
+            advance(); e0, e1 = e1, self.energy(terms=self.terms); batches += 1
+        t0 = self.max_torque()
+        while batches < max_batches:
+            advance(); t1 = self.max_torque(); batches += 1
+            if t1 < t0:
+                t0 = t1
+                continue
+            if self.max_err <= 1e-9:
+                break
+            self.max_err = max(self.max_err / np.sqrt(2.0), 1e-9)
+            t0 = t1
+        self.solver, self.precession, self.max_err, self.fix_dt = saved
+        self.k1 = None
+        return batches
+
     def avg_m(self):
         return self.m.reshape(3, -1).mean(axis=1)

@@ -74,6 +74,7 @@ _SIGNATURES = {
     "mm_run": (C.c_int, [C.c_void_p, C.c_double]),
     "mm_energy": (C.c_int, [C.c_void_p, C.c_uint, C.POINTER(C.c_double)]),
     "mm_max_torque": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
+    "mm_relax": (C.c_int, [C.c_void_p]),
     "mm_get_time": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
     "mm_set_time": (C.c_int, [C.c_void_p, C.c_double]),
     "mm_get_avg_m": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
@@ -276,6 +277,9 @@ class Sim:
         v = C.c_double()
         _check(lib().mm_max_torque(self._h, C.byref(v)), self._h)
         return v.value
+
+    def relax(self):
+        _check(lib().mm_relax(self._h), self._h)
 
     def set_time(self, t):
         _check(lib().mm_set_time(self._h, float(t)), self._h)

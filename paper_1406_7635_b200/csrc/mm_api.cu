@@ -1,6 +1,7 @@
 // mm_api.cu - the C ABI of include/mm.h: handle, host-side planning, launch sequences.
 // Every step of the path runs in the kernels of this directory; nothing here computes fields on
 // the host and there is no CPU fallback.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -652,6 +653,57 @@ int mm_max_torque(mm_sim* s, double* tesla) {
   memcpy(&f, &b, sizeof(f));
   *tesla = (double)f;
   return f == f ? MM_OK : mm_fail(s, MM_ENAN, "non-finite torque");
+}
+
+int mm_relax(mm_sim* s) {
+  int rc;
+  if ((rc = check_ready(s))) return rc;
+  if ((rc = pull_state(s))) return rc;
+  const int solver0 = s->solver;
+  const bool prec0 = s->precession;
+  const double err0 = s->hst.max_err, fix0 = s->hst.fix_dt;
+  if ((rc = mm_set_solver_kind(s, MM_RK23))) return rc;
+  s->precession = false;
+  s->have_k1 = false;
+  auto set_err = [&](double max_err, double fix_dt) {
+    int r = pull_state(s);
+    if (r) return r;
+    s->hst.max_err = max_err; s->hst.fix_dt = fix_dt;
+    return push_state(s);
+  };
+  auto advance = [&]() { for (int i = 0; i < 3; ++i) enqueue_step(s); };     // sampled every 3 steps (#15)
+  auto finish = [&](int code) {
+    s->precession = prec0;
+    int r = mm_set_solver_kind(s, solver0);
+    if (!r) r = set_err(err0, fix0);
+    s->have_k1 = false;
+    return code ? code : r;
+  };
+  if ((rc = set_err(err0, 0.0))) return finish(rc);
+  const long max_batches = 200000;
+  long batches = 0;
+  double e0, e1, t0, t1, max_err = err0;
+  // energy phase: advance while the total energy keeps falling (until it cuts into the noise floor)
+  advance(); if ((rc = mm_energy(s, s->terms, &e0))) return finish(rc);
+  advance(); if ((rc = mm_energy(s, s->terms, &e1))) return finish(rc);
+  while (e1 < e0 && batches++ < max_batches) {
+    advance();
+    e0 = e1;
+    if ((rc = mm_energy(s, s->terms, &e1))) return finish(rc);
+  }
+  // torque phase: advance while the maximum torque keeps falling; each time it stops, tighten MaxErr
+  if ((rc = mm_max_torque(s, &t0))) return finish(rc);
+  while (batches++ < max_batches) {
+    advance();
+    if ((rc = mm_max_torque(s, &t1))) return finish(rc);
+    if (t1 < t0) { t0 = t1; continue; }
+    if (max_err <= 1e-9) break;
+    max_err = std::max(max_err / std::sqrt(2.0), 1e-9);
+    if ((rc = set_err(max_err, 0.0))) return finish(rc);
+    t0 = t1;
+  }
+  if ((rc = pull_state(s))) return finish(rc);
+  return finish(status_to_error(s));
 }
 
 int mm_get_stats(mm_sim* s, long* steps, long* rejected, long* evals, size_t* peak) {

@@ -403,3 +403,23 @@ def test_energy_and_max_torque(mm):
         tr = ref.torque(ref.m) / ref.p.gamma_LL
         tmax = np.sqrt((tr * tr).sum(axis=0)).max()
         assert abs(sim.max_torque() - tmax) <= FIELD_TOL * tmax
+
+
+def test_relax_matches_the_oracle_equilibrium(mm):
+    # relax() (L388-L392) on a small SP4-like film from the paper's initial state m = (1, 0.1, 0) (L963)
+    grid, cell = (64, 16, 1), (4e-9, 4e-9, 3e-9)
+    p = Params.uniform(1, Msat=8e5, Aex=1.3e-11, alpha=0.5)
+    m0 = np.zeros((3, 1, 16, 64), dtype=np.float32); m0[0] = 1.0; m0[1] = 0.1
+    cfg = dict(grid=grid, cell=cell, pbc=(0, 0, 0), regions=None, params=p, m0=m0)
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    e0 = sim.energy()
+    sim.relax(); ref.relax()
+    assert sim.energy() < e0
+    assert sim.max_torque() < 1e-4                      # paper: residual torques 1e-4 .. 1e-7 T (L390)
+    assert np.abs(sim.avg_m() - ref.avg_m()).max() < 1e-3
+    assert abs(sim.energy() - ref.energy()) < 1e-4 * abs(ref.energy())
+    # settings are restored: the next step is a Dormand-Prince step with precession (6 evaluations + FSAL refresh)
+    ev = sim.stats()["evals"]
+    sim.step()
+    assert sim.stats()["evals"] - ev == 7

@@ -300,3 +300,20 @@ def test_term_mask_sums():
     sim.p.Ku1[:] = 1e5; sim.p.B_ext = np.array([0.01, -0.02, 0.03])
     parts = sum(sim.b_eff(t) for t in (MM_DEMAG, MM_EXCH, MM_ANIS, MM_ZEEMAN))
     assert np.allclose(parts, sim.b_eff(MM_ALL), rtol=1e-13, atol=1e-15)
+
+
+def test_relax_reaches_a_torque_free_state_of_lower_energy():
+    # relax() (L388-L392): the procedure's sampling details are readings (unpinned), its outcome is not:
+    # an equilibrium - lower energy, residual torque far below the paper's 1e-4..1e-7 T, nothing moves after
+    sim = RefSim((32, 8, 1), (4e-9, 4e-9, 3e-9), demag_method="fft")
+    sim.set_params(Params.uniform(1, Msat=8e5, Aex=1.3e-11, alpha=0.5))
+    m0 = np.zeros((3, 1, 8, 32)); m0[0] = 1.0; m0[1] = 0.1
+    sim.set_m(m0)
+    e0 = sim.energy()
+    sim.relax()
+    assert sim.energy() < e0 and sim.max_torque() < 1e-7
+    assert (sim.solver, sim.precession, sim.max_err, sim.fix_dt) == ("rk45", True, 1e-5, 0.0)
+    assert abs(np.sqrt((sim.m ** 2).sum(axis=0)) - 1).max() < 1e-12
+    before = sim.avg_m().copy()
+    sim.run(0.1e-9)                                   # full LLG with precession: an equilibrium stays put
+    assert np.abs(sim.avg_m() - before).max() < 1e-6
