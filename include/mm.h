@@ -80,7 +80,9 @@ typedef struct {
  * (0 = open boundary). Builds the demagnetising kernel (fp64 on the device, L143) and its
  * real, mirror-symmetric spectrum (L145); cost grows with N and with the PBC repeats.
  * Padded FFT length per open axis: the smallest 2^a 3^b 5^c >= 2N-1 (1 if N == 1), per periodic
- * axis N itself (L509), each <= 8192 (MM_EINVAL beyond, or if a periodic N is not 5-smooth).
+ * axis N itself (L509), each <= 8192 (MM_EINVAL beyond, or if a periodic N is not 5-smooth). Open
+ * one-layer films of 64..4096 cells per side use twice the next power of two instead (register-FFT
+ * kernels; any padded length >= 2N-1 gives the same linear convolution).
  * On success *out owns device memory obtained with cudaMalloc on the current device. */
 int mm_create(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, double dz, int pbc_x, int pbc_y,
               int pbc_z);
