@@ -108,7 +108,8 @@ int mm_set_terms(mm_sim* sim, unsigned term_mask);
 
 /* Implementation switches. MM_OPT_GENERIC_FFT = 1 forces the generic any-size convolution kernels
  * even where a specialised path exists (used by the tests to check the two against each other). */
-enum { MM_OPT_GENERIC_FFT = 1 };
+enum { MM_OPT_GENERIC_FFT = 1,
+       MM_OPT_NO_TMA = 2 /* fast 2D x kernels with plain loads/stores instead of TMA tensor copies */ };
 int mm_set_option(mm_sim* sim, int option, int value);
 
 /* Solver settings (L372-L374). max_err: MaxErr eps0 (default 1e-5); headroom (default 0.8);

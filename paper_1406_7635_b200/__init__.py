@@ -14,6 +14,7 @@ MM_OK, MM_EINVAL, MM_ENOMEM, MM_ECUDA, MM_ESTATE, MM_ENAN, MM_EDT = 0, -1, -2, -
 MM_DEMAG, MM_EXCH, MM_ANIS, MM_ZEEMAN, MM_ALL = 1, 2, 4, 8, 15
 MM_MAX_REGIONS = 256
 MM_OPT_GENERIC_FFT = 1
+MM_OPT_NO_TMA = 2
 MM_RK45, MM_RK23 = 0, 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))

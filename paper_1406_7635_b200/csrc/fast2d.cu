@@ -120,7 +120,8 @@ void launch_x(mm_sim* s, bool inverse, int role) {
   constexpr int GF = F::NTF / F::P::T, GI = F::NTI / F::P::T;
   const dim3 gf(s->g.Ny / (2 * GF), 3);
   const bool ragged = s->f2.nxp < s->f2.Nx;
-  if (!inverse && s->f2_tma) {
+  const bool tma_on = s->f2_tma && !s->f2_no_tma;
+  if (!inverse && tma_on) {
     const size_t b = k2_tma_store_smem<typename F::P, F::NTF>();
     if (ragged) k2_xfwd_tma<typename F::P, F::NTF, true><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd);
     else k2_xfwd_tma<typename F::P, F::NTF, false><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd);
@@ -129,7 +130,7 @@ void launch_x(mm_sim* s, bool inverse, int role) {
     if (ragged) k2_xfwd<typename F::P, F::NTF, true><<<gf, F::NTF, b, s->stream>>>(s->f2, role);
     else k2_xfwd<typename F::P, F::NTF, false><<<gf, F::NTF, b, s->stream>>>(s->f2, role);
   }
-  else if (s->f2_tma)
+  else if (tma_on)
     k2_xinv_tma<typename F::P, F::NTI><<<dim3(s->g.Ny / (2 * GI), 3), F::NTI, k2_tma_smem<typename F::P, F::NTI>(), s->stream>>>(s->f2, role, s->f2_map_inv);
   else
     k2_xinv<typename F::P, F::NTI><<<dim3(s->g.Ny / (2 * GI), 3), F::NTI, k2_smem<typename F::P, F::NTI>(), s->stream>>>(s->f2, role);

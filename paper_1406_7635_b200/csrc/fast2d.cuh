@@ -240,6 +240,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_ycol(Fast2DArgs a, int nxy) {
   constexpr int N = P::N, T = P::T, E = P::E, G = NT / T;
   extern __shared__ float4 smem4[];
   const int tid = threadIdx.x, gid = tid / T, t = tid % T;
+  __builtin_assume(t >= 0 && t < T);          // lets the mirror tests of k2_kidx fold per register slot
   char* mine = reinterpret_cast<char*>(smem4) + (size_t)gid * K2YShape<P>::GROUP_BYTES;
   float4* stash = reinterpret_cast<float4*>(mine);
   float2* xb = reinterpret_cast<float2*>(mine + (size_t)N * 16);

@@ -477,6 +477,7 @@ int mm_set_option(mm_sim* s, int option, int value) {
   if (!s) return MM_EINVAL;
   switch (option) {
     case MM_OPT_GENERIC_FFT: s->force_generic = value != 0; s->have_k1 = false; return MM_OK;
+    case MM_OPT_NO_TMA: s->f2_no_tma = value != 0; s->have_k1 = false; return MM_OK;
     default: return mm_fail(s, MM_EINVAL, "unknown option");
   }
 }

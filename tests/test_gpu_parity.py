@@ -119,8 +119,12 @@ def test_fast2d_path_fields(mm, grid):
     prof = sim.profile_read()
     sim.profile(False)
     assert "f2_ycol" in prof and "f2_xfwd" in prof and "f2_xinv" in prof and "last_xy" not in prof
-    # the generic any-size kernels must agree with it
+    # the x kernels without TMA (fallback when the driver cannot encode tensor maps) must agree exactly
     Bf = sim.b_eff(MM_DEMAG)
+    sim.set_option(mm.MM_OPT_NO_TMA, 1)
+    assert np.array_equal(sim.b_eff(MM_DEMAG), Bf)
+    sim.set_option(mm.MM_OPT_NO_TMA, 0)
+    # the generic any-size kernels must agree with it
     sim.set_option(mm.MM_OPT_GENERIC_FFT, 1)
     Bg = sim.b_eff(MM_DEMAG)
     assert np.abs(Bf - Bg).max() <= 2e-5 * np.abs(Bg).max()
