@@ -33,8 +33,18 @@ BS_B3 = (2 / 9, 1 / 3, 4 / 9, 0.0)
 BS_B2 = (7 / 24, 1 / 4, 1 / 3, 1 / 8)
 BS_E = tuple(b3 - b2 for b3, b2 in zip(BS_B3, BS_B2))
 
-# solver -> (a rows, error weights, exponent of the step-size rule = 1 / order of the solution)
-SOLVERS = {"rk45": (DP_A, DP_E, 1 / 5), "rk23": (BS_A, BS_E, 1 / 3)}
+# Heun 2(1), 2 stages, no FSAL ("RK12, Heun's method, 2nd order convergence and a 1st order error estimate
+# ... used for finite temperature simulations"): result m0 + h (k1 + k2) / 2
+HEUN_A = ((), (1.0,))
+HEUN_B2 = (1 / 2, 1 / 2)
+HEUN_E = (1 / 2 - 1.0, 1 / 2)            # b(2nd) - b(1st, Euler)
+
+# solver -> (a rows, error weights, exponent of the step-size rule = 1 / order of the solution,
+#            weights of the result if the last stage input is not the result (no FSAL))
+SOLVERS = {"rk45": (DP_A, DP_E, 1 / 5, None), "rk23": (BS_A, BS_E, 1 / 3, None),
+           "rk12": (HEUN_A, HEUN_E, 1 / 2, HEUN_B2)}
+
+K_BOLTZMANN = 1.380649e-23               # J/K
 
 DIRECT_SUM_MAX_CELLS = 2048
 
@@ -66,9 +76,35 @@ class RefSim:
         self.terms = MM_ALL
         self.solver = "rk45"
         self.precession = True
+        self.temp, self.seed = 0.0, 0
+
+    def set_temperature(self, temp, seed=0):
+        """Thermal field of Eq. 24 (L303-L310) at `temp` kelvin; eta comes from the counter-based
+        generator synth.rng (seed, component stream, step * N + cell). Needs a fixed step and the
+        Heun solver (L310)."""
+        self.temp, self.seed = float(temp), int(seed)
+        self.k1 = None
+
+    def b_thermal(self, h):
+        """Eq. 24: eta * sqrt(2 mu0 alpha kB T / (Bsat gamma dV dt)); one eta per cell, component, step."""
+        from synth import rng
+        n = self.ncells
+        idx = np.uint64(self.n_steps + self.n_rejected) * np.uint64(n) + np.arange(n, dtype=np.uint64)
+        eta = np.empty((3, n))
+        for c in range(3):
+            u1 = rng.uniform01(self.seed, c, idx)
+            u2 = rng.uniform01(self.seed, 3 + c, idx)
+            eta[c] = np.sqrt(-2.0 * np.log(1.0 - u1)) * np.cos(2.0 * np.pi * u2)       # Box-Muller
+        Bsat = fld.MU0 * self.p.Msat[self.regions]
+        alpha = self.p.alpha[self.regions]
+        dV = self.cell[0] * self.cell[1] * self.cell[2]
+        with np.errstate(divide="ignore", invalid="ignore"):
+            amp = np.sqrt(2.0 * fld.MU0 * alpha * K_BOLTZMANN * self.temp / (Bsat * self.p.gamma_LL * dV * h))
+        amp = np.where(Bsat > 0, amp, 0.0)
+        return eta.reshape((3,) + self.shape) * amp[None]
 
     def set_solver_kind(self, name):
-        """"rk45" (default) or "rk23" (L366). Invalidates the FSAL slope."""
+        """"rk45" (default), "rk23" (L366) or "rk12" (Heun, L367). Invalidates the FSAL slope."""
         assert name in SOLVERS
         self.solver = name
         self.k1 = None
@@ -126,11 +162,11 @@ class RefSim:
             B += np.asarray(self.p.B_ext, dtype=np.float64)[:, None, None, None]
         return B
 
-    def torque(self, m):
-        """dm/dt [1/s] (Eq. 1-2)."""
+    def torque(self, m, b_extra=0.0):
+        """dm/dt [1/s] (Eq. 1-2); b_extra: an additional field term (the thermal field of the step)."""
         self.n_eval += 1
         alpha = self.p.alpha[self.regions]
-        return self.p.gamma_LL * fld.ll_torque_over_gamma(m, self.b_eff(self.terms, m), alpha, self.precession)
+        return self.p.gamma_LL * fld.ll_torque_over_gamma(m, self.b_eff(self.terms, m) + b_extra, alpha, self.precession)
 
     # ---- energies (Eq. 4, 8, 20, 23; Zeeman -M.B_ext), joules
     def energy(self, m=None, terms=MM_ALL):
@@ -154,23 +190,31 @@ class RefSim:
 
     # ---- one attempted Runge-Kutta step of the selected embedded pair
     def step(self, dt_force=None):
-        A, E, expo = SOLVERS[self.solver]
+        A, E, expo, B = SOLVERS[self.solver]
         ns = len(A)
-        if self.k1 is None:
-            self.k1 = self.torque(self.m)
         h = self.dt if dt_force is None else dt_force
+        bth = 0.0
+        if self.temp > 0:
+            assert self.fix_dt > 0 and self.solver == "rk12", "thermal field: fixed step and Heun only (L310)"
+            bth = self.b_thermal(h)                    # constant during the step, new after it (L308)
+            self.k1 = None                             # no torque continuity between steps
+        if self.k1 is None:
+            self.k1 = self.torque(self.m, bth)
         m0 = self.m
         k = [self.k1]
         y = None
         for i in range(1, ns):
             y = _normalise(m0 + h * sum(a * kj for a, kj in zip(A[i], k)))       # every stage input
-            k.append(self.torque(y))                                              # is renormalised (#9)
+            k.append(self.torque(y, bth))                                         # is renormalised (#9)
         err_vec = sum(e * kj for e, kj in zip(E, k))
         err = h * np.sqrt((err_vec * err_vec).sum(axis=0)).max()
         fixed = self.fix_dt > 0
         accepted = fixed or (err <= self.max_err)
         if accepted:
-            self.m, self.k1 = y, k[ns - 1]       # last stage input = the high-order result; FSAL
+            if B is None:
+                self.m, self.k1 = y, k[ns - 1]   # last stage input = the high-order result; FSAL
+            else:
+                self.m, self.k1 = _normalise(m0 + h * sum(b * kj for b, kj in zip(B, k))), None
             self.t += h
             self.n_steps += 1
         else:

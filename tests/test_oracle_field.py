@@ -317,3 +317,57 @@ def test_relax_reaches_a_torque_free_state_of_lower_energy():
     before = sim.avg_m().copy()
     sim.run(0.1e-9)                                   # full LLG with precession: an equilibrium stays put
     assert np.abs(sim.avg_m() - before).max() < 1e-6
+
+
+def test_heun_second_order_convergence_and_adaptive_rule():
+    # RK12 (L367): 2nd-order solution, 1st-order (Euler) embedded estimate; Fig. 10 shows its 2nd-order slope
+    assert abs(sum(osim.HEUN_B2) - 1) < 1e-15 and abs(sum(osim.HEUN_E)) < 1e-15
+    assert abs(osim.HEUN_B2[1] * osim.HEUN_A[1][0] - 0.5) < 1e-15                  # order-2 condition b2 c2 = 1/2
+    period = 2 * np.pi / (0.1 * GAMMA)
+    errs = []
+    for n in (100, 200, 400):
+        sim = _macrospin(m0=(1, 0, 1))
+        sim.set_solver_kind("rk12")
+        sim.set_solver(fix_dt=period / n)
+        for _ in range(n):
+            sim.step()
+        errs.append(np.linalg.norm(sim.m[:, 0, 0, 0] - np.array([1, 0, 1]) / np.sqrt(2)))
+    assert 3.8 < errs[0] / errs[1] < 4.2 and 3.9 < errs[1] / errs[2] < 4.1       # 2^2
+    sim = _macrospin(m0=(1, 0, 1))
+    sim.set_solver_kind("rk12")
+    sim.set_solver(max_err=1e-6, dt_init=1e-13)
+    sim.run(period)
+    assert abs(sim.t - period) < 1e-24 and sim.n_eval == 2 * sim.n_steps + sim.n_rejected   # no FSAL; k1 survives a rejection
+
+
+def test_thermal_field_amplitude_and_langevin_equilibrium():
+    # Eq. 24 (L303-L308). (i) the field of one step has zero mean and the standard deviation of the formula,
+    # is reproducible from (seed, step) and changes with the step; (ii) an ensemble of uncoupled macrospins
+    # in a field B reaches the Boltzmann distribution: <m_z> = coth(xi) - 1/xi, <m_z^2> = 1 - 2 <m_z>/xi,
+    # xi = Msat V B / kT - which fixes the amplitude (twice the variance would give <m_z> = 0.60, not 0.79).
+    n, Ms, B, T, c, dt = 64, 1e6, 0.02, 300.0, 10e-9, 2e-12
+    sim = RefSim((n, n, 1), (c, c, c))
+    sim.set_params(Params.uniform(1, Msat=Ms, Aex=0.0, alpha=1.0, B_ext=(0, 0, B)))
+    sim.set_terms(MM_ZEEMAN)
+    m = np.zeros((3, 1, n, n)); m[2] = 1.0
+    sim.set_m(m)
+    sim.set_solver_kind("rk12")
+    sim.set_temperature(T, seed=7)
+    with pytest.raises(AssertionError):
+        sim.step()                                    # adaptive step + thermal field is refused (L310)
+    sim.set_solver(fix_dt=dt)
+    b0 = sim.b_thermal(dt)
+    amp = np.sqrt(2 * fld.MU0 * 1.0 * 1.380649e-23 * T / (fld.MU0 * Ms * GAMMA * c ** 3 * dt))
+    assert abs(b0.mean()) < 0.03 * amp and abs(b0.std() / amp - 1) < 0.02
+    assert np.array_equal(b0, sim.b_thermal(dt))
+    acc1, acc2 = [], []
+    for i in range(4000):
+        sim.step()
+        if i == 0:
+            assert not np.array_equal(b0, sim.b_thermal(dt))
+        if i > 1500 and i % 10 == 0:
+            acc1.append(sim.avg_m()[2]); acc2.append((sim.m[2] ** 2).mean())
+    xi = Ms * c ** 3 * B / (1.380649e-23 * T)
+    L = 1 / np.tanh(xi) - 1 / xi
+    assert abs(np.mean(acc1) - L) < 0.01 and abs(np.mean(acc2) - (1 - 2 * L / xi)) < 0.012
+    assert abs(np.sqrt((sim.m ** 2).sum(axis=0)) - 1).max() < 1e-12
