@@ -123,8 +123,15 @@ int mm_set_solver(mm_sim* sim, double max_err, double headroom, double fix_dt, d
  * L805, L853): MM_RK45 = Dormand-Prince 5(4), 7 stages, the default for dynamics (L365); MM_RK23 =
  * Bogacki-Shampine 3(2), 4 stages, used when relaxing (L366, L392). Both are FSAL; the step-size rule
  * uses the exponent 1/5 resp. 1/3. Invalidates the FSAL slope. */
-enum { MM_RK45 = 0, MM_RK23 = 1 };
+enum { MM_RK45 = 0, MM_RK23 = 1, MM_RK12 = 2 /* Heun 2(1), no FSAL: finite temperature (L367) */ };
 int mm_set_solver_kind(mm_sim* sim, int kind);
+
+/* Temperature in kelvin (default 0): inside steps adds the fluctuating field of Eq. 24 (L303-L308),
+ * B_therm = eta sqrt(2 mu0 alpha kB T / (Bsat gamma_LL dV dt)), eta standard normal per cell, component and
+ * step from a counter-based generator (seed, component, step * N + cell). As the paper requires (L310) a
+ * temperature needs the Heun solver and a fixed step: stepping otherwise returns MM_ESTATE.
+ * mm_b_eff / mm_torque never include the thermal field. */
+int mm_set_temperature(mm_sim* sim, double kelvin, unsigned long long seed);
 
 /* Precession term of Eq. 2 on (default) or off: off leaves tau = -gamma alpha/(1+alpha^2) m x (m x B),
  * "so that the effective field points towards decreasing energy" (relax(), L388). */

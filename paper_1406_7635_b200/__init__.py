@@ -15,7 +15,7 @@ MM_DEMAG, MM_EXCH, MM_ANIS, MM_ZEEMAN, MM_ALL = 1, 2, 4, 8, 15
 MM_MAX_REGIONS = 256
 MM_OPT_GENERIC_FFT = 1
 MM_OPT_NO_TMA = 2
-MM_RK45, MM_RK23 = 0, 1
+MM_RK45, MM_RK23, MM_RK12 = 0, 1, 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmm_b200.so")
@@ -69,6 +69,7 @@ _SIGNATURES = {
     "mm_torque": (C.c_int, [C.c_void_p, C.c_void_p]),
     "mm_set_solver_kind": (C.c_int, [C.c_void_p, C.c_int]),
     "mm_set_precession": (C.c_int, [C.c_void_p, C.c_int]),
+    "mm_set_temperature": (C.c_int, [C.c_void_p, C.c_double, C.c_ulonglong]),
     "mm_step_rk45": (C.c_int, [C.c_void_p, C.POINTER(mm_step_info)]),
     "mm_step": (C.c_int, [C.c_void_p, C.POINTER(mm_step_info)]),
     "mm_steps": (C.c_int, [C.c_void_p, C.c_int]),
@@ -219,6 +220,9 @@ class Sim:
     def set_solver_kind(self, kind):
         """MM_RK45 (default) or MM_RK23."""
         _check(lib().mm_set_solver_kind(self._h, int(kind)), self._h)
+
+    def set_temperature(self, kelvin, seed=0):
+        _check(lib().mm_set_temperature(self._h, float(kelvin), int(seed)), self._h)
 
     def set_precession(self, on):
         _check(lib().mm_set_precession(self._h, 1 if on else 0), self._h)

@@ -5,6 +5,7 @@
 #include <stddef.h>
 #include "../../include/mm.h"
 
+#define MM_THERMAL 16u   /* internal term bit: thermal field of the current step (never part of MM_ALL) */
 #define MM_TRI_ENTRIES (MM_MAX_REGIONS * (MM_MAX_REGIONS + 1) / 2)
 
 // ---- buffer roles: every kernel fetches its array pointers from DevState::ptr[role], so that the
@@ -23,7 +24,11 @@ struct DevState {
   float hg;          // gamma * h as float (torque slopes are kept in tesla)
   unsigned err_bits; // float bits of max || sum_j e_j k_j ||  (atomicMax; non-negative floats order as uints)
   float last_err;
-  int nstage;        // stages of the embedded pair: 7 (Dormand-Prince) or 4 (Bogacki-Shampine)
+  int nstage;        // stages of the embedded pair: 7 (Dormand-Prince), 4 (Bogacki-Shampine), 2 (Heun)
+  int nevals;        // torque evaluations per attempted step: 6, 3, 2
+  double temperature;            // kelvin; > 0 adds the thermal field of Eq. 24 inside steps
+  unsigned long long seed;       // of the counter-based generator behind eta
+  float therm_scale;             // sqrt(T / h) of the current attempt
   double expo;       // exponent of the step-size rule: 1/5 or 1/3
   int run_mode;      // 1: stop at t_end
   int clipped;       // current attempt was clipped to land on t_end
@@ -39,6 +44,7 @@ struct Luts {
   float Bsat[MM_MAX_REGIONS];   // mu0 * Msat [T]
   float alpha[MM_MAX_REGIONS];
   float live[MM_MAX_REGIONS];   // 1 if Msat > 0 else 0
+  float therm[MM_MAX_REGIONS];  // sqrt(2 mu0 alpha kB / (Bsat gamma dV)) [T sqrt(s/K)]   (Eq. 24 without T and dt)
   float ku1[MM_MAX_REGIONS];    // 2 Ku1 / Msat [T]           (Eq. 18)
   float ku2[MM_MAX_REGIONS];    // 4 Ku2 / Msat [T]
   float u[3][MM_MAX_REGIONS];

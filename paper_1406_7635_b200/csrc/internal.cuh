@@ -49,6 +49,7 @@ struct mm_sim {
   unsigned terms = MM_ALL;
   int solver = MM_RK45;
   bool precession = true;
+  double temperature = 0.0;
   int nregions = 1;
   long launches = 0;
   long extra_evals = 0;

@@ -7,6 +7,25 @@ __device__ __forceinline__ int tri_index(int a, int b) {  // lower-triangular ta
   return i * (i + 1) / 2 + j;
 }
 
+// Standard normal eta(seed, component, counter) of the thermal field (Eq. 24): the counter-based generator
+// of synth/rng.py restated (splitmix64 finaliser over seed, stream, index; 53-bit uniforms; Box-Muller)
+// in fp64, so that both sides draw the same numbers.
+__device__ __forceinline__ unsigned long long mm_mix64(unsigned long long z) {
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+__device__ __forceinline__ double mm_uniform01(unsigned long long seed, unsigned long long stream, unsigned long long index) {
+  unsigned long long z = mm_mix64(seed + 0x9E3779B97F4A7C15ull);
+  z = mm_mix64(z ^ (stream * 0xD1B54A32D192ED03ull));
+  z = mm_mix64(z + index * 0x9E3779B97F4A7C15ull);
+  return (double)(z >> 11) * (1.0 / 9007199254740992.0);
+}
+__device__ __forceinline__ float mm_eta(unsigned long long seed, int comp, unsigned long long index) {
+  const double u1 = mm_uniform01(seed, comp, index), u2 = mm_uniform01(seed, 3 + comp, index);
+  return (float)(sqrt(-2.0 * log(1.0 - u1)) * cospi(2.0 * u2));
+}
+
 // B_eff = [B_demag] + B_exch (Eq. 6 / Eq. 9) + B_anis (Eq. 18, 21) + B_ext, then either stored as the
 // field (out_torque = 0) or turned into the torque over gamma (Eq. 2, sign reading DESIGN.md #5).
 // One thread per cell; x fastest so every global access of a warp is one contiguous segment.
@@ -71,6 +90,11 @@ __global__ void k_local(Geometry g, const uint8_t* __restrict__ regions, const L
     }
   }
   if (mask & MM_ZEEMAN) { bx += lut->bext[0]; by += lut->bext[1]; bz += lut->bext[2]; }
+  if (mask & MM_THERMAL) {     // Eq. 24: one eta per cell, component and step
+    const float amp = lut->therm[r] * st->therm_scale;
+    const unsigned long long idx = (unsigned long long)(st->steps + st->rejected) * (unsigned long long)N + (unsigned long long)i;
+    bx += amp * mm_eta(st->seed, 0, idx); by += amp * mm_eta(st->seed, 1, idx); bz += amp * mm_eta(st->seed, 2, idx);
+  }
   if (out_torque) {
     const float al = lut->alpha[r];
     const float pre = -lut->live[r] / (1.f + al * al);
@@ -195,6 +219,11 @@ __global__ void __launch_bounds__(128) k_local4(Geometry g, const uint8_t* __res
       bz += f1 * c1z + f2 * c2z + f3 * c3z;
     }
     if (mask & MM_ZEEMAN) { bx += lut->bext[0]; by += lut->bext[1]; bz += lut->bext[2]; }
+    if (mask & MM_THERMAL) {   // Eq. 24: one eta per cell, component and step
+      const float amp = lut->therm[rr] * st->therm_scale;
+      const unsigned long long idx = (unsigned long long)(st->steps + st->rejected) * (unsigned long long)N + (unsigned long long)(i + l);
+      bx += amp * mm_eta(st->seed, 0, idx); by += amp * mm_eta(st->seed, 1, idx); bz += amp * mm_eta(st->seed, 2, idx);
+    }
     if (out_torque) {
       const float al = lut->alpha[rr];
       const float pre = -lut->live[rr] / (1.f + al * al);
@@ -278,6 +307,7 @@ __global__ void k_ctrl_begin(DevState* st) {
   st->skip = 0;
   st->h = h;
   st->hg = (float)(st->gamma * h);
+  st->therm_scale = (float)sqrt(st->temperature / h);
   st->err_bits = 0u;
 }
 
@@ -290,7 +320,7 @@ __global__ void k_ctrl_end(DevState* st) {
   const double h = st->h;
   const double err = (double)emax * st->gamma * h;
   st->last_err = (float)err;
-  st->evals += st->nstage - 1;
+  st->evals += st->nevals;
   if (!(err == err) || isinf(err)) { st->status = MM_ENAN; st->last_accepted = 0; st->skip = 1; return; }
   const bool fixed = st->fix_dt > 0;
   const bool accept = fixed || err <= st->max_err;

@@ -191,9 +191,31 @@ void launch_eval(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_t
 
 void enqueue_step(mm_sim* s) {
   const long long N = s->g.N;
+  const int tq = s->precession ? 1 : 2;                       // torque with / without the precession term
+  if (s->solver == MM_RK12) {
+    // Heun (L367): y = m + h k1, k2 = tau(y), result m + h (k1 + k2) / 2; no FSAL. With a temperature the
+    // thermal field of Eq. 24 is part of both evaluations and changes with the step counter, so k1 is
+    // evaluated after k_ctrl_begin has fixed h (the field's amplitude depends on it).
+    const unsigned mask = s->terms | (s->temperature > 0 ? MM_THERMAL : 0u);
+    { Launch l(s, KK_CTRL); k_ctrl_begin<<<1, 1, 0, s->stream>>>(s->dstate); }
+    launch_eval(s, R_M, R_K0, mask, tq);
+    StageCoef sc;
+    for (int j = 0; j < 6; ++j) sc.a[j] = 0.f;
+    sc.n = 1; sc.a[0] = 1.f;
+    { Launch l(s, KK_STAGE); k_stage<<<blocks_for(N, 256), 256, 0, s->stream>>>(N, s->dstate, sc, R_Y); }
+    launch_eval(s, R_Y, R_K1, mask, tq);
+    sc.n = 2; sc.a[0] = 0.5f; sc.a[1] = 0.5f;
+    { Launch l(s, KK_STAGE); k_stage<<<blocks_for(N, 256), 256, 0, s->stream>>>(N, s->dstate, sc, R_MNEW); }
+    ErrCoef ec;
+    for (int j = 0; j < 7; ++j) ec.e[j] = 0.f;
+    ec.e[0] = -0.5f; ec.e[1] = 0.5f;                          // 2nd-order minus Euler weights
+    { Launch l(s, KK_ERROR); k_error<<<148 * 8, 256, 0, s->stream>>>(N, s->dstate, ec); }
+    { Launch l(s, KK_CTRL); k_ctrl_end<<<1, 1, 0, s->stream>>>(s->dstate); }
+    s->have_k1 = false;
+    return;
+  }
   const bool bs = s->solver == MM_RK23;
   const int ns = bs ? 4 : 7;                                  // stages; the last one is the FSAL evaluation
-  const int tq = s->precession ? 1 : 2;                       // torque with / without the precession term
   if (!s->have_k1) {
     launch_eval(s, R_M, R_K0, s->terms, tq);
     s->have_k1 = true;
@@ -212,6 +234,13 @@ void enqueue_step(mm_sim* s) {
   for (int j = 0; j < 7; ++j) ec.e[j] = (float)(bs ? BS_E[j] : DP_E[j]);
   { Launch l(s, KK_ERROR); k_error<<<148 * 8, 256, 0, s->stream>>>(N, s->dstate, ec); }
   { Launch l(s, KK_CTRL); k_ctrl_end<<<1, 1, 0, s->stream>>>(s->dstate); }
+}
+
+// thermal field: Heun and a fixed step only (L310)
+int check_thermal(mm_sim* s) {
+  if (s->temperature > 0 && (s->solver != MM_RK12 || !(s->hst.fix_dt > 0)))
+    return mm_fail(s, MM_ESTATE, "a temperature needs the Heun solver (MM_RK12) and a fixed step (PAPER.md L310)");
+  return MM_OK;
 }
 
 int check_ready(mm_sim* s) {
@@ -342,7 +371,7 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
   for (int r = 0; r < R_COUNT; ++r) h.ptr[r] = s->field[r];
   h.max_err = 1e-5; h.headroom = 0.8; h.fix_dt = 0.0; h.dt = 1e-14; h.dt_min = 1e-18; h.dt_max = 1e-9;
   h.gamma = 1.7595e11;
-  h.nstage = 7; h.expo = 0.2;
+  h.nstage = 7; h.nevals = 6; h.expo = 0.2;
   h.status = MM_OK;
   if ((rc = push_state(s))) { std::string m = s->err; return bail(rc, m.c_str()); }
   *out = s;
@@ -409,6 +438,10 @@ int mm_set_params(mm_sim* s, const mm_params* p) {
     L->Bsat[r] = (float)(mu0 * Ms);
     L->alpha[r] = (float)p->alpha[r];
     L->live[r] = Ms > 0 ? 1.f : 0.f;
+    {   // Eq. 24 without T and dt: sqrt(2 mu0 alpha kB / (Bsat gamma dV))
+      const double gam = p->gamma_LL > 0 ? p->gamma_LL : 1.7595e11, dV = s->cell[0] * s->cell[1] * s->cell[2];
+      L->therm[r] = Ms > 0 && p->alpha[r] > 0 ? (float)std::sqrt(2.0 * mu0 * p->alpha[r] * 1.380649e-23 / (mu0 * Ms * gam * dV)) : 0.f;
+    }
     L->ku1[r] = (float)(2.0 * p->Ku1[r] * iMs);
     L->ku2[r] = (float)(4.0 * p->Ku2[r] * iMs);
     L->kc1[r] = (float)(-2.0 * p->Kc1[r] * iMs);
@@ -454,12 +487,25 @@ int mm_set_terms(mm_sim* s, unsigned mask) {
 
 int mm_set_solver_kind(mm_sim* s, int kind) {
   if (!s) return MM_EINVAL;
-  if (kind != MM_RK45 && kind != MM_RK23) return mm_fail(s, MM_EINVAL, "unknown solver");
+  if (kind != MM_RK45 && kind != MM_RK23 && kind != MM_RK12) return mm_fail(s, MM_EINVAL, "unknown solver");
   int rc;
   if ((rc = pull_state(s))) return rc;
   s->solver = kind;
-  s->hst.nstage = kind == MM_RK23 ? 4 : 7;
-  s->hst.expo = kind == MM_RK23 ? 1.0 / 3.0 : 0.2;
+  s->hst.nstage = kind == MM_RK23 ? 4 : (kind == MM_RK12 ? 2 : 7);
+  s->hst.nevals = kind == MM_RK23 ? 3 : (kind == MM_RK12 ? 2 : 6);
+  s->hst.expo = kind == MM_RK23 ? 1.0 / 3.0 : (kind == MM_RK12 ? 0.5 : 0.2);
+  s->have_k1 = false;
+  return push_state(s);
+}
+
+int mm_set_temperature(mm_sim* s, double kelvin, unsigned long long seed) {
+  if (!s) return MM_EINVAL;
+  if (!(kelvin >= 0) || !std::isfinite(kelvin)) return mm_fail(s, MM_EINVAL, "bad temperature");
+  int rc;
+  if ((rc = pull_state(s))) return rc;
+  s->temperature = kelvin;
+  s->hst.temperature = kelvin;
+  s->hst.seed = seed;
   s->have_k1 = false;
   return push_state(s);
 }
@@ -544,7 +590,7 @@ int mm_torque(mm_sim* s, float* out) {
 
 int mm_step_rk45(mm_sim* s, mm_step_info* info) {
   int rc;
-  if ((rc = check_ready(s))) return rc;
+  if ((rc = check_ready(s)) || (rc = check_thermal(s))) return rc;
   enqueue_step(s);
   CUDA_TRY(s, cudaGetLastError());
   if (!info) return MM_OK;
@@ -557,7 +603,7 @@ int mm_step_rk45(mm_sim* s, mm_step_info* info) {
 
 int mm_steps(mm_sim* s, int n) {
   int rc;
-  if ((rc = check_ready(s))) return rc;
+  if ((rc = check_ready(s)) || (rc = check_thermal(s))) return rc;
   if (n < 0) return mm_fail(s, MM_EINVAL, "negative step count");
   for (int i = 0; i < n; ++i) enqueue_step(s);
   CUDA_TRY(s, cudaGetLastError());
@@ -567,7 +613,7 @@ int mm_steps(mm_sim* s, int n) {
 
 int mm_run(mm_sim* s, double duration) {
   int rc;
-  if ((rc = check_ready(s))) return rc;
+  if ((rc = check_ready(s)) || (rc = check_thermal(s))) return rc;
   if (!(duration >= 0) || !std::isfinite(duration)) return mm_fail(s, MM_EINVAL, "bad duration");
   if (duration == 0) return MM_OK;
   if ((rc = pull_state(s))) return rc;

@@ -481,3 +481,71 @@ def test_sp3_ground_state_transitions_printed_in_the_paper(mm):
     assert relaxed_energy(8.3, "flower")[1][2] > 0.96
     mv = relaxed_energy(8.5, "vortex")[1]
     assert abs(mv[2]) < 1e-3 and 0.3 < abs(mv[0]) < 0.4
+
+
+# --------------------------------------------------------------------------- Heun and the thermal field
+def test_heun_and_thermal_field_trajectory(mm):
+    # RK12 (L367) with and without the fluctuating field of Eq. 24: both sides draw eta from the same
+    # counter-based generator, so even the stochastic trajectory must agree cell by cell
+    cfg = _rand_cfg((32, 8, 1), (4e-9, 4e-9, 3e-9), nreg=2, anis=True, seed=17)
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    sim.set_solver_kind(mm.MM_RK12); ref.set_solver_kind("rk12")
+    sim.set_solver(fix_dt=2e-14); ref.set_solver(fix_dt=2e-14)
+    sim.steps(30)
+    for _ in range(30):
+        ref.step()
+    assert np.abs(sim.get_m() - ref.m).max() < 2e-5
+    sim.set_temperature(300.0, seed=99); ref.set_temperature(300.0, seed=99)
+    e0 = sim.stats()["evals"]
+    sim.steps(40)
+    for _ in range(40):
+        ref.step()
+    assert np.abs(sim.get_m() - ref.m).max() < 1e-4
+    assert sim.stats()["evals"] - e0 == 2 * 40
+    assert abs(np.linalg.norm(sim.get_m().reshape(3, -1), axis=0) - 1).max() < 1e-6
+    # the paper's solver constraints (L310): no adaptive step, no RK45 with a temperature
+    sim.set_solver(fix_dt=0.0)
+    with pytest.raises(mm.MMError):
+        sim.step()
+    sim.set_solver(fix_dt=2e-14)
+    sim.set_solver_kind(mm.MM_RK45)
+    with pytest.raises(mm.MMError):
+        sim.step()
+    sim.set_temperature(0.0)
+    sim.step()
+
+
+def test_thermal_equilibrium_and_switching_rate(mm):
+    # (i) Langevin law of an ensemble of uncoupled macrospins in a field (closed form, as in the oracle's
+    # pin); (ii) the paper's own verification (Fig. 8, script L790-L810): thermal switching rate of a
+    # uniaxial macrospin against Eq. 25 (L316), f = gamma alpha/(1+alpha^2) sqrt(8 K^3 V / (2 pi Msat^2 kT)) e^{-KV/kT}
+    kB, gam = 1.380649e-23, 1.7595e11
+    n, Ms, c = 256, 1e6, 10e-9
+    m0 = np.zeros((3, 1, n, n), dtype=np.float32); m0[2] = 1.0
+    B, T, dt = 0.02, 300.0, 2e-12
+    p = Params.uniform(1, Msat=Ms, Aex=0.0, alpha=1.0, B_ext=(0, 0, B))
+    sim = mm.from_config(dict(grid=(n, n, 1), cell=(c, c, c), pbc=(0, 0, 0), regions=None, params=p, m0=m0))
+    sim.set_terms(MM_ZEEMAN)
+    sim.set_solver_kind(mm.MM_RK12); sim.set_solver(fix_dt=dt); sim.set_temperature(T, seed=3)
+    sim.steps(1500)
+    acc = []
+    for _ in range(50):
+        sim.steps(50)
+        acc.append(sim.avg_m()[2])
+    xi = Ms * c ** 3 * B / (kB * T)
+    assert abs(np.mean(acc) - (1 / np.tanh(xi) - 1 / xi)) < 0.005
+    # (ii) all spins up in a uniaxial well, no field: <m_z> decays as exp(-2 f t) (two-state relaxation)
+    K, alpha, T, dt = 1e4, 0.1, 150.0, 1e-12
+    p = Params.uniform(1, Msat=Ms, Aex=0.0, alpha=alpha, Ku1=K, anisU=(0, 0, 1))
+    sim = mm.from_config(dict(grid=(n, n, 1), cell=(c, c, c), pbc=(0, 0, 0), regions=None, params=p, m0=m0))
+    sim.set_terms(MM_ANIS)
+    sim.set_solver_kind(mm.MM_RK12); sim.set_solver(fix_dt=dt); sim.set_temperature(T, seed=5)
+    sim.steps(5000)                                   # equilibrate inside the well (5 ns)
+    t0, z0 = sim.t, sim.avg_m()[2]
+    sim.steps(60000)
+    t1, z1 = sim.t, sim.avg_m()[2]
+    f_meas = np.log(z0 / z1) / (2 * (t1 - t0))
+    V = c ** 3
+    f_eq25 = gam * alpha / (1 + alpha ** 2) * np.sqrt(8 * K ** 3 * V / (2 * np.pi * Ms ** 2 * kB * T)) * np.exp(-K * V / (kB * T))
+    assert 0.7 < f_meas / f_eq25 < 1.3, (f_meas, f_eq25)
