@@ -472,6 +472,11 @@ def test_sp3_ground_state_transitions_printed_in_the_paper(mm):
         assert d0 * d1 < 0, (kind_a, kind_b, d0, d1)
         return L0 + (L1 - L0) * d0 / (d0 - d1)
 
+    # parity with the oracle's own relaxed energies at the same edge lengths (stored: 25 min of fp64 relax)
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "sp3_oracle_energies.txt")):
+        if not line.startswith("#"):
+            L, kind, val = line.split()[:3]
+            assert abs(relaxed_energy(float(L), kind)[0] - float(val)) < 2e-6, (L, kind)
     Lv = crossing("twisted", "vortex", 8.44, 8.50)
     assert abs(Lv - gold["twisted_flower_to_vortex"]) < 0.02, Lv
     Lt = crossing("twisted", "flower", 8.12, 8.20)

@@ -371,3 +371,23 @@ def test_thermal_field_amplitude_and_langevin_equilibrium():
     L = 1 / np.tanh(xi) - 1 / xi
     assert abs(np.mean(acc1) - L) < 0.01 and abs(np.mean(acc2) - (1 - 2 * L / xi)) < 0.012
     assert abs(np.sqrt((sim.m ** 2).sum(axis=0)) - 1).max() < 1e-12
+
+
+def test_sp3_vortex_transition_from_the_stored_oracle_energies():
+    # Standard problem 3 (L414-L428): the oracle's relaxed twisted-flower and vortex energies (stored by
+    # tests/golden/make_sp3_oracle.py, which calls only oracle/ - 25 minutes of relax() in fp64) must cross
+    # at the edge length the paper prints, L = 8.47 (L426, tests/golden/sp3_transitions.txt). This pins
+    # relax(), the energies and the 3D field terms of the oracle to a number printed in the paper.
+    import os
+    g = os.path.join(os.path.dirname(__file__), "golden")
+    e = {}
+    for line in open(os.path.join(g, "sp3_oracle_energies.txt")):
+        if not line.startswith("#"):
+            L, kind, val = line.split()[:3]
+            e[(float(L), kind)] = float(val)
+    paper = {l.split()[0]: float(l.split()[1]) for l in open(os.path.join(g, "sp3_transitions.txt"))
+             if l.strip() and not l.startswith("#")}
+    d0 = e[(8.44, "twisted")] - e[(8.44, "vortex")]
+    d1 = e[(8.50, "twisted")] - e[(8.50, "vortex")]
+    assert d0 < 0 < d1
+    assert abs(8.44 + 0.06 * d0 / (d0 - d1) - paper["twisted_flower_to_vortex"]) < 0.01
