@@ -109,8 +109,9 @@ __global__ void k_local(Geometry g, const uint8_t* __restrict__ regions, const L
 // Same computation, four consecutive x cells per thread (Nx % 4 == 0): 16-byte loads of m, its y/z
 // neighbour rows, B_demag and the region bytes; only the two x-edge neighbours are scalar loads.
 // UNIFORM = one region: no region gathers, the exchange coefficient is a constant.
+// THERMAL = add the fluctuating field of the current step (instantiated apart: it costs registers).
 // grid = (Nx/4 / blockDim.x, Ny, Nz)
-template <bool UNIFORM>
+template <bool UNIFORM, bool THERMAL>
 __global__ void __launch_bounds__(128) k_local4(Geometry g, const uint8_t* __restrict__ regions, const Luts* __restrict__ lut,
                                                 DevState* st, int m_role, int bd_role, int dst_role, unsigned mask,
                                                 int out_torque) {
@@ -219,7 +220,7 @@ __global__ void __launch_bounds__(128) k_local4(Geometry g, const uint8_t* __res
       bz += f1 * c1z + f2 * c2z + f3 * c3z;
     }
     if (mask & MM_ZEEMAN) { bx += lut->bext[0]; by += lut->bext[1]; bz += lut->bext[2]; }
-    if (mask & MM_THERMAL) {   // Eq. 24: one eta per cell, component and step
+    if (THERMAL) {             // Eq. 24: one eta per cell, component and step
       const float amp = lut->therm[rr] * st->therm_scale;
       const unsigned long long idx = (unsigned long long)(st->steps + st->rejected) * (unsigned long long)N + (unsigned long long)(i + l);
       bx += amp * mm_eta(st->seed, 0, idx); by += amp * mm_eta(st->seed, 1, idx); bz += amp * mm_eta(st->seed, 2, idx);

@@ -179,10 +179,11 @@ void launch_eval(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_t
   if (g.Nx % 4 == 0 && g.Ny <= 65535 && g.Nz <= 65535) {
     const int q = g.Nx / 4, bt = q >= 128 ? 128 : (q >= 64 ? 64 : 32);
     const dim3 grid((q + bt - 1) / bt, g.Ny, g.Nz);
-    if (s->nregions == 1)
-      k_local4<true><<<grid, bt, 0, s->stream>>>(g, s->regions, s->luts, s->dstate, src_role, R_B, dst_role, mask, out_torque);
-    else
-      k_local4<false><<<grid, bt, 0, s->stream>>>(g, s->regions, s->luts, s->dstate, src_role, R_B, dst_role, mask, out_torque);
+    const bool th = (mask & MM_THERMAL) != 0;
+#define MM_LOCAL4(U, T) k_local4<U, T><<<grid, bt, 0, s->stream>>>(g, s->regions, s->luts, s->dstate, src_role, R_B, dst_role, mask, out_torque)
+    if (s->nregions == 1) { if (th) MM_LOCAL4(true, true); else MM_LOCAL4(true, false); }
+    else { if (th) MM_LOCAL4(false, true); else MM_LOCAL4(false, false); }
+#undef MM_LOCAL4
     return;
   }
   k_local<<<blocks_for(g.N, 256), 256, 0, s->stream>>>(g, s->regions, s->luts, s->dstate, src_role, R_B, dst_role, mask,
