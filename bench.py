@@ -46,8 +46,10 @@ def kernel_bytes(kind, n, P):
         "last_xy": 2 * spec + 3 * Hy * Cx * 4 + 2 * spec,
         "last_z": spec + Hy * Cx * 4 + spec,
         "x_inv": 3 * spec + 12 * N,
-        "local": 12 * N + 12 * N + N + 12 * N,
-        "rk_stage": 12 * N * (1 + 26.0 / 6.0) + 12 * N,      # m0 + on average 26/6 slopes in, y out
+        # fused local kernels (Nx % 4 == 0): per step 6 x (y, B_demag, regions in; k out) + 5 x (m0 in, next y out)
+        # + 19 slope reads of the non-zero tableau / error weights = 570 N bytes over 6 launches
+        "local": 95 * N,
+        "rk_stage": 36 * N,                                   # only y_2 = m0 + h a21 k1 is left to the stage kernel
         "rk_error": 12 * N * 6,
         # register-FFT kernels of the fast 2D path (transposed spectrum, Cx = n + 1 stored kx)
         "f2_xfwd": 12 * N + N + 3 * spec,

@@ -10,7 +10,7 @@
 
 // ---- buffer roles: every kernel fetches its array pointers from DevState::ptr[role], so that the
 // accept/reject decision (taken on the device) can swap roles without a host round trip.
-enum Role { R_M = 0, R_MNEW, R_Y, R_K0, R_K1, R_K2, R_K3, R_K4, R_K5, R_K6, R_B, R_COUNT };
+enum Role { R_M = 0, R_MNEW, R_Y, R_K0, R_K1, R_K2, R_K3, R_K4, R_K5, R_K6, R_B, R_Y2, R_COUNT };   // R_Y / R_Y2: stage inputs, alternating
 
 struct DevState {
   float* ptr[R_COUNT];

@@ -106,15 +106,23 @@ __global__ void k_local(Geometry g, const uint8_t* __restrict__ regions, const L
   dst[i] = bx; dst[N + i] = by; dst[2 * N + i] = bz;
 }
 
+struct StageCoef { float a[6]; int n; };   // a_ij of one tableau row, n = number of slopes it combines
+struct ErrCoef { float e[7]; };            // b(high) - b(low) of the embedded pair
+
 // Same computation, four consecutive x cells per thread (Nx % 4 == 0): 16-byte loads of m, its y/z
 // neighbour rows, B_demag and the region bytes; only the two x-edge neighbours are scalar loads.
 // UNIFORM = one region: no region gathers, the exchange coefficient is a constant.
 // THERMAL = add the fluctuating field of the current step (instantiated apart: it costs registers).
+// FUSE = 1: the torque just formed is slope k_i; the kernel also forms the NEXT stage input
+//          y_{i+1} = normalise(m0 + h gamma (sum_{j<i} a_j k_j + a_i k_i)) (sc = that tableau row, the last
+//          coefficient belongs to k_i) into role ynext - a different buffer than the one the exchange
+//          stencil is reading. Saves re-reading k_i and one launch per stage.
+// FUSE = 2: last stage of a step: the error norm max || sum_j e_j k_j || (L372) is reduced here.
 // grid = (Nx/4 / blockDim.x, Ny, Nz)
-template <bool UNIFORM, bool THERMAL>
+template <bool UNIFORM, bool THERMAL, int FUSE>
 __global__ void __launch_bounds__(128) k_local4(Geometry g, const uint8_t* __restrict__ regions, const Luts* __restrict__ lut,
                                                 DevState* st, int m_role, int bd_role, int dst_role, unsigned mask,
-                                                int out_torque) {
+                                                int out_torque, StageCoef sc, ErrCoef ec, int ynext_role) {
   if (st->skip) return;
   const int x4 = blockIdx.x * blockDim.x + threadIdx.x;
   if (x4 * 4 >= g.Nx) return;
@@ -237,11 +245,81 @@ __global__ void __launch_bounds__(128) k_local4(Geometry g, const uint8_t* __res
   }
 #pragma unroll
   for (int c = 0; c < 3; ++c) *reinterpret_cast<float4*>(dst + c * N + i) = make_float4(b[c][0], b[c][1], b[c][2], b[c][3]);
+  if (FUSE == 1) {
+    float sv[3][4];
+    float al = 0.f;
+#pragma unroll
+    for (int j = 0; j < 6; ++j) al = (j == sc.n - 1) ? sc.a[j] : al;      // coefficient of the slope just formed
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+      for (int l = 0; l < 4; ++l) sv[c][l] = al * b[c][l];
+#pragma unroll
+    for (int j = 0; j < 5; ++j) {
+      if (j < sc.n - 1 && sc.a[j] != 0.f) {
+        const float* __restrict__ k = st->ptr[R_K0 + j];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          const float4 q = *reinterpret_cast<const float4*>(k + c * N + i);
+          sv[c][0] += sc.a[j] * q.x; sv[c][1] += sc.a[j] * q.y; sv[c][2] += sc.a[j] * q.z; sv[c][3] += sc.a[j] * q.w;
+        }
+      }
+    }
+    const float* __restrict__ m0 = st->ptr[R_M];
+    float* __restrict__ yn = st->ptr[ynext_role];
+    const float hg = st->hg;
+    float y[3][4];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const float4 q = *reinterpret_cast<const float4*>(m0 + c * N + i);
+      y[c][0] = q.x + hg * sv[c][0]; y[c][1] = q.y + hg * sv[c][1]; y[c][2] = q.z + hg * sv[c][2]; y[c][3] = q.w + hg * sv[c][3];
+    }
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      const float n2 = y[0][l] * y[0][l] + y[1][l] * y[1][l] + y[2][l] * y[2][l];
+      const float inv = n2 > 0.f ? rsqrtf(n2) : 0.f;
+      y[0][l] *= inv; y[1][l] *= inv; y[2][l] *= inv;
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) *reinterpret_cast<float4*>(yn + c * N + i) = make_float4(y[c][0], y[c][1], y[c][2], y[c][3]);
+  }
+  if (FUSE == 2) {
+    float sv[3][4];
+    const int last = dst_role - R_K0;
+    float el = 0.f;
+#pragma unroll
+    for (int j = 0; j < 7; ++j) el = (j == last) ? ec.e[j] : el;          // weight of the slope just formed
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+      for (int l = 0; l < 4; ++l) sv[c][l] = el * b[c][l];
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+      if (j < last && ec.e[j] != 0.f) {
+        const float* __restrict__ k = st->ptr[R_K0 + j];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+          const float4 q = *reinterpret_cast<const float4*>(k + c * N + i);
+          sv[c][0] += ec.e[j] * q.x; sv[c][1] += ec.e[j] * q.y; sv[c][2] += ec.e[j] * q.z; sv[c][3] += ec.e[j] * q.w;
+        }
+      }
+    }
+    float best = 0.f;
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      const float n = sqrtf(sv[0][l] * sv[0][l] + sv[1][l] * sv[1][l] + sv[2][l] * sv[2][l]);
+      best = (n > best || n != n) ? n : best;          // NaN propagates
+    }
+    // warp maximum over the lanes that are here (a ragged last block has partial warps); non-negative
+    // floats order like their bit patterns, NaN is mapped above +inf
+    const unsigned act = __activemask();
+    const unsigned bits = __reduce_max_sync(act, (best != best) ? 0x7fc00000u : __float_as_uint(best));
+    if ((int)(threadIdx.x & 31) == __ffs(act) - 1) atomicMax(&st->err_bits, bits);
+  }
 }
 
 // Dormand-Prince stage input y_i = normalise(m0 + h sum_j a_ij k_j) (L365; every stage input is
 // renormalised, reading #9). k_j are torques over gamma [T], hg = gamma * h.
-struct StageCoef { float a[6]; int n; };
 
 __global__ void k_stage(long long N, DevState* st, StageCoef sc, int dst_role) {
   if (st->skip) return;
@@ -265,7 +343,6 @@ __global__ void k_stage(long long N, DevState* st, StageCoef sc, int dst_role) {
 }
 
 // eps / h = max_cells || sum_j e_j k_j ||_2   (L372; Euclidean norm, reading #8)
-struct ErrCoef { float e[7]; };
 
 __global__ void k_error(long long N, DevState* st, ErrCoef ec) {
   if (st->skip) return;

@@ -171,18 +171,31 @@ void launch_demag(mm_sim* s, int src_role) {
   { Launch l(s, KK_XINV); k_x_inv<<<gx, T, s->xSmem, s->stream>>>(s->conv, R_B, s->xL); }
 }
 
-// field (out_torque = 0) or torque over gamma (out_torque = 1) of role `src` into role `dst`
-void launch_eval(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_torque) {
+// can the four-cells-per-thread local kernel (and with it the fused stage / error variants) run on this box?
+bool local4_ok(const mm_sim* s) { return s->g.Nx % 4 == 0 && s->g.Ny <= 65535 && s->g.Nz <= 65535; }
+
+// field (out_torque = 0) or torque over gamma (out_torque = 1, 2) of role `src` into role `dst`.
+// fuse = 1: also form the next stage input (tableau row sc) into role ynext; fuse = 2: also reduce the
+// error norm with weights ec (both need local4_ok and a torque evaluation).
+void launch_eval(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_torque, int fuse = 0,
+                 const StageCoef* scp = nullptr, const ErrCoef* ecp = nullptr, int ynext = R_Y) {
   if (mask & MM_DEMAG) launch_demag(s, src_role);
   Launch l(s, KK_LOCAL);
   const Geometry& g = s->g;
-  if (g.Nx % 4 == 0 && g.Ny <= 65535 && g.Nz <= 65535) {
+  StageCoef sc = {};
+  ErrCoef ec = {};
+  if (scp) sc = *scp;
+  if (ecp) ec = *ecp;
+  if (local4_ok(s)) {
     const int q = g.Nx / 4, bt = q >= 128 ? 128 : (q >= 64 ? 64 : 32);
     const dim3 grid((q + bt - 1) / bt, g.Ny, g.Nz);
     const bool th = (mask & MM_THERMAL) != 0;
-#define MM_LOCAL4(U, T) k_local4<U, T><<<grid, bt, 0, s->stream>>>(g, s->regions, s->luts, s->dstate, src_role, R_B, dst_role, mask, out_torque)
-    if (s->nregions == 1) { if (th) MM_LOCAL4(true, true); else MM_LOCAL4(true, false); }
-    else { if (th) MM_LOCAL4(false, true); else MM_LOCAL4(false, false); }
+#define MM_LOCAL4(U, T, F) k_local4<U, T, F><<<grid, bt, 0, s->stream>>>(g, s->regions, s->luts, s->dstate, src_role, R_B, dst_role, mask, out_torque, sc, ec, ynext)
+    if (s->nregions == 1) {
+      if (th) MM_LOCAL4(true, true, 0); else if (fuse == 1) MM_LOCAL4(true, false, 1); else if (fuse == 2) MM_LOCAL4(true, false, 2); else MM_LOCAL4(true, false, 0);
+    } else {
+      if (th) MM_LOCAL4(false, true, 0); else if (fuse == 1) MM_LOCAL4(false, false, 1); else if (fuse == 2) MM_LOCAL4(false, false, 2); else MM_LOCAL4(false, false, 0);
+    }
 #undef MM_LOCAL4
     return;
   }
@@ -223,17 +236,40 @@ void enqueue_step(mm_sim* s) {
     s->extra_evals++;
   }
   { Launch l(s, KK_CTRL); k_ctrl_begin<<<1, 1, 0, s->stream>>>(s->dstate); }
-  for (int i = 1; i < ns; ++i) {
+  auto row = [&](int i) {
     StageCoef sc;
     sc.n = i;
     for (int j = 0; j < 6; ++j) sc.a[j] = (float)(bs ? BS_A[i][j] : DP_A[i][j]);
-    const int yrole = (i == ns - 1) ? R_MNEW : R_Y;
-    { Launch l(s, KK_STAGE); k_stage<<<blocks_for(N, 256), 256, 0, s->stream>>>(N, s->dstate, sc, yrole); }
-    launch_eval(s, yrole, R_K0 + i, s->terms, tq);
-  }
+    return sc;
+  };
   ErrCoef ec;
   for (int j = 0; j < 7; ++j) ec.e[j] = (float)(bs ? BS_E[j] : DP_E[j]);
-  { Launch l(s, KK_ERROR); k_error<<<148 * 8, 256, 0, s->stream>>>(N, s->dstate, ec); }
+  if (local4_ok(s)) {
+    // fused sequence: y_2 by the stage kernel, then every evaluation also forms the next stage input
+    // (alternating between two buffers: the exchange stencil is still reading the current one) and the
+    // last one reduces the error norm: ns + 1 fewer launches, no slope is read back right after it is written
+    const StageCoef s1 = row(1);
+    int cur = (ns == 2) ? R_MNEW : R_Y;
+    { Launch l(s, KK_STAGE); k_stage<<<blocks_for(N, 256), 256, 0, s->stream>>>(N, s->dstate, s1, cur); }
+    for (int i = 1; i < ns; ++i) {
+      if (i < ns - 1) {
+        const StageCoef sn = row(i + 1);
+        const int next = (i + 1 == ns - 1) ? R_MNEW : (cur == R_Y ? R_Y2 : R_Y);
+        launch_eval(s, cur, R_K0 + i, s->terms, tq, 1, &sn, nullptr, next);
+        cur = next;
+      } else {
+        launch_eval(s, cur, R_K0 + i, s->terms, tq, 2, nullptr, &ec);
+      }
+    }
+  } else {
+    for (int i = 1; i < ns; ++i) {
+      const StageCoef sc = row(i);
+      const int yrole = (i == ns - 1) ? R_MNEW : R_Y;
+      { Launch l(s, KK_STAGE); k_stage<<<blocks_for(N, 256), 256, 0, s->stream>>>(N, s->dstate, sc, yrole); }
+      launch_eval(s, yrole, R_K0 + i, s->terms, tq);
+    }
+    { Launch l(s, KK_ERROR); k_error<<<148 * 8, 256, 0, s->stream>>>(N, s->dstate, ec); }
+  }
   { Launch l(s, KK_CTRL); k_ctrl_end<<<1, 1, 0, s->stream>>>(s->dstate); }
 }
 
