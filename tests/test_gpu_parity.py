@@ -320,6 +320,25 @@ def test_c2_full_protocol_one_nanosecond(mm):
     assert abs(sim.t - 6e-9) < 1e-20
 
 
+def test_unfused_step_sequence_on_a_ragged_width(mm):
+    # Nx % 4 != 0: the one-cell-per-thread local kernel with separate stage and error kernels (the fused
+    # variants need four cells per thread); RK45 and RK23, fixed and adaptive
+    cfg = _rand_cfg((30, 10, 2), (3e-9, 3e-9, 2e-9), nreg=3, anis=True, seed=31)
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    sim.set_solver(fix_dt=5e-14); ref.set_solver(fix_dt=5e-14)
+    sim.steps(25)
+    for _ in range(25):
+        ref.step()
+    assert np.abs(sim.get_m() - ref.m).max() < 5e-5
+    sim.set_solver_kind(mm.MM_RK23); ref.set_solver_kind("rk23")
+    sim.set_solver(max_err=1e-5, dt_init=1e-14); ref.set_solver(max_err=1e-5, dt_init=1e-14)
+    sim.run(5e-12); ref.run(5e-12)
+    assert np.abs(sim.avg_m() - ref.avg_m()).max() < 1e-3
+    info = sim.step()
+    assert info["err"] > 0 and info["dt_taken"] > 0
+
+
 def test_c3_reduced_adaptive_steps(mm):
     cfg = config_c3(grid=(32, 32, 8), ngrains=12)
     sim = mm.from_config(cfg)
