@@ -163,3 +163,24 @@ def ll_torque_over_gamma(m, B, alpha_cell, precession=True):
     mxB = cross(m, B)
     damp = alpha_cell[None] * cross(m, mxB)
     return -((mxB if precession else 0.0) + damp) / (1.0 + alpha_cell[None] ** 2)
+
+
+HBAR = 1.054571817e-34       # J s
+E_CHARGE = 1.602176634e-19   # C
+
+
+def slonczewski_torque_over_gamma(m, Msat_cell, alpha_cell, jz, pol, lam, eps_prime, mp, thickness):
+    """Eq. 28-30 (L336-L347), divided by gamma_LL [T]:
+       tau_SL = beta (eps - alpha eps')/(1+alpha^2) m x (m_P x m) - beta (eps' - alpha eps)/(1+alpha^2) m x m_P,
+       beta = j_z hbar / (Msat e d),  eps = P Lambda^2 / ((Lambda^2 + 1) + (Lambda^2 - 1) m.m_P).
+    As printed beta is a field (tesla) while Eq. 1 wants 1/s: the torque is gamma_LL times this (#18)."""
+    mp = np.asarray(mp, dtype=float)
+    mp = mp / np.linalg.norm(mp)
+    mpv = mp[:, None, None, None] * np.ones_like(m)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        beta = np.where(Msat_cell > 0, jz * HBAR / (Msat_cell * E_CHARGE * thickness), 0.0)[None]
+    l2 = lam * lam
+    eps = pol * l2 / ((l2 + 1.0) + (l2 - 1.0) * (m * mpv).sum(axis=0, keepdims=True))
+    a = alpha_cell[None]
+    den = 1.0 + a * a
+    return beta * ((eps - a * eps_prime) / den * cross(m, cross(mpv, m)) - (eps_prime - a * eps) / den * cross(m, mpv))

@@ -77,6 +77,13 @@ class RefSim:
         self.solver = "rk45"
         self.precession = True
         self.temp, self.seed = 0.0, 0
+        self.stt = None
+
+    def set_slonczewski(self, jz, pol, lam=1.0, eps_prime=0.0, mp=(0, 0, 1)):
+        """Spin-transfer torque of Eq. 28-30 (L336-L347): current density j_z [A/m^2] through the layer
+        thickness d = Nz dz, polarisation P, Slonczewski Lambda, secondary term eps', fixed layer m_P."""
+        self.stt = None if jz == 0 else (float(jz), float(pol), float(lam), float(eps_prime), tuple(mp))
+        self.k1 = None
 
     def set_temperature(self, temp, seed=0):
         """Thermal field of Eq. 24 (L303-L310) at `temp` kelvin; eta comes from the counter-based
@@ -166,7 +173,12 @@ class RefSim:
         """dm/dt [1/s] (Eq. 1-2); b_extra: an additional field term (the thermal field of the step)."""
         self.n_eval += 1
         alpha = self.p.alpha[self.regions]
-        return self.p.gamma_LL * fld.ll_torque_over_gamma(m, self.b_eff(self.terms, m) + b_extra, alpha, self.precession)
+        tq = fld.ll_torque_over_gamma(m, self.b_eff(self.terms, m) + b_extra, alpha, self.precession)
+        if self.stt is not None:
+            jz, pol, lam, epsp, mp = self.stt
+            tq = tq + fld.slonczewski_torque_over_gamma(m, self.p.Msat[self.regions], alpha, jz, pol, lam, epsp, mp,
+                                                        self.grid[2] * self.cell[2])
+        return self.p.gamma_LL * tq
 
     # ---- energies (Eq. 4, 8, 20, 23; Zeeman -M.B_ext), joules
     def energy(self, m=None, terms=MM_ALL):

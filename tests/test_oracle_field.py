@@ -391,3 +391,37 @@ def test_sp3_vortex_transition_from_the_stored_oracle_energies():
     d1 = e[(8.50, "twisted")] - e[(8.50, "vortex")]
     assert d0 < 0 < d1
     assert abs(8.44 + 0.06 * d0 / (d0 - d1) - paper["twisted_flower_to_vortex"]) < 0.01
+
+
+def test_slonczewski_torque_closed_form_for_a_macrospin():
+    # Eq. 28-30 (L336-L347) with Lambda = 1 (eps = P/2), eps' = 0, no field: the polar angle to m_P obeys
+    # d theta/dt = -gamma beta eps/(1+alpha^2) sin theta, i.e. tan(theta/2) = tan(theta0/2) exp(-gamma beta eps t/(1+alpha^2)),
+    # and the azimuth turns at the constant rate -alpha gamma beta eps/(1+alpha^2) (the +alpha eps m x m_P term:
+    # m x z = (m_y, -m_x, 0) turns m clockwise about m_P).
+    Ms, d, jz, P, alpha = 8e5, 2e-9, 4e11, 0.6, 0.05
+    sim = RefSim((1, 1, 1), (5e-9, 5e-9, d))
+    sim.set_params(Params.uniform(1, Msat=Ms, Aex=0.0, alpha=alpha))
+    sim.set_terms(MM_ZEEMAN)                             # no field at all
+    th0 = 2.0
+    sim.set_m(np.array([np.sin(th0), 0.0, np.cos(th0)]).reshape(3, 1, 1, 1))
+    sim.set_slonczewski(jz, P, lam=1.0, eps_prime=0.0, mp=(0, 0, 1))
+    sim.set_solver(max_err=1e-8)
+    beta = jz * fld.HBAR / (Ms * fld.E_CHARGE * d)       # tesla
+    rate = GAMMA * beta * (P / 2) / (1 + alpha ** 2)
+    t = 1.5 / rate
+    sim.run(t)
+    mx, my, mz = sim.m[:, 0, 0, 0]
+    th = 2 * np.arctan(np.tan(th0 / 2) * np.exp(-rate * t))
+    assert abs(np.arccos(mz) - th) < 1e-6
+    assert abs(np.arctan2(my, mx) + alpha * rate * t) < 1e-6
+    # angle dependence of eps (Eq. 30) and the eps' term: torque components against the printed expression
+    lam, epsp = 1.7, 0.3
+    m = np.array([0.36, -0.48, 0.8]).reshape(3, 1, 1, 1)
+    mp = np.array([0.0, 0.6, 0.8])
+    tq = fld.slonczewski_torque_over_gamma(m, np.array([[[Ms]]]), np.array([[[alpha]]]), jz, P, lam, epsp, mp, d)[:, 0, 0, 0]
+    mm_, c = m[:, 0, 0, 0], float(m[:, 0, 0, 0] @ mp)
+    eps = P * lam ** 2 / ((lam ** 2 + 1) + (lam ** 2 - 1) * c)
+    want = beta * ((eps - alpha * epsp) * np.cross(mm_, np.cross(mp, mm_)) - (epsp - alpha * eps) * np.cross(mm_, mp)) / (1 + alpha ** 2)
+    assert np.allclose(tq, want, rtol=1e-13) and abs(tq @ mm_) < 1e-18
+    # sign: reversing the current reverses the torque (switching in both directions, Fig. 9)
+    assert np.allclose(fld.slonczewski_torque_over_gamma(m, np.array([[[Ms]]]), np.array([[[alpha]]]), -jz, P, lam, epsp, mp, d)[:, 0, 0, 0], -tq)
