@@ -133,6 +133,14 @@ int mm_set_solver_kind(mm_sim* sim, int kind);
  * mm_b_eff / mm_torque never include the thermal field. */
 int mm_set_temperature(mm_sim* sim, double kelvin, unsigned long long seed);
 
+/* Slonczewski spin-transfer torque (Eq. 28-30) added to every torque evaluation:
+ *   tau_SL = beta (eps - alpha eps')/(1+alpha^2) m x (m_P x m) - beta (eps' - alpha eps)/(1+alpha^2) m x m_P,
+ *   beta = j_z hbar / (Msat e d), eps = P Lambda^2 / ((Lambda^2+1) + (Lambda^2-1) m.m_P),
+ * j_z [A/m^2] through the layer thickness d = Nz dz, polarisation P, Lambda > 0, secondary term eps',
+ * fixed-layer direction m_P (normalised by the library; host pointer). As printed beta is a field, so the
+ * torque is gamma_LL times the expression (#18). jz = 0 switches the term off. */
+int mm_set_slonczewski(mm_sim* sim, double jz, double pol, double lambda, double eps_prime, const double mp[3]);
+
 /* Precession term of Eq. 2 on (default) or off: off leaves tau = -gamma alpha/(1+alpha^2) m x (m x B),
  * "so that the effective field points towards decreasing energy" (relax(), L388). */
 int mm_set_precession(mm_sim* sim, int on);

@@ -50,6 +50,8 @@ struct mm_sim {
   int solver = MM_RK45;
   bool precession = true;
   double temperature = 0.0;
+  bool stt_on = false;         // Slonczewski torque enabled (mm_set_slonczewski)
+  float stt[7] = {};           // pref, pol, lam2, eps_prime, mp[3]  (SttArgs of local_rk.cuh)
   int nregions = 1;
   long launches = 0;
   long extra_evals = 0;

@@ -527,3 +527,32 @@ __global__ void k_maxnorm(long long N, const float* __restrict__ v, unsigned* __
   }
   if ((threadIdx.x & 31) == 0) atomicMax(out, (best != best) ? 0x7fc00000u : __float_as_uint(best));
 }
+
+// Slonczewski spin-transfer torque (Eq. 28-30) over gamma_LL [T], added to the torque in role
+// tq_role for the magnetisation in role m_role (a kernel of its own: the hot path does not pay for it):
+//   tau_SL = beta (eps - alpha eps')/(1+alpha^2) m x (m_P x m) - beta (eps' - alpha eps)/(1+alpha^2) m x m_P,
+//   beta = j_z hbar / (Msat e d) = pref / Bsat,  eps = P L^2 / ((L^2+1) + (L^2-1) m.m_P).
+struct SttArgs { float pref, pol, lam2, eps_prime, mp[3]; };   // pref = j_z hbar mu0 / (e d)  [T^2]
+
+__global__ void k_add_stt(long long N, const uint8_t* __restrict__ regions, const Luts* __restrict__ lut, DevState* st,
+                          int m_role, int tq_role, SttArgs p) {
+  if (st->skip) return;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const float* __restrict__ m = st->ptr[m_role];
+  float* __restrict__ tq = st->ptr[tq_role];
+  const int r = regions[i];
+  const float bs = lut->Bsat[r];
+  if (!(bs > 0.f)) return;
+  const float al = lut->alpha[r], beta = p.pref / bs, den = 1.f / (1.f + al * al);
+  const float mx = m[i], my = m[N + i], mz = m[2 * N + i];
+  const float px = p.mp[0], py = p.mp[1], pz = p.mp[2];
+  const float c = mx * px + my * py + mz * pz;
+  const float eps = p.pol * p.lam2 / ((p.lam2 + 1.f) + (p.lam2 - 1.f) * c);
+  const float a = beta * (eps - al * p.eps_prime) * den, b = -beta * (p.eps_prime - al * eps) * den;
+  // m x (m_P x m) = m_P - (m.m_P) m for |m| = 1, written out as the double cross product
+  const float qx = py * mz - pz * my, qy = pz * mx - px * mz, qz = px * my - py * mx;      // m_P x m
+  const float dx = my * qz - mz * qy, dy = mz * qx - mx * qz, dz = mx * qy - my * qx;      // m x (m_P x m)
+  const float ex = my * pz - mz * py, ey = mz * px - mx * pz, ez = mx * py - my * px;      // m x m_P
+  tq[i] += a * dx + b * ex; tq[N + i] += a * dy + b * ey; tq[2 * N + i] += a * dz + b * ez;
+}

@@ -177,9 +177,24 @@ bool local4_ok(const mm_sim* s) { return s->g.Nx % 4 == 0 && s->g.Ny <= 65535 &&
 // field (out_torque = 0) or torque over gamma (out_torque = 1, 2) of role `src` into role `dst`.
 // fuse = 1: also form the next stage input (tableau row sc) into role ynext; fuse = 2: also reduce the
 // error norm with weights ec (both need local4_ok and a torque evaluation).
+void launch_local(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_torque, int fuse, const StageCoef* scp,
+                  const ErrCoef* ecp, int ynext);
+
 void launch_eval(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_torque, int fuse = 0,
                  const StageCoef* scp = nullptr, const ErrCoef* ecp = nullptr, int ynext = R_Y) {
   if (mask & MM_DEMAG) launch_demag(s, src_role);
+  launch_local(s, src_role, dst_role, mask, out_torque, fuse, scp, ecp, ynext);
+  if (out_torque && s->stt_on) {      // Slonczewski torque on top (Eq. 28); only reached with fuse == 0
+    SttArgs p;
+    p.pref = s->stt[0]; p.pol = s->stt[1]; p.lam2 = s->stt[2]; p.eps_prime = s->stt[3];
+    p.mp[0] = s->stt[4]; p.mp[1] = s->stt[5]; p.mp[2] = s->stt[6];
+    Launch l(s, KK_OTHER);
+    k_add_stt<<<blocks_for(s->g.N, 256), 256, 0, s->stream>>>(s->g.N, s->regions, s->luts, s->dstate, src_role, dst_role, p);
+  }
+}
+
+void launch_local(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_torque, int fuse, const StageCoef* scp,
+                  const ErrCoef* ecp, int ynext) {
   Launch l(s, KK_LOCAL);
   const Geometry& g = s->g;
   StageCoef sc = {};
@@ -244,7 +259,7 @@ void enqueue_step(mm_sim* s) {
   };
   ErrCoef ec;
   for (int j = 0; j < 7; ++j) ec.e[j] = (float)(bs ? BS_E[j] : DP_E[j]);
-  if (local4_ok(s)) {
+  if (local4_ok(s) && !s->stt_on) {
     // fused sequence: y_2 by the stage kernel, then every evaluation also forms the next stage input
     // (alternating between two buffers: the exchange stencil is still reading the current one) and the
     // last one reduces the error norm: ns + 1 fewer launches, no slope is read back right after it is written
@@ -545,6 +560,22 @@ int mm_set_temperature(mm_sim* s, double kelvin, unsigned long long seed) {
   s->hst.seed = seed;
   s->have_k1 = false;
   return push_state(s);
+}
+
+int mm_set_slonczewski(mm_sim* s, double jz, double pol, double lambda, double eps_prime, const double mp[3]) {
+  if (!s) return MM_EINVAL;
+  if (jz == 0) { s->stt_on = false; s->have_k1 = false; return MM_OK; }
+  if (!mp || !std::isfinite(jz) || !std::isfinite(pol) || !(lambda > 0) || !std::isfinite(eps_prime))
+    return mm_fail(s, MM_EINVAL, "bad spin-torque parameter");
+  const double n = std::sqrt(mp[0] * mp[0] + mp[1] * mp[1] + mp[2] * mp[2]);
+  if (!(n > 0)) return mm_fail(s, MM_EINVAL, "fixed-layer direction is zero");
+  const double hbar = 1.054571817e-34, e = 1.602176634e-19, mu0 = 4e-7 * M_PI, d = s->g.Nz * s->cell[2];
+  s->stt[0] = (float)(jz * hbar * mu0 / (e * d));       // beta = this / Bsat
+  s->stt[1] = (float)pol; s->stt[2] = (float)(lambda * lambda); s->stt[3] = (float)eps_prime;
+  for (int c = 0; c < 3; ++c) s->stt[4 + c] = (float)(mp[c] / n);
+  s->stt_on = true;
+  s->have_k1 = false;
+  return MM_OK;
 }
 
 int mm_set_precession(mm_sim* s, int on) {

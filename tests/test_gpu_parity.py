@@ -596,3 +596,37 @@ def test_thermal_equilibrium_and_switching_rate(mm):
     V = c ** 3
     f_eq25 = gam * alpha / (1 + alpha ** 2) * np.sqrt(8 * K ** 3 * V / (2 * np.pi * Ms ** 2 * kB * T)) * np.exp(-K * V / (kB * T))
     assert 0.7 < f_meas / f_eq25 < 1.3, (f_meas, f_eq25)
+
+
+def test_slonczewski_torque_and_switching(mm):
+    # Eq. 28-30 (L336-L347): parity of the torque with the extra term and of a trajectory; a macrospin with
+    # Lambda = 1 follows tan(theta/2) = tan(theta0/2) exp(-gamma beta eps t/(1+alpha^2)) (closed form, as in the oracle's pin)
+    cfg = _rand_cfg((32, 16, 2), (4e-9, 4e-9, 2e-9), nreg=3, anis=True, seed=8)
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    args = dict(jz=6e11, pol=0.57, lam=1.6, eps_prime=0.2, mp=(0.3, -0.2, 0.9))
+    sim.set_slonczewski(**args); ref.set_slonczewski(**args)
+    tq = sim.torque().astype(np.float64)
+    tr = ref.torque(ref.m) / ref.p.gamma_LL
+    assert np.abs(tq - tr).max() <= FIELD_TOL * np.abs(tr).max()
+    sim.set_slonczewski(0.0, 0.0)
+    assert np.abs(sim.torque() - tq).max() > 1e-3 * np.abs(tq).max()          # the term was really there
+    sim.set_slonczewski(**args)
+    sim.set_solver(fix_dt=5e-14); ref.set_solver(fix_dt=5e-14)
+    sim.steps(30)
+    for _ in range(30):
+        ref.step()
+    assert np.abs(sim.get_m() - ref.m).max() < 5e-5
+    # macrospin closed form
+    Ms, d, jz, P, alpha, th0 = 8e5, 2e-9, 4e11, 0.6, 0.05, 2.0
+    p = Params.uniform(1, Msat=Ms, Aex=0.0, alpha=alpha)
+    m0 = np.zeros((3, 1, 4, 4), dtype=np.float32); m0[0] = np.sin(th0); m0[2] = np.cos(th0)
+    sim = mm.from_config(dict(grid=(4, 4, 1), cell=(5e-9, 5e-9, d), pbc=(0, 0, 0), regions=None, params=p, m0=m0))
+    sim.set_terms(MM_ZEEMAN)
+    sim.set_slonczewski(jz, P, 1.0, 0.0, (0, 0, 1))
+    sim.set_solver(max_err=1e-7)
+    rate = 1.7595e11 * (jz * 1.054571817e-34 / (Ms * 1.602176634e-19 * d)) * (P / 2) / (1 + alpha ** 2)
+    t = 1.5 / rate
+    sim.run(t)
+    mz = sim.avg_m()[2]
+    assert abs(np.arccos(mz) - 2 * np.arctan(np.tan(th0 / 2) * np.exp(-rate * t))) < 2e-5
