@@ -184,3 +184,35 @@ def slonczewski_torque_over_gamma(m, Msat_cell, alpha_cell, jz, pol, lam, eps_pr
     a = alpha_cell[None]
     den = 1.0 + a * a
     return beta * ((eps - a * eps_prime) / den * cross(m, cross(mpv, m)) - (eps_prime - a * eps) / den * cross(m, mpv))
+
+
+MU_BOHR = 9.2740100783e-24   # J/T
+
+
+def zhang_li_torque_over_gamma(m, Msat_cell, alpha_cell, j, xi, cell, pbc, gamma):
+    """Zhang-Li spin-transfer torque, Eq. 26 (L327-L331), divided by gamma_LL [T]:
+       tau_ZL = 1/(1+alpha^2) [ (1 + xi alpha) m x (m x (u.grad) m) + (xi - alpha) m x (u.grad) m ],
+       u = mu_B mu0 / (2 e gamma_LL Bsat (1 + xi^2)) j      [T m].
+    PAPER.md prints the two terms identically (garbled); the double cross product in the first term is the
+    reading of DESIGN.md #19. (u.grad) m by central differences; a missing neighbour at an open boundary is
+    replaced by the cell's own m (as for the exchange stencil, L196); periodic axes wrap."""
+    j = np.asarray(j, dtype=float)
+    D = np.zeros_like(m)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        pref = np.where(Msat_cell > 0, MU_BOHR * MU0 / (2.0 * E_CHARGE * gamma * (MU0 * Msat_cell) * (1.0 + xi * xi)), 0.0)
+    for axis_m, (ja, d, per) in enumerate(zip(j[::-1], cell[::-1], pbc[::-1])):      # array axes are z, y, x
+        if ja == 0 or m.shape[1 + axis_m] == 1:
+            continue
+        ax = 1 + axis_m
+        if per:
+            up, dn = np.roll(m, -1, axis=ax), np.roll(m, 1, axis=ax)
+        else:
+            up, dn = m.copy(), m.copy()
+            sl_hi = [slice(None)] * 4; sl_lo = [slice(None)] * 4
+            sl_hi[ax] = slice(1, None); sl_lo[ax] = slice(None, -1)
+            up[tuple(sl_lo)] = m[tuple(sl_hi)]        # neighbour at +1 (the last cell keeps its own m)
+            dn[tuple(sl_hi)] = m[tuple(sl_lo)]        # neighbour at -1 (the first cell keeps its own m)
+        D += (pref * ja)[None] * (up - dn) / (2.0 * d)
+    a = alpha_cell[None]
+    mxD = cross(m, D)
+    return ((1.0 + xi * a) * cross(m, mxD) + (xi - a) * mxD) / (1.0 + a * a)

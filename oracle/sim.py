@@ -78,11 +78,17 @@ class RefSim:
         self.precession = True
         self.temp, self.seed = 0.0, 0
         self.stt = None
+        self.zl = None
 
     def set_slonczewski(self, jz, pol, lam=1.0, eps_prime=0.0, mp=(0, 0, 1)):
         """Spin-transfer torque of Eq. 28-30 (L336-L347): current density j_z [A/m^2] through the layer
         thickness d = Nz dz, polarisation P, Slonczewski Lambda, secondary term eps', fixed layer m_P."""
         self.stt = None if jz == 0 else (float(jz), float(pol), float(lam), float(eps_prime), tuple(mp))
+        self.k1 = None
+
+    def set_zhang_li(self, j, xi):
+        """Zhang-Li torque of Eq. 26 (L327-L331): current density vector j [A/m^2], non-adiabaticity xi."""
+        self.zl = None if not np.any(np.asarray(j)) else (tuple(float(x) for x in j), float(xi))
         self.k1 = None
 
     def set_temperature(self, temp, seed=0):
@@ -178,6 +184,9 @@ class RefSim:
             jz, pol, lam, epsp, mp = self.stt
             tq = tq + fld.slonczewski_torque_over_gamma(m, self.p.Msat[self.regions], alpha, jz, pol, lam, epsp, mp,
                                                         self.grid[2] * self.cell[2])
+        if self.zl is not None:
+            tq = tq + fld.zhang_li_torque_over_gamma(m, self.p.Msat[self.regions], alpha, self.zl[0], self.zl[1], self.cell,
+                                                     self.pbc, self.p.gamma_LL)
         return self.p.gamma_LL * tq
 
     # ---- energies (Eq. 4, 8, 20, 23; Zeeman -M.B_ext), joules

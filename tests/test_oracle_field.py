@@ -425,3 +425,39 @@ def test_slonczewski_torque_closed_form_for_a_macrospin():
     assert np.allclose(tq, want, rtol=1e-13) and abs(tq @ mm_) < 1e-15
     # sign: reversing the current reverses the torque (switching in both directions, Fig. 9)
     assert np.allclose(fld.slonczewski_torque_over_gamma(m, np.array([[[Ms]]]), np.array([[[alpha]]]), -jz, P, lam, epsp, mp, d)[:, 0, 0, 0], -tq)
+
+
+def test_zhang_li_torque_advects_a_spiral():
+    # Eq. 26 (L327-L331, reading #19). With xi = alpha the torque is -(gamma u . grad) m: any texture is carried
+    # along with velocity gamma u. For the spiral m = (cos kx, sin kx, 0) on a periodic chain the central
+    # difference gives exactly m(x, t) = (cos(kx - w t), sin(kx - w t), 0), w = gamma u sin(k dx)/dx.
+    n, dx, Ms, alpha, j = 32, 4e-9, 8e5, 0.1, 2e12
+    sim = RefSim((n, 1, 1), (dx, dx, dx), pbc=(1, 0, 0))
+    sim.set_params(Params.uniform(1, Msat=Ms, Aex=0.0, alpha=alpha))
+    sim.set_terms(MM_ZEEMAN)                             # no field at all
+    k = 2 * np.pi * 2 / (n * dx)
+    x = np.arange(n) * dx
+    m0 = np.zeros((3, 1, 1, n)); m0[0, 0, 0] = np.cos(k * x); m0[1, 0, 0] = np.sin(k * x)
+    sim.set_m(m0)
+    sim.set_zhang_li((j, 0, 0), xi=alpha)
+    sim.set_solver(max_err=1e-8)
+    u = fld.MU_BOHR * fld.MU0 / (2 * fld.E_CHARGE * GAMMA * fld.MU0 * Ms * (1 + alpha ** 2)) * j      # T m
+    assert abs(GAMMA * u - fld.MU_BOHR * j / (2 * fld.E_CHARGE * Ms * (1 + alpha ** 2))) < 1e-9 * GAMMA * u   # a velocity, m/s
+    w = GAMMA * u * np.sin(k * dx) / dx
+    t = 1.0 / w
+    sim.run(t)
+    assert np.abs(sim.m[0, 0, 0] - np.cos(k * x - w * t)).max() < 1e-6
+    assert np.abs(sim.m[1, 0, 0] - np.sin(k * x - w * t)).max() < 1e-6 and np.abs(sim.m[2]).max() < 1e-12
+    # xi != alpha: the field-like term tilts the spiral out of the plane at the printed rate
+    sim.set_m(m0); sim.set_zhang_li((j, 0, 0), xi=0.4)
+    tq = sim.torque(sim.m) / GAMMA
+    u4 = u * (1 + alpha ** 2) / (1 + 0.4 ** 2)
+    assert np.allclose(tq[2, 0, 0], (0.4 - alpha) / (1 + alpha ** 2) * u4 * np.sin(k * dx) / dx, rtol=1e-12)
+    # open boundary: the end cells see a one-sided half difference (own m stands in for the missing neighbour)
+    sim2 = RefSim((n, 1, 1), (dx, dx, dx))
+    sim2.set_params(Params.uniform(1, Msat=Ms, Aex=0.0, alpha=alpha)); sim2.set_terms(MM_ZEEMAN)
+    sim2.set_m(m0); sim2.set_zhang_li((j, 0, 0), xi=alpha)
+    t2 = sim2.torque(sim2.m) / GAMMA
+    want0 = -u * (m0[:, 0, 0, 1] - m0[:, 0, 0, 0]) / (2 * dx)
+    want0 = want0 - (want0 @ m0[:, 0, 0, 0]) * m0[:, 0, 0, 0]        # m x (m x D) = -(D - (m.D) m)
+    assert np.allclose(t2[:, 0, 0, 0], want0, rtol=1e-10, atol=1e-18)
