@@ -141,6 +141,15 @@ int mm_set_temperature(mm_sim* sim, double kelvin, unsigned long long seed);
  * torque is gamma_LL times the expression (#18). jz = 0 switches the term off. */
 int mm_set_slonczewski(mm_sim* sim, double jz, double pol, double lambda, double eps_prime, const double mp[3]);
 
+/* Zhang-Li spin-transfer torque (Eq. 26) added to every torque evaluation:
+ *   tau_ZL = 1/(1+alpha^2) [ (1 + xi alpha) m x (m x (u.grad) m) + (xi - alpha) m x (u.grad) m ],
+ *   u = mu_B mu0 / (2 e gamma_LL Bsat (1 + xi^2)) j,
+ * j [A/m^2] uniform current density (host pointer, 3 doubles), xi the non-adiabaticity. PAPER.md prints both
+ * terms identically; the double cross product in the first is DESIGN.md reading #19. Central differences;
+ * a missing neighbour at an open boundary is the cell's own m. Uses gamma_LL of the last mm_set_params.
+ * j = 0 switches the term off. */
+int mm_set_zhang_li(mm_sim* sim, const double j[3], double xi);
+
 /* Precession term of Eq. 2 on (default) or off: off leaves tau = -gamma alpha/(1+alpha^2) m x (m x B),
  * "so that the effective field points towards decreasing energy" (relax(), L388). */
 int mm_set_precession(mm_sim* sim, int on);

@@ -69,6 +69,7 @@ _SIGNATURES = {
     "mm_torque": (C.c_int, [C.c_void_p, C.c_void_p]),
     "mm_set_solver_kind": (C.c_int, [C.c_void_p, C.c_int]),
     "mm_set_precession": (C.c_int, [C.c_void_p, C.c_int]),
+    "mm_set_zhang_li": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.c_double]),
     "mm_set_slonczewski": (C.c_int, [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_double)]),
     "mm_set_temperature": (C.c_int, [C.c_void_p, C.c_double, C.c_ulonglong]),
     "mm_step_rk45": (C.c_int, [C.c_void_p, C.POINTER(mm_step_info)]),
@@ -228,6 +229,10 @@ class Sim:
     def set_slonczewski(self, jz, pol, lam=1.0, eps_prime=0.0, mp=(0, 0, 1)):
         v = (C.c_double * 3)(*[float(x) for x in mp])
         _check(lib().mm_set_slonczewski(self._h, float(jz), float(pol), float(lam), float(eps_prime), v), self._h)
+
+    def set_zhang_li(self, j, xi):
+        v = (C.c_double * 3)(*[float(x) for x in j])
+        _check(lib().mm_set_zhang_li(self._h, v, float(xi)), self._h)
 
     def set_precession(self, on):
         _check(lib().mm_set_precession(self._h, 1 if on else 0), self._h)

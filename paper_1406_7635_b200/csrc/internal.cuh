@@ -50,6 +50,8 @@ struct mm_sim {
   int solver = MM_RK45;
   bool precession = true;
   double temperature = 0.0;
+  bool zl_on = false;          // Zhang-Li torque enabled (mm_set_zhang_li)
+  float zl[4] = {};            // ZlArgs of local_rk.cuh
   bool stt_on = false;         // Slonczewski torque enabled (mm_set_slonczewski)
   float stt[7] = {};           // pref, pol, lam2, eps_prime, mp[3]  (SttArgs of local_rk.cuh)
   int nregions = 1;

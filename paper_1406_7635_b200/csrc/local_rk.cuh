@@ -556,3 +556,49 @@ __global__ void k_add_stt(long long N, const uint8_t* __restrict__ regions, cons
   const float ex = my * pz - mz * py, ey = mz * px - mx * pz, ez = mx * py - my * px;      // m x m_P
   tq[i] += a * dx + b * ex; tq[N + i] += a * dy + b * ey; tq[2 * N + i] += a * dz + b * ez;
 }
+
+// Zhang-Li spin-transfer torque (Eq. 26; #19) over gamma_LL [T], added to the torque in
+// role tq_role:  1/(1+alpha^2) [ (1 + xi alpha) m x (m x D) + (xi - alpha) m x D ],  D = (u . grad) m,
+// u = mu_B mu0 j / (2 e gamma_LL Bsat (1 + xi^2)); central differences, a missing neighbour at an open
+// boundary is the cell's own m (L196), periodic axes wrap.
+struct ZlArgs { float c[3]; float xi; };     // c[a] = mu_B mu0 j_a / (2 e gamma (1 + xi^2)) / (2 d_a)  [T^2]
+
+__global__ void k_add_zl(Geometry g, const uint8_t* __restrict__ regions, const Luts* __restrict__ lut, DevState* st,
+                         int m_role, int tq_role, ZlArgs p) {
+  if (st->skip) return;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= g.N) return;
+  const long long N = g.N;
+  const float* __restrict__ m = st->ptr[m_role];
+  float* __restrict__ tq = st->ptr[tq_role];
+  const int r = regions[i];
+  const float bs = lut->Bsat[r];
+  if (!(bs > 0.f)) return;
+  const int x = (int)(i % g.Nx);
+  const long long t = i / g.Nx;
+  const int y = (int)(t % g.Ny), z = (int)(t / g.Ny);
+  float dx = 0.f, dy = 0.f, dz = 0.f;
+  auto diff = [&](long long up, long long dn, float c) {
+    dx += c * (m[up] - m[dn]); dy += c * (m[N + up] - m[N + dn]); dz += c * (m[2 * N + up] - m[2 * N + dn]);
+  };
+  if (g.Nx > 1 && p.c[0] != 0.f) {
+    const long long up = x + 1 < g.Nx ? i + 1 : (g.pbc[0] ? i + 1 - g.Nx : i), dn = x > 0 ? i - 1 : (g.pbc[0] ? i - 1 + g.Nx : i);
+    diff(up, dn, p.c[0] / bs);
+  }
+  if (g.Ny > 1 && p.c[1] != 0.f) {
+    const long long s = g.Nx;
+    const long long up = y + 1 < g.Ny ? i + s : (g.pbc[1] ? i + s - s * g.Ny : i), dn = y > 0 ? i - s : (g.pbc[1] ? i - s + s * g.Ny : i);
+    diff(up, dn, p.c[1] / bs);
+  }
+  if (g.Nz > 1 && p.c[2] != 0.f) {
+    const long long s = (long long)g.Nx * g.Ny;
+    const long long up = z + 1 < g.Nz ? i + s : (g.pbc[2] ? i + s - s * g.Nz : i), dn = z > 0 ? i - s : (g.pbc[2] ? i - s + s * g.Nz : i);
+    diff(up, dn, p.c[2] / bs);
+  }
+  const float al = lut->alpha[r], den = 1.f / (1.f + al * al);
+  const float mx = m[i], my = m[N + i], mz = m[2 * N + i];
+  const float ex = my * dz - mz * dy, ey = mz * dx - mx * dz, ez = mx * dy - my * dx;      // m x D
+  const float fx = my * ez - mz * ey, fy = mz * ex - mx * ez, fz = mx * ey - my * ex;      // m x (m x D)
+  const float a = (1.f + p.xi * al) * den, b = (p.xi - al) * den;
+  tq[i] += a * fx + b * ex; tq[N + i] += a * fy + b * ey; tq[2 * N + i] += a * fz + b * ez;
+}

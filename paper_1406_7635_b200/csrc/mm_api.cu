@@ -191,6 +191,12 @@ void launch_eval(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_t
     Launch l(s, KK_OTHER);
     k_add_stt<<<blocks_for(s->g.N, 256), 256, 0, s->stream>>>(s->g.N, s->regions, s->luts, s->dstate, src_role, dst_role, p);
   }
+  if (out_torque && s->zl_on) {       // Zhang-Li torque on top (Eq. 26)
+    ZlArgs p;
+    p.c[0] = s->zl[0]; p.c[1] = s->zl[1]; p.c[2] = s->zl[2]; p.xi = s->zl[3];
+    Launch l(s, KK_OTHER);
+    k_add_zl<<<blocks_for(s->g.N, 256), 256, 0, s->stream>>>(s->g, s->regions, s->luts, s->dstate, src_role, dst_role, p);
+  }
 }
 
 void launch_local(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_torque, int fuse, const StageCoef* scp,
@@ -259,7 +265,7 @@ void enqueue_step(mm_sim* s) {
   };
   ErrCoef ec;
   for (int j = 0; j < 7; ++j) ec.e[j] = (float)(bs ? BS_E[j] : DP_E[j]);
-  if (local4_ok(s) && !s->stt_on) {
+  if (local4_ok(s) && !s->stt_on && !s->zl_on) {
     // fused sequence: y_2 by the stage kernel, then every evaluation also forms the next stage input
     // (alternating between two buffers: the exchange stencil is still reading the current one) and the
     // last one reduces the error norm: ns + 1 fewer launches, no slope is read back right after it is written
@@ -575,6 +581,22 @@ int mm_set_slonczewski(mm_sim* s, double jz, double pol, double lambda, double e
   for (int c = 0; c < 3; ++c) s->stt[4 + c] = (float)(mp[c] / n);
   s->stt_on = true;
   s->have_k1 = false;
+  return MM_OK;
+}
+
+int mm_set_zhang_li(mm_sim* s, const double j[3], double xi) {
+  if (!s || !j) return mm_fail(s, MM_EINVAL, "null argument");
+  if (!std::isfinite(j[0]) || !std::isfinite(j[1]) || !std::isfinite(j[2]) || !std::isfinite(xi))
+    return mm_fail(s, MM_EINVAL, "bad spin-torque parameter");
+  s->have_k1 = false;
+  if (j[0] == 0 && j[1] == 0 && j[2] == 0) { s->zl_on = false; return MM_OK; }
+  int rc;
+  if ((rc = pull_state(s))) return rc;
+  const double muB = 9.2740100783e-24, e = 1.602176634e-19, mu0 = 4e-7 * M_PI;
+  const double c = muB * mu0 / (2.0 * e * s->hst.gamma * (1.0 + xi * xi));           // u = c j / Bsat  [T m]
+  for (int a = 0; a < 3; ++a) s->zl[a] = (float)(c * j[a] / (2.0 * s->cell[a]));
+  s->zl[3] = (float)xi;
+  s->zl_on = true;
   return MM_OK;
 }
 

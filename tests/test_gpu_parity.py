@@ -630,3 +630,39 @@ def test_slonczewski_torque_and_switching(mm):
     sim.run(t)
     mz = sim.avg_m()[2]
     assert abs(np.arccos(mz) - 2 * np.arctan(np.tan(th0 / 2) * np.exp(-rate * t))) < 2e-5
+
+
+def test_zhang_li_torque_and_advection(mm):
+    # Eq. 26 (L327-L331, reading #19): torque and trajectory parity on a 3D multi-region box with open and
+    # periodic axes; with xi = alpha a spiral on a periodic chain is carried along at gamma u sin(k dx)/(k dx)
+    cfg = _rand_cfg((24, 12, 4), (4e-9, 3e-9, 2e-9), pbc=(0, 2, 0), nreg=3, anis=True, seed=12)
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    j, xi = (3e12, -1e12, 2e12), 0.3
+    sim.set_zhang_li(j, xi); ref.set_zhang_li(j, xi)
+    tq = sim.torque().astype(np.float64)
+    tr = ref.torque(ref.m) / ref.p.gamma_LL
+    assert np.abs(tq - tr).max() <= FIELD_TOL * np.abs(tr).max()
+    sim.set_zhang_li((0, 0, 0), xi)
+    assert np.abs(sim.torque() - tq).max() > 1e-3 * np.abs(tq).max()
+    sim.set_zhang_li(j, xi)
+    sim.set_solver(fix_dt=5e-14); ref.set_solver(fix_dt=5e-14)
+    sim.steps(30)
+    for _ in range(30):
+        ref.step()
+    assert np.abs(sim.get_m() - ref.m).max() < 5e-5
+    n, dx, Ms, alpha, jx = 64, 4e-9, 8e5, 0.1, 2e12
+    k = 2 * np.pi * 3 / (n * dx)
+    x = np.arange(n) * dx
+    m0 = np.zeros((3, 1, 1, n), dtype=np.float32); m0[0, 0, 0] = np.cos(k * x); m0[1, 0, 0] = np.sin(k * x)
+    p = Params.uniform(1, Msat=Ms, Aex=0.0, alpha=alpha)
+    sim = mm.from_config(dict(grid=(n, 1, 1), cell=(dx, dx, dx), pbc=(1, 0, 0), regions=None, params=p, m0=m0))
+    sim.set_terms(MM_ZEEMAN)
+    sim.set_zhang_li((jx, 0, 0), alpha)
+    sim.set_solver(max_err=1e-7)
+    v = 9.2740100783e-24 * jx / (2 * 1.602176634e-19 * Ms * (1 + alpha ** 2))        # gamma u, m/s
+    w = v * np.sin(k * dx) / dx
+    t = 1.0 / w
+    sim.run(t)
+    m = sim.get_m()
+    assert np.abs(m[0, 0, 0] - np.cos(k * x - w * t)).max() < 2e-5 and np.abs(m[2]).max() < 1e-5
