@@ -911,6 +911,6 @@ const char* mm_strerror(int code) {
   }
 }
 
-const char* mm_version(void) { return "mm_b200 0.1 (sm_100a)"; }
+const char* mm_version(void) { return "mm_b200 0.2 (sm_100a)"; }
 
 }  // extern "C"
