@@ -161,8 +161,9 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--size", type=int, default=4096)
-    ap.add_argument("--workload", default="c4", choices=["c4", "c5", "c5pbc"],
-                    help="c4: size x size x 1 film (default, the metric's workload); c5 / c5pbc: size^3 cube, open / PBC(4,4,0)")
+    ap.add_argument("--workload", default="c4", choices=["c4", "c5", "c5pbc", "c3"],
+                    help="c4: size x size x 1 film (default, the metric's workload); c5 / c5pbc: size^3 cube, open / "
+                         "PBC(4,4,0); c3: 128 x 128 x 32 multi-region block, adaptive steps (--size is ignored)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-size", type=int, default=256)
     ap.add_argument("--cpu-steps", type=int, default=36)
@@ -200,6 +201,13 @@ def main():
         cfg = config_c4(n, seed_offset=replicas.replica_seed(0, rank))     # one independent replica per rank
         cells, step_bytes = n * n, STEP_BYTES_PER_CELL
         wname = "C4 film %dx%dx1, 4x4x2 nm, Permalloy, random m, B_ext 10 mT, fix_dt 1e-13 s" % (n, n)
+    elif args.workload == "c3":
+        from synth import config_c3
+        cfg = config_c3()
+        cfg["fix_dt"] = 0.0                                   # adaptive RK45, MaxErr 1e-5; attempts are counted as steps
+        nx, ny, nz = cfg["grid"]
+        cells, step_bytes = nx * ny * nz, 2472.0
+        wname = "C3 block %dx%dx%d, 2 nm, 64 Voronoi regions, Ku1 + inter-region exchange, random m, adaptive RK45" % (nx, ny, nz)
     else:
         from synth import config_c5
         cfg = config_c5(n, pbc=args.workload == "c5pbc")
