@@ -18,9 +18,12 @@
  *     vector field is 3N floats and the region map N bytes.
  *   - Every array argument may be a HOST pointer or a DEVICE pointer (told apart with
  *     cudaPointerGetAttributes). The caller owns every buffer it passes; the library copies
- *     during the call and keeps no reference. The handle owns its device memory.
- *   - All work is enqueued on the handle's CUDA stream. Calls that return data to the caller
- *     (mm_get_*, mm_b_eff, mm_step_rk45 with info != NULL, mm_run) synchronise that stream.
+ *     during the call (the handle's stream is synchronised before an input call returns, for host
+ *     and device sources alike) and keeps no reference. The handle owns its device memory.
+ *   - All work is enqueued on the handle's CUDA stream: the one passed to mm_create_ex, or, if none
+ *     was passed, a stream the handle creates for itself (a blocking stream: it stays ordered with
+ *     work on the legacy default stream; mm_get_stream returns it). Calls that return data to the
+ *     caller (mm_get_*, mm_b_eff, mm_step_rk45 with info != NULL, mm_run) synchronise that stream.
  *   - Every call returns MM_OK (0) or a negative error code; nothing throws or aborts across the
  *     ABI. mm_last_error() gives a text for the last failure on a handle.
  *   - A handle is not thread-safe; distinct handles are independent.
@@ -109,7 +112,8 @@ int mm_set_terms(mm_sim* sim, unsigned term_mask);
 /* Implementation switches. MM_OPT_GENERIC_FFT = 1 forces the generic any-size convolution kernels
  * even where a specialised path exists (used by the tests to check the two against each other). */
 enum { MM_OPT_GENERIC_FFT = 1,
-       MM_OPT_NO_TMA = 2 /* fast 2D x kernels with plain loads/stores instead of TMA tensor copies */ };
+       MM_OPT_NO_TMA = 2 /* fast 2D x kernels with plain loads/stores instead of TMA tensor copies */,
+       MM_OPT_NO_GRAPH = 3 /* launch the kernels of a step one by one instead of replaying a CUDA graph */ };
 int mm_set_option(mm_sim* sim, int option, int value);
 
 /* Solver settings (L372-L374). max_err: MaxErr eps0 (default 1e-5); headroom (default 0.8);
@@ -146,8 +150,8 @@ int mm_set_slonczewski(mm_sim* sim, double jz, double pol, double lambda, double
  *   u = mu_B mu0 / (2 e gamma_LL Bsat (1 + xi^2)) j,
  * j [A/m^2] uniform current density (host pointer, 3 doubles), xi the non-adiabaticity. PAPER.md prints both
  * terms identically; the double cross product in the first is DESIGN.md reading #19. Central differences;
- * a missing neighbour at an open boundary is the cell's own m. Uses gamma_LL of the last mm_set_params.
- * j = 0 switches the term off. */
+ * a missing neighbour at an open boundary is the cell's own m. gamma_LL is the one in force when the
+ * torque is evaluated (a later mm_set_params takes effect). j = 0 switches the term off. */
 int mm_set_zhang_li(mm_sim* sim, const double j[3], double xi);
 
 /* Precession term of Eq. 2 on (default) or off: off leaves tau = -gamma alpha/(1+alpha^2) m x (m x B),
@@ -167,7 +171,10 @@ int mm_torque(mm_sim* sim, float* tau_over_gamma_out);
 
 /* One attempted Dormand-Prince step (L365). With info == NULL the step is only enqueued (no
  * synchronisation); otherwise the stream is synchronised and *info filled.
- * MM_ESTATE before mm_set_params + mm_set_m; MM_ENAN if the error estimate is not finite. */
+ * MM_ESTATE before mm_set_params + mm_set_m; MM_ENAN if the error estimate is not finite; MM_EDT if a
+ * rejected attempt was already at dt_min. After such a failure further steps are no-ops that report the
+ * same code until mm_set_solver or mm_set_m clears it; mm_b_eff, mm_torque, mm_energy and mm_max_torque
+ * keep working on the (unchanged) magnetisation. */
 int mm_step_rk45(mm_sim* sim, mm_step_info* info_or_null);
 /* The same call under a solver-neutral name: one attempted step of the selected pair. */
 int mm_step(mm_sim* sim, mm_step_info* info_or_null);
@@ -202,6 +209,8 @@ int mm_set_time(mm_sim* sim, double t);
 int mm_get_avg_m(mm_sim* sim, double avg[3]);
 /* Counters: accepted steps, rejected attempts, torque evaluations, peak device bytes owned. */
 int mm_get_stats(mm_sim* sim, long* steps, long* rejected, long* evals, size_t* peak_device_bytes);
+/* The CUDA stream all work of this handle is enqueued on (a cudaStream_t). */
+int mm_get_stream(mm_sim* sim, void** cuda_stream);
 /* Padded FFT sizes chosen for this box (Px, Py, Pz). */
 int mm_get_fft_size(mm_sim* sim, int P[3]);
 /* Number of kernel launches the library has issued on this handle (for bench.py). */
@@ -214,6 +223,7 @@ int mm_get_launch_count(mm_sim* sim, long* launches);
 int mm_profile(mm_sim* sim, int enable);
 int mm_profile_read(mm_sim* sim, int kind, const char** name, double* total_ms, long* launches);
 
+/* Text of the last failure on a handle; with sim == NULL, of the last failed mm_create on this thread. */
 const char* mm_last_error(const mm_sim* sim);
 const char* mm_strerror(int code);
 const char* mm_version(void);

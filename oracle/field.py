@@ -1,9 +1,13 @@
 """Effective-field terms, torque and energies, fp64, written out from the paper's definitions.
 Test infrastructure.  Arrays are [component][z][y][x]; `Lnnn` = PAPER.md line.
 """
+import os
+
 import numpy as np
+from scipy import fft as _fft          # same pocketfft routine as numpy.fft, with a `workers` argument
 
 MU0 = 4e-7 * np.pi
+FFT_WORKERS = int(os.environ.get("ORACLE_FFT_WORKERS", "0")) or (os.cpu_count() or 1)   # threads of the library FFT
 COMPS = (("xx", "xy", "xz"), ("xy", "yy", "yz"), ("xz", "yz", "zz"))
 
 
@@ -48,22 +52,23 @@ def kernel_spectrum(K, origin, P):
             d = np.arange(arr.shape[a]) - origin[a]          # displacement of every stored entry
             idx.append(np.mod(d, P[a]))
         buf[np.ix_(*idx)] = arr
-        Kp[k] = np.fft.rfftn(buf)
+        Kp[k] = _fft.rfftn(buf, workers=FFT_WORKERS)
     return Kp
 
 
 def b_demag_fft(M, K, origin, pbc, Kp=None):
-    """The same sum through the convolution theorem (L123) with numpy's fp64 FFT.
+    """The same sum through the convolution theorem (L123) with the library's fp64 FFT (scipy.fft = pocketfft,
+    threaded over the host cores; a library primitive, no blocking or reordering of the method here).
     `Kp` may carry the kernel spectrum computed once by kernel_spectrum()."""
     _, nz, ny, nx = M.shape
     P = padded_shape((nz, ny, nx), pbc)
     if Kp is None:
         Kp = kernel_spectrum(K, origin, P)
-    Mf = [np.fft.rfftn(M[j], s=P, axes=(0, 1, 2)) for j in range(3)]
+    Mf = [_fft.rfftn(M[j], s=P, axes=(0, 1, 2), workers=FFT_WORKERS) for j in range(3)]
     B = np.empty_like(M)
     for i in range(3):
         acc = sum(Kp[COMPS[i][j]] * Mf[j] for j in range(3))
-        B[i] = np.fft.irfftn(acc, s=P, axes=(0, 1, 2))[:nz, :ny, :nx]
+        B[i] = _fft.irfftn(acc, s=P, axes=(0, 1, 2), workers=FFT_WORKERS)[:nz, :ny, :nx]
     return B
 
 
@@ -108,6 +113,67 @@ def b_exchange(m, regions, L, cell, pbc):
                 w[tuple(sl)] = 0.0
             B += w[None] * (mi - m)
     return B
+
+
+# ---------------------------------------------------------------- Dzyaloshinskii-Moriya exchange (Eq. 10-17)
+def _neighbour_with_bc(m, live, axis, shift, d, periodic, bc):
+    """m of the neighbour cell at +shift along array axis `axis` (1 = z, 2 = y, 3 = x of [c][z][y][x]).
+
+    Where the neighbour is missing - outside an open box, or a cell without magnetisation (Msat = 0: geometry,
+    L53) - "its magnetization is replaced by m + dm/di|_dV Delta_i n" (L246) with the boundary derivatives of
+    Eq. 11-15 (bc = D / 2A of the central cell):
+        x boundary:  d(m_x, m_y, m_z)/dx = (-bc m_z, 0, bc m_x)      (Eq. 11, 13, 14)
+        y boundary:  d(m_x, m_y, m_z)/dy = (0, -bc m_z, bc m_y)      (Eq. 12, 13, 14)
+        z boundary:  0                                                (Eq. 15)
+    and n = shift the outward direction.  Returns (neighbour m, mask of cells whose neighbour is real)."""
+    n = m.shape[axis]
+    mi = np.roll(m, -shift, axis=axis)
+    real = np.roll(live, -shift, axis=axis - 1).copy()
+    if not periodic:
+        sl = [slice(None)] * 3
+        sl[axis - 1] = (n - 1) if shift == +1 else 0
+        real[tuple(sl)] = False
+    if axis == 3:
+        dm = np.stack([-bc * m[2], np.zeros_like(bc), bc * m[0]])
+    elif axis == 2:
+        dm = np.stack([np.zeros_like(bc), -bc * m[2], bc * m[1]])
+    else:
+        dm = np.zeros_like(m)
+    virtual = m + shift * d * dm
+    return np.where(real[None], mi, virtual), real
+
+
+def b_exchange_dmi(m, regions, L, cell, pbc, Msat, Aex, Dind):
+    """Heisenberg exchange (Eq. 6) plus the interfacial Dzyaloshinskii-Moriya field of Eq. 10,
+        B_DM = (2D / Msat) ( dm_z/dx, dm_z/dy, -dm_x/dx - dm_y/dy ),
+    with central differences (m_{i+1} - m_{i-1}) / (2 Delta_i) (L246) and the boundary conditions of Eq. 11-15,
+    which "in case of nonzero D ... are simultaneously applied to the Heisenberg exchange field" (L248).
+    Msat, Aex, Dind: per-region tables; D and D/2A are those of the central cell's region (#20)."""
+    Ms = Msat[regions]
+    live = Ms > 0
+    with np.errstate(divide="ignore", invalid="ignore"):
+        bc = np.where(live & (Aex[regions] > 0), Dind[regions] / (2.0 * Aex[regions]), 0.0)
+        cD = np.where(live, 2.0 * Dind[regions] / Ms, 0.0)
+    B = np.zeros_like(m)
+    for axis, d in ((3, cell[0]), (2, cell[1]), (1, cell[2])):
+        n = m.shape[axis]
+        periodic = pbc[3 - axis] > 0
+        if n == 1 and not periodic:
+            continue
+        nb = {}
+        for shift in (+1, -1):
+            mi, real = _neighbour_with_bc(m, live, axis, shift, d, periodic, bc)
+            ri = np.where(real, np.roll(regions, -shift, axis=axis - 1), regions)     # virtual neighbour: own material
+            B += ((2.0 / (d * d)) * L[regions, ri])[None] * (mi - m)                    # Eq. 6 / Eq. 9
+            nb[shift] = mi
+        diff = (nb[+1] - nb[-1]) / (2.0 * d)                                            # central difference (L246)
+        if axis == 3:      # d/dx
+            B[0] += cD * diff[2]
+            B[2] -= cD * diff[0]
+        elif axis == 2:    # d/dy
+            B[1] += cD * diff[2]
+            B[2] -= cD * diff[1]
+    return B * live[None]
 
 
 # ---------------------------------------------------------------- anisotropy (Eq. 18, 21)

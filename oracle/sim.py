@@ -79,6 +79,19 @@ class RefSim:
         self.temp, self.seed = 0.0, 0
         self.stt = None
         self.zl = None
+        self.Dind = None
+
+    def set_dmi(self, D):
+        """Interfacial Dzyaloshinskii-Moriya strength D [J/m^2] (Eq. 10): a scalar or one value per
+        region. Part of the exchange term (the paper's E_exch(DM), Eq. 16-17): MM_EXCH selects both."""
+        D = np.atleast_1d(np.asarray(D, dtype=np.float64))
+        self.Dind = None if not np.any(D) else (np.full(self.p.nregions, D[0]) if D.size == 1 else D.copy())
+        self.k1 = None
+
+    def b_exch(self, m):
+        if self.Dind is None:
+            return fld.b_exchange(m, self.regions, self.L, self.cell, self.pbc)
+        return fld.b_exchange_dmi(m, self.regions, self.L, self.cell, self.pbc, self.p.Msat, self.p.Aex, self.Dind)
 
     def set_slonczewski(self, jz, pol, lam=1.0, eps_prime=0.0, mp=(0, 0, 1)):
         """Spin-transfer torque of Eq. 28-30 (L336-L347): current density j_z [A/m^2] through the layer
@@ -168,7 +181,7 @@ class RefSim:
         if term_mask & MM_DEMAG:
             B += self.b_demag(m)
         if term_mask & MM_EXCH:
-            B += fld.b_exchange(m, self.regions, self.L, self.cell, self.pbc)
+            B += self.b_exch(m)
         if term_mask & MM_ANIS:
             B += fld.b_anis_uniaxial(m, self.regions, self.p) + fld.b_anis_cubic(m, self.regions, self.p)
         if term_mask & MM_ZEEMAN:
@@ -198,7 +211,7 @@ class RefSim:
         if terms & MM_DEMAG:
             e += -0.5 * (M * self.b_demag(m)).sum()                                            # Eq. 4
         if terms & MM_EXCH:
-            e += -0.5 * (M * fld.b_exchange(m, self.regions, self.L, self.cell, self.pbc)).sum()   # Eq. 8
+            e += -0.5 * (M * self.b_exch(m)).sum()                                             # Eq. 8 (+ Eq. 17)
         if terms & MM_ANIS:
             e += -0.5 * (M * fld.b_anis_uniaxial(m, self.regions, self.p, only=1)).sum()       # Eq. 20
             e += -0.25 * (M * fld.b_anis_uniaxial(m, self.regions, self.p, only=2)).sum()

@@ -15,6 +15,7 @@ MM_DEMAG, MM_EXCH, MM_ANIS, MM_ZEEMAN, MM_ALL = 1, 2, 4, 8, 15
 MM_MAX_REGIONS = 256
 MM_OPT_GENERIC_FFT = 1
 MM_OPT_NO_TMA = 2
+MM_OPT_NO_GRAPH = 3
 MM_RK45, MM_RK23, MM_RK12 = 0, 1, 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -84,6 +85,7 @@ _SIGNATURES = {
     "mm_get_avg_m": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
     "mm_get_stats": (C.c_int, [C.c_void_p, C.POINTER(C.c_long), C.POINTER(C.c_long), C.POINTER(C.c_long),
                                C.POINTER(C.c_size_t)]),
+    "mm_get_stream": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p)]),
     "mm_get_fft_size": (C.c_int, [C.c_void_p, C.POINTER(C.c_int)]),
     "mm_get_launch_count": (C.c_int, [C.c_void_p, C.POINTER(C.c_long)]),
     "mm_profile": (C.c_int, [C.c_void_p, C.c_int]),
@@ -166,7 +168,7 @@ class Sim:
         self.shape = (3, nz, ny, nx)
         self._h = C.c_void_p()
         dev = torch.cuda.current_device()
-        stream = torch.cuda.current_stream().cuda_stream
+        stream = torch.cuda.current_stream().cuda_stream     # 0 (the legacy default stream): the handle makes its own
         if use_torch_allocator:
             _new, _delete = torch.cuda.caching_allocator_alloc, torch.cuda.caching_allocator_delete
 
@@ -187,7 +189,15 @@ class Sim:
                                       self._cb[0], self._cb[1], None, C.c_void_p(stream))
         else:
             code = lib().mm_create(C.byref(self._h), nx, ny, nz, cell[0], cell[1], cell[2], pbc[0], pbc[1], pbc[2])
-        _check(code)
+        if code != MM_OK:
+            raise MMError(code, lib().mm_strerror(code).decode() + " (" + lib().mm_last_error(None).decode() + ")")
+
+    @property
+    def stream(self):
+        """torch view of the CUDA stream the handle enqueues its work on (for events around its kernels)."""
+        v = C.c_void_p()
+        _check(lib().mm_get_stream(self._h, C.byref(v)), self._h)
+        return self._torch.cuda.ExternalStream(v.value or 0)
 
     def close(self):
         if getattr(self, "_h", None) and self._h.value:

@@ -21,6 +21,8 @@ struct mm_sim {
   double cell[3];
   int rep[3];
   cudaStream_t stream = nullptr;
+  bool own_stream = false;     // created by mm_create (no stream was passed): destroyed with the handle
+  int nsm = 148;               // SMs of the device (grid sizing of the reductions and persistent kernels)
   void* (*alloc)(size_t, void*) = mm_default_alloc;
   void (*dealloc)(void*, void*) = mm_default_free;
   void* alloc_ctx = nullptr;
@@ -46,12 +48,17 @@ struct mm_sim {
   // host state
   DevState hst;
   bool have_params = false, have_m = false, have_k1 = false;
+  cudaGraphExec_t graph_exec = nullptr;   // one attempted step of the current configuration (mm_api.cu: step_once)
+  long graph_launches = 0;                // kernel launches inside it
+  bool graph_dirty = false;               // configuration changed: capture again
+  bool no_graph = false;                  // mm_set_option(MM_OPT_NO_GRAPH), or capture failed once
   unsigned terms = MM_ALL;
   int solver = MM_RK45;
   bool precession = true;
   double temperature = 0.0;
   bool zl_on = false;          // Zhang-Li torque enabled (mm_set_zhang_li)
-  float zl[4] = {};            // ZlArgs of local_rk.cuh
+  double zl_j[3] = {};         // current density [A/m^2] and non-adiabaticity as passed; the kernel arguments are
+  double zl_xi = 0.0;          // formed at launch time from the gamma_LL in force (mm_set_params may change it)
   bool stt_on = false;         // Slonczewski torque enabled (mm_set_slonczewski)
   float stt[7] = {};           // pref, pol, lam2, eps_prime, mp[3]  (SttArgs of local_rk.cuh)
   int nregions = 1;

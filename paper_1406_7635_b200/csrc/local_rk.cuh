@@ -425,6 +425,19 @@ __global__ void k_ctrl_end(DevState* st) {
   }
 }
 
+// largest region id of the map (validated against nregions without copying the map to the host)
+__global__ void k_max_region(long long N, const uint8_t* __restrict__ regions, unsigned* __restrict__ out) {
+  unsigned best = 0;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x)
+    best = max(best, (unsigned)regions[i]);
+  best = __reduce_max_sync(0xffffffffu, best);
+  if ((threadIdx.x & 31) == 0 && best > 0) atomicMax(out, best);
+}
+
+// diagnostics (mm_b_eff, mm_torque, mm_energy, mm_max_torque) evaluate fields whatever the state of the last
+// step: a failed step (MM_ENAN / MM_EDT) leaves skip = 1 until the error is cleared
+__global__ void k_clear_skip(DevState* st) { st->skip = 0; }
+
 // |m| = 1 on entry (L85); vacuum cells (Msat = 0) and zero vectors stay 0
 __global__ void k_normalise(long long N, float* __restrict__ m, const uint8_t* __restrict__ regions,
                             const Luts* __restrict__ lut) {

@@ -72,7 +72,7 @@ bool is_device_ptr(const void* p) {
 int copy_in(mm_sim* s, void* dst, const void* src, size_t bytes) {
   CUDA_TRY(s, cudaMemcpyAsync(dst, src, bytes, is_device_ptr(src) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice,
                               s->stream));
-  if (!is_device_ptr(src)) CUDA_TRY(s, cudaStreamSynchronize(s->stream));  // caller may free its buffer on return
+  CUDA_TRY(s, cudaStreamSynchronize(s->stream));  // host or device source: the caller may reuse or free it on return
   return MM_OK;
 }
 
@@ -193,7 +193,10 @@ void launch_eval(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_t
   }
   if (out_torque && s->zl_on) {       // Zhang-Li torque on top (Eq. 26)
     ZlArgs p;
-    p.c[0] = s->zl[0]; p.c[1] = s->zl[1]; p.c[2] = s->zl[2]; p.xi = s->zl[3];
+    const double muB = 9.2740100783e-24, e = 1.602176634e-19, mu0 = 4e-7 * M_PI, xi = s->zl_xi;
+    const double c = muB * mu0 / (2.0 * e * s->hst.gamma * (1.0 + xi * xi));           // u = c j / Bsat  [T m]
+    for (int a = 0; a < 3; ++a) p.c[a] = (float)(c * s->zl_j[a] / (2.0 * s->cell[a]));
+    p.xi = (float)xi;
     Launch l(s, KK_OTHER);
     k_add_zl<<<blocks_for(s->g.N, 256), 256, 0, s->stream>>>(s->g, s->regions, s->luts, s->dstate, src_role, dst_role, p);
   }
@@ -244,7 +247,7 @@ void enqueue_step(mm_sim* s) {
     ErrCoef ec;
     for (int j = 0; j < 7; ++j) ec.e[j] = 0.f;
     ec.e[0] = -0.5f; ec.e[1] = 0.5f;                          // 2nd-order minus Euler weights
-    { Launch l(s, KK_ERROR); k_error<<<148 * 8, 256, 0, s->stream>>>(N, s->dstate, ec); }
+    { Launch l(s, KK_ERROR); k_error<<<s->nsm * 8, 256, 0, s->stream>>>(N, s->dstate, ec); }
     { Launch l(s, KK_CTRL); k_ctrl_end<<<1, 1, 0, s->stream>>>(s->dstate); }
     s->have_k1 = false;
     return;
@@ -289,9 +292,40 @@ void enqueue_step(mm_sim* s) {
       { Launch l(s, KK_STAGE); k_stage<<<blocks_for(N, 256), 256, 0, s->stream>>>(N, s->dstate, sc, yrole); }
       launch_eval(s, yrole, R_K0 + i, s->terms, tq);
     }
-    { Launch l(s, KK_ERROR); k_error<<<148 * 8, 256, 0, s->stream>>>(N, s->dstate, ec); }
+    { Launch l(s, KK_ERROR); k_error<<<s->nsm * 8, 256, 0, s->stream>>>(N, s->dstate, ec); }
   }
   { Launch l(s, KK_CTRL); k_ctrl_end<<<1, 1, 0, s->stream>>>(s->dstate); }
+}
+
+// One attempted step through a CUDA graph of the launch sequence: all control is on the device (DevState), so the
+// sequence of a step is the same every time once the FSAL slope exists; small boxes are launch-bound
+// (PAPER.md L503 finds the same below 256 000 cells) and the replay removes the per-kernel launch cost.
+// Falls back to plain launches while profiling (events bracket every kernel) or if capture is unavailable.
+void drop_graph(mm_sim* s) {
+  if (s->graph_exec) { cudaGraphExecDestroy(s->graph_exec); s->graph_exec = nullptr; }
+  s->graph_dirty = false;
+}
+
+void step_once(mm_sim* s) {
+  const bool steady = s->have_k1 || s->solver == MM_RK12;      // Heun evaluates k1 inside every step
+  if (s->prof_on || s->no_graph || !steady) { enqueue_step(s); return; }
+  if (s->graph_dirty) drop_graph(s);
+  if (!s->graph_exec) {
+    const long before = s->launches;
+    if (cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+      cudaGetLastError(); s->no_graph = true; enqueue_step(s); return;
+    }
+    enqueue_step(s);
+    cudaGraph_t g = nullptr;
+    cudaError_t e = cudaStreamEndCapture(s->stream, &g);
+    s->graph_launches = s->launches - before;
+    s->launches = before;                                      // captured, not executed
+    if (e == cudaSuccess) e = cudaGraphInstantiate(&s->graph_exec, g, 0);
+    if (g) cudaGraphDestroy(g);
+    if (e != cudaSuccess) { cudaGetLastError(); s->graph_exec = nullptr; s->no_graph = true; enqueue_step(s); return; }
+  }
+  if (cudaGraphLaunch(s->graph_exec, s->stream) != cudaSuccess) { cudaGetLastError(); s->no_graph = true; drop_graph(s); enqueue_step(s); return; }
+  s->launches += s->graph_launches;
 }
 
 // thermal field: Heun and a fixed step only (L310)
@@ -299,6 +333,11 @@ int check_thermal(mm_sim* s) {
   if (s->temperature > 0 && (s->solver != MM_RK12 || !(s->hst.fix_dt > 0)))
     return mm_fail(s, MM_ESTATE, "a temperature needs the Heun solver (MM_RK12) and a fixed step (PAPER.md L310)");
   return MM_OK;
+}
+
+void clear_skip(mm_sim* s) {
+  Launch l(s, KK_OTHER);
+  k_clear_skip<<<1, 1, 0, s->stream>>>(s->dstate);
 }
 
 int check_ready(mm_sim* s) {
@@ -316,6 +355,8 @@ int status_to_error(mm_sim* s) {
 
 }  // namespace
 
+
+static thread_local std::string g_create_error;   // text of the last failed mm_create on this thread
 
 void* mm_default_alloc(size_t bytes, void*) {
   void* p = nullptr;
@@ -360,15 +401,30 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
                  void* cuda_stream) {
   if (!out) return MM_EINVAL;
   *out = nullptr;
+  g_create_error.clear();
   if (Nx < 1 || Ny < 1 || Nz < 1 || !(dx > 0) || !(dy > 0) || !(dz > 0) || pbc_x < 0 || pbc_y < 0 || pbc_z < 0 ||
       !std::isfinite(dx) || !std::isfinite(dy) || !std::isfinite(dz) || (dev_alloc_cb == nullptr) != (dev_free_cb == nullptr))
-    return MM_EINVAL;
+  { g_create_error = "bad grid size, cell size, PBC repeats or allocator pair"; return MM_EINVAL; }
   int ndev = 0;
-  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return MM_ECUDA; }
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); g_create_error = "no CUDA device"; return MM_ECUDA; }
   mm_sim* s = new (std::nothrow) mm_sim();
   if (!s) return MM_ENOMEM;
   if (dev_alloc_cb) { s->alloc = dev_alloc_cb; s->dealloc = dev_free_cb; s->alloc_ctx = alloc_ctx; }
   s->stream = (cudaStream_t)cuda_stream;
+  if (!s->stream) {
+    // No stream given: a stream of the handle's own. It is a blocking stream, so it stays ordered with work the
+    // caller issues on the legacy default stream (PyTorch's default), and unlike that one it can be captured
+    // into a CUDA graph (the step replay of mm_steps / mm_run).
+    if (cudaStreamCreate(&s->stream) != cudaSuccess) { cudaGetLastError(); delete s; g_create_error = "cudaStreamCreate"; return MM_ECUDA; }
+    s->own_stream = true;
+  }
+  {
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0)
+      s->nsm = nsm;
+    else
+      cudaGetLastError();
+  }
   s->cell[0] = dx; s->cell[1] = dy; s->cell[2] = dz;
   s->rep[0] = pbc_x; s->rep[1] = pbc_y; s->rep[2] = pbc_z;
   Geometry& g = s->g;
@@ -383,7 +439,7 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
   g.pbc[0] = pbc_x > 0; g.pbc[1] = pbc_y > 0; g.pbc[2] = pbc_z > 0;
   g.inv_dx2 = (float)(1.0 / (dx * dx)); g.inv_dy2 = (float)(1.0 / (dy * dy)); g.inv_dz2 = (float)(1.0 / (dz * dz));
   auto bail = [&](int code, const char* msg) {
-    fprintf(stderr, "mm_create: %s\n", msg);
+    g_create_error = msg;
     mm_destroy(s);
     return code;
   };
@@ -439,29 +495,41 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
 int mm_destroy(mm_sim* s) {
   if (!s) return MM_OK;
   cudaStreamSynchronize(s->stream);
+  drop_graph(s);
   for (auto& e : s->prof) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   for (auto& e : s->ev_pool) cudaEventDestroy(e);
   while (!s->owned.empty()) mm_dev_free(s, s->owned.back().first);
+  if (s->own_stream) cudaStreamDestroy(s->stream);
   delete s;
+  return MM_OK;
+}
+
+// largest region id of a map that lives on the device (4 bytes come back, not the map)
+static int max_region_on_device(mm_sim* s, const uint8_t* dev_regions, unsigned* out) {
+  unsigned* bits = reinterpret_cast<unsigned*>(s->scratch3);
+  CUDA_TRY(s, cudaMemsetAsync(bits, 0, sizeof(unsigned), s->stream));
+  { Launch l(s, KK_OTHER); k_max_region<<<s->nsm * 4, 256, 0, s->stream>>>(s->g.N, dev_regions, bits); }
+  CUDA_TRY(s, cudaGetLastError());
+  CUDA_TRY(s, cudaMemcpyAsync(out, bits, sizeof(unsigned), cudaMemcpyDeviceToHost, s->stream));
+  CUDA_TRY(s, cudaStreamSynchronize(s->stream));
   return MM_OK;
 }
 
 int mm_set_regions(mm_sim* s, const uint8_t* regions) {
   if (!s || !regions) return mm_fail(s, MM_EINVAL, "null argument");
-  // validate ids against the current table size on the host copy
-  std::vector<uint8_t> tmp;
-  const uint8_t* host = regions;
-  if (is_device_ptr(regions)) {
-    tmp.resize((size_t)s->g.N);
-    CUDA_TRY(s, cudaMemcpy(tmp.data(), regions, (size_t)s->g.N, cudaMemcpyDeviceToHost));
-    host = tmp.data();
-  }
+  // validate the ids against the current table size before the handle's map is touched
   if (s->have_params) {
-    for (long long i = 0; i < s->g.N; ++i)
-      if (host[i] >= s->nregions) return mm_fail(s, MM_EINVAL, "region id >= nregions");
+    unsigned top = 0;
+    if (is_device_ptr(regions)) {
+      int rc = max_region_on_device(s, regions, &top);
+      if (rc) return rc;
+    } else {
+      for (long long i = 0; i < s->g.N; ++i) top = regions[i] > top ? regions[i] : top;
+    }
+    if ((int)top >= s->nregions) return mm_fail(s, MM_EINVAL, "region id >= nregions");
   }
   int rc = copy_in(s, s->regions, regions, (size_t)s->g.N);
-  s->have_k1 = false;
+  s->have_k1 = false; s->graph_dirty = true;
   return rc;
 }
 
@@ -475,11 +543,12 @@ int mm_set_params(mm_sim* s, const mm_params* p) {
         !std::isfinite(p->Kc1[r]) || !std::isfinite(p->Kc2[r]) || !std::isfinite(p->Kc3[r]))
       return mm_fail(s, MM_EINVAL, "non-finite or negative material parameter");
   }
-  std::vector<uint8_t> reg((size_t)s->g.N);
-  CUDA_TRY(s, cudaMemcpyAsync(reg.data(), s->regions, (size_t)s->g.N, cudaMemcpyDeviceToHost, s->stream));
-  CUDA_TRY(s, cudaStreamSynchronize(s->stream));
-  for (long long i = 0; i < s->g.N; ++i)
-    if (reg[i] >= n) return mm_fail(s, MM_EINVAL, "region map holds an id >= nregions");
+  {
+    unsigned top = 0;
+    int rc = max_region_on_device(s, s->regions, &top);
+    if (rc) return rc;
+    if ((int)top >= n) return mm_fail(s, MM_EINVAL, "region map holds an id >= nregions");
+  }
   Luts* L = new (std::nothrow) Luts();
   if (!L) return mm_fail(s, MM_ENOMEM, "host LUT");
   memset(L, 0, sizeof(Luts));
@@ -532,14 +601,14 @@ int mm_set_params(mm_sim* s, const mm_params* p) {
   if ((rc = push_state(s))) return rc;
   s->nregions = n;
   s->have_params = true;
-  s->have_k1 = false;
+  s->have_k1 = false; s->graph_dirty = true;
   return MM_OK;
 }
 
 int mm_set_terms(mm_sim* s, unsigned mask) {
   if (!s) return MM_EINVAL;
   s->terms = mask & MM_ALL;
-  s->have_k1 = false;
+  s->have_k1 = false; s->graph_dirty = true;
   return MM_OK;
 }
 
@@ -552,7 +621,7 @@ int mm_set_solver_kind(mm_sim* s, int kind) {
   s->hst.nstage = kind == MM_RK23 ? 4 : (kind == MM_RK12 ? 2 : 7);
   s->hst.nevals = kind == MM_RK23 ? 3 : (kind == MM_RK12 ? 2 : 6);
   s->hst.expo = kind == MM_RK23 ? 1.0 / 3.0 : (kind == MM_RK12 ? 0.5 : 0.2);
-  s->have_k1 = false;
+  s->have_k1 = false; s->graph_dirty = true;
   return push_state(s);
 }
 
@@ -564,13 +633,13 @@ int mm_set_temperature(mm_sim* s, double kelvin, unsigned long long seed) {
   s->temperature = kelvin;
   s->hst.temperature = kelvin;
   s->hst.seed = seed;
-  s->have_k1 = false;
+  s->have_k1 = false; s->graph_dirty = true;
   return push_state(s);
 }
 
 int mm_set_slonczewski(mm_sim* s, double jz, double pol, double lambda, double eps_prime, const double mp[3]) {
   if (!s) return MM_EINVAL;
-  if (jz == 0) { s->stt_on = false; s->have_k1 = false; return MM_OK; }
+  if (jz == 0) { s->stt_on = false; s->have_k1 = false; s->graph_dirty = true; return MM_OK; }
   if (!mp || !std::isfinite(jz) || !std::isfinite(pol) || !(lambda > 0) || !std::isfinite(eps_prime))
     return mm_fail(s, MM_EINVAL, "bad spin-torque parameter");
   const double n = std::sqrt(mp[0] * mp[0] + mp[1] * mp[1] + mp[2] * mp[2]);
@@ -580,7 +649,7 @@ int mm_set_slonczewski(mm_sim* s, double jz, double pol, double lambda, double e
   s->stt[1] = (float)pol; s->stt[2] = (float)(lambda * lambda); s->stt[3] = (float)eps_prime;
   for (int c = 0; c < 3; ++c) s->stt[4 + c] = (float)(mp[c] / n);
   s->stt_on = true;
-  s->have_k1 = false;
+  s->have_k1 = false; s->graph_dirty = true;
   return MM_OK;
 }
 
@@ -588,14 +657,10 @@ int mm_set_zhang_li(mm_sim* s, const double j[3], double xi) {
   if (!s || !j) return mm_fail(s, MM_EINVAL, "null argument");
   if (!std::isfinite(j[0]) || !std::isfinite(j[1]) || !std::isfinite(j[2]) || !std::isfinite(xi))
     return mm_fail(s, MM_EINVAL, "bad spin-torque parameter");
-  s->have_k1 = false;
+  s->have_k1 = false; s->graph_dirty = true;
   if (j[0] == 0 && j[1] == 0 && j[2] == 0) { s->zl_on = false; return MM_OK; }
-  int rc;
-  if ((rc = pull_state(s))) return rc;
-  const double muB = 9.2740100783e-24, e = 1.602176634e-19, mu0 = 4e-7 * M_PI;
-  const double c = muB * mu0 / (2.0 * e * s->hst.gamma * (1.0 + xi * xi));           // u = c j / Bsat  [T m]
-  for (int a = 0; a < 3; ++a) s->zl[a] = (float)(c * j[a] / (2.0 * s->cell[a]));
-  s->zl[3] = (float)xi;
+  for (int a = 0; a < 3; ++a) s->zl_j[a] = j[a];
+  s->zl_xi = xi;
   s->zl_on = true;
   return MM_OK;
 }
@@ -603,7 +668,7 @@ int mm_set_zhang_li(mm_sim* s, const double j[3], double xi) {
 int mm_set_precession(mm_sim* s, int on) {
   if (!s) return MM_EINVAL;
   s->precession = on != 0;
-  s->have_k1 = false;
+  s->have_k1 = false; s->graph_dirty = true;
   return MM_OK;
 }
 
@@ -612,8 +677,9 @@ int mm_step(mm_sim* s, mm_step_info* info) { return mm_step_rk45(s, info); }
 int mm_set_option(mm_sim* s, int option, int value) {
   if (!s) return MM_EINVAL;
   switch (option) {
-    case MM_OPT_GENERIC_FFT: s->force_generic = value != 0; s->have_k1 = false; return MM_OK;
-    case MM_OPT_NO_TMA: s->f2_no_tma = value != 0; s->have_k1 = false; return MM_OK;
+    case MM_OPT_GENERIC_FFT: s->force_generic = value != 0; s->have_k1 = false; s->graph_dirty = true; return MM_OK;
+    case MM_OPT_NO_TMA: s->f2_no_tma = value != 0; s->have_k1 = false; s->graph_dirty = true; return MM_OK;
+    case MM_OPT_NO_GRAPH: s->no_graph = value != 0; return MM_OK;
     default: return mm_fail(s, MM_EINVAL, "unknown option");
   }
 }
@@ -631,7 +697,9 @@ int mm_set_solver(mm_sim* s, double max_err, double headroom, double fix_dt, dou
   h.dt_min = dt_min > 0 ? dt_min : 1e-18;
   h.dt_max = dt_max > 0 ? dt_max : 1e-9;
   h.dt = fix_dt > 0 ? fix_dt : (dt_init > 0 ? dt_init : 1e-14);
-  h.status = MM_OK;
+  h.status = MM_OK;     // a failed step (MM_ENAN / MM_EDT) is cleared here or by mm_set_m; its FSAL slope is not trusted
+  h.skip = 0;
+  s->have_k1 = false;
   return push_state(s);
 }
 
@@ -662,6 +730,7 @@ int mm_b_eff(mm_sim* s, unsigned mask, float* B_out) {
   int rc;
   if ((rc = check_ready(s))) return rc;
   if (!B_out) return mm_fail(s, MM_EINVAL, "null argument");
+  clear_skip(s);
   launch_eval(s, R_M, R_B, mask & MM_ALL, 0);
   CUDA_TRY(s, cudaGetLastError());
   if ((rc = pull_state(s))) return rc;
@@ -672,6 +741,7 @@ int mm_torque(mm_sim* s, float* out) {
   int rc;
   if ((rc = check_ready(s))) return rc;
   if (!out) return mm_fail(s, MM_EINVAL, "null argument");
+  clear_skip(s);
   launch_eval(s, R_M, R_Y, s->terms, s->precession ? 1 : 2);
   CUDA_TRY(s, cudaGetLastError());
   if ((rc = pull_state(s))) return rc;
@@ -681,7 +751,7 @@ int mm_torque(mm_sim* s, float* out) {
 int mm_step_rk45(mm_sim* s, mm_step_info* info) {
   int rc;
   if ((rc = check_ready(s)) || (rc = check_thermal(s))) return rc;
-  enqueue_step(s);
+  step_once(s);
   CUDA_TRY(s, cudaGetLastError());
   if (!info) return MM_OK;
   if ((rc = pull_state(s))) return rc;
@@ -695,7 +765,7 @@ int mm_steps(mm_sim* s, int n) {
   int rc;
   if ((rc = check_ready(s)) || (rc = check_thermal(s))) return rc;
   if (n < 0) return mm_fail(s, MM_EINVAL, "negative step count");
-  for (int i = 0; i < n; ++i) enqueue_step(s);
+  for (int i = 0; i < n; ++i) step_once(s);
   CUDA_TRY(s, cudaGetLastError());
   if ((rc = pull_state(s))) return rc;
   return status_to_error(s);
@@ -712,16 +782,21 @@ int mm_run(mm_sim* s, double duration) {
   s->hst.run_duration = duration;
   s->hst.skip = 0;
   if ((rc = push_state(s))) return rc;
-  int batch = 4;
+  // Steps are enqueued in batches sized from the remaining time and the controller's current suggestion, so that
+  // few (if any) attempts are enqueued past t_end (those return at once on the device, but small boxes are
+  // launch-bound); the host polls the device time once per batch.
   for (;;) {
-    for (int i = 0; i < batch; ++i) enqueue_step(s);
+    const double dt = s->hst.fix_dt > 0 ? s->hst.fix_dt : s->hst.dt;
+    const double est = (s->hst.t_end - s->hst.t) / (dt > 0 ? dt : 1e-18);
+    int batch;
+    if (s->hst.fix_dt > 0) batch = est > 64 ? 64 : (int)std::ceil(est - 1e-9);
+    else batch = est > 86 ? 64 : (int)std::floor(0.75 * est);       // the step may grow (fewer attempts) or be rejected
+    if (batch < 1) batch = 1;
+    for (int i = 0; i < batch; ++i) step_once(s);
     CUDA_TRY(s, cudaGetLastError());
     if ((rc = pull_state(s))) return rc;
     if (s->hst.skip || s->hst.status != MM_OK) break;
-    // size the next batch from the remaining time and the current step suggestion (host only polls)
-    double dt = s->hst.fix_dt > 0 ? s->hst.fix_dt : s->hst.dt;
-    double est = (s->hst.t_end - s->hst.t) / (dt > 0 ? dt : 1e-18);
-    batch = est > 256 ? 64 : (est > 32 ? 16 : 4);
+    if (!(s->hst.t_end - s->hst.t > 1e-12 * std::max(duration, 1e-30))) break;      // landed on t_end
   }
   const int st = s->hst.status;
   s->hst.run_mode = 0;
@@ -752,7 +827,7 @@ int mm_get_avg_m(mm_sim* s, double avg[3]) {
   int rc;
   if ((rc = pull_state(s))) return rc;
   CUDA_TRY(s, cudaMemsetAsync(s->scratch3, 0, 3 * sizeof(double), s->stream));
-  { Launch l(s, KK_OTHER); k_sum3<<<148 * 4, 256, 0, s->stream>>>(s->g.N, s->hst.ptr[R_M], s->scratch3); }
+  { Launch l(s, KK_OTHER); k_sum3<<<s->nsm * 4, 256, 0, s->stream>>>(s->g.N, s->hst.ptr[R_M], s->scratch3); }
   CUDA_TRY(s, cudaGetLastError());
   if ((rc = copy_out(s, avg, s->scratch3, 3 * sizeof(double)))) return rc;
   for (int c = 0; c < 3; ++c) avg[c] /= (double)s->g.N;
@@ -764,9 +839,10 @@ int mm_energy(mm_sim* s, unsigned mask, double* joules) {
   if ((rc = check_ready(s))) return rc;
   if (!joules) return mm_fail(s, MM_EINVAL, "null argument");
   mask &= MM_ALL;
+  clear_skip(s);
   if (mask & MM_DEMAG) launch_demag(s, R_M);
   CUDA_TRY(s, cudaMemsetAsync(s->scratch3, 0, 3 * sizeof(double), s->stream));
-  { Launch l(s, KK_OTHER); k_energy<<<148 * 8, 256, 0, s->stream>>>(s->g, s->regions, s->luts, s->dstate, R_M, R_B, mask, s->scratch3); }
+  { Launch l(s, KK_OTHER); k_energy<<<s->nsm * 8, 256, 0, s->stream>>>(s->g, s->regions, s->luts, s->dstate, R_M, R_B, mask, s->scratch3); }
   CUDA_TRY(s, cudaGetLastError());
   double e = 0.0;
   if ((rc = copy_out(s, &e, s->scratch3, sizeof(double)))) return rc;
@@ -779,10 +855,11 @@ int mm_max_torque(mm_sim* s, double* tesla) {
   if ((rc = check_ready(s))) return rc;
   if (!tesla) return mm_fail(s, MM_EINVAL, "null argument");
   if ((rc = pull_state(s))) return rc;
+  clear_skip(s);
   launch_eval(s, R_M, R_Y, s->terms, s->precession ? 1 : 2);
   unsigned* bits = reinterpret_cast<unsigned*>(s->scratch3);
   CUDA_TRY(s, cudaMemsetAsync(bits, 0, sizeof(unsigned), s->stream));
-  { Launch l(s, KK_OTHER); k_maxnorm<<<148 * 8, 256, 0, s->stream>>>(s->g.N, s->hst.ptr[R_Y], bits); }
+  { Launch l(s, KK_OTHER); k_maxnorm<<<s->nsm * 8, 256, 0, s->stream>>>(s->g.N, s->hst.ptr[R_Y], bits); }
   CUDA_TRY(s, cudaGetLastError());
   unsigned b = 0;
   if ((rc = copy_out(s, &b, bits, sizeof(unsigned)))) return rc;
@@ -801,19 +878,19 @@ int mm_relax(mm_sim* s) {
   const double err0 = s->hst.max_err, fix0 = s->hst.fix_dt;
   if ((rc = mm_set_solver_kind(s, MM_RK23))) return rc;
   s->precession = false;
-  s->have_k1 = false;
+  s->have_k1 = false; s->graph_dirty = true;
   auto set_err = [&](double max_err, double fix_dt) {
     int r = pull_state(s);
     if (r) return r;
     s->hst.max_err = max_err; s->hst.fix_dt = fix_dt;
     return push_state(s);
   };
-  auto advance = [&]() { for (int i = 0; i < 3; ++i) enqueue_step(s); };     // sampled every 3 steps (#15)
+  auto advance = [&]() { for (int i = 0; i < 3; ++i) step_once(s); };     // sampled every 3 steps (#15)
   auto finish = [&](int code) {
     s->precession = prec0;
     int r = mm_set_solver_kind(s, solver0);
     if (!r) r = set_err(err0, fix0);
-    s->have_k1 = false;
+    s->have_k1 = false; s->graph_dirty = true;
     return code ? code : r;
   };
   if ((rc = set_err(err0, 0.0))) return finish(rc);
@@ -851,6 +928,12 @@ int mm_get_stats(mm_sim* s, long* steps, long* rejected, long* evals, size_t* pe
   if (rejected) *rejected = (long)s->hst.rejected;
   if (evals) *evals = (long)s->hst.evals + s->extra_evals;
   if (peak) *peak = s->peak_bytes;
+  return MM_OK;
+}
+
+int mm_get_stream(mm_sim* s, void** cuda_stream) {
+  if (!s || !cuda_stream) return MM_EINVAL;
+  *cuda_stream = (void*)s->stream;
   return MM_OK;
 }
 
@@ -896,7 +979,7 @@ int mm_profile_read(mm_sim* s, int kind, const char** name, double* total_ms, lo
   return MM_OK;
 }
 
-const char* mm_last_error(const mm_sim* s) { return s ? s->err.c_str() : "null handle"; }
+const char* mm_last_error(const mm_sim* s) { return s ? s->err.c_str() : g_create_error.c_str(); }
 
 const char* mm_strerror(int code) {
   switch (code) {

@@ -5,6 +5,8 @@ Tolerances (DESIGN.md "Tolerances"):
   <m>     |d<m>| <= 1e-3 at equal physical time (north_star, C2);
   m(t)    element-wise bounds stated at each test (fp32 round-off amplified by the dynamics).
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -106,7 +108,8 @@ def test_multi_tile_2d_and_3d_fields(mm):
 
 
 @pytest.mark.parametrize("grid", [(256, 256, 1), (512, 256, 1), (256, 1024, 1), (2048, 256, 1), (256, 4096, 1),
-                                  (4096, 256, 1), (1024, 1024, 1), (384, 320, 1), (1000, 600, 1), (66, 1536, 1)])
+                                  (4096, 256, 1), (1024, 1024, 1), (384, 320, 1), (1000, 600, 1), (66, 1536, 1),
+                                  (3000, 256, 1), (2048, 3000, 1), (1536, 1536, 1)])
 def test_fast2d_path_fields(mm, grid):
     # open 2D films take the register-FFT kernels (fast2d.cuh); several CTAs per kernel, rectangular
     # shapes exercise every plan on either axis; regions exercise the B_sat gather; sizes that are not
@@ -171,8 +174,9 @@ def _direct_sum_at(cells, M, cell):
 
 
 def test_c4_full_size_sampled_cells(mm):
-    # the bench workload and launch configuration (4096 x 4096 x 1, fast 2D kernels): sampled cells
-    # against the plain double sum; corners, edges, tile seams and interior points
+    # the bench workload and launch configuration (4096 x 4096 x 1, fast 2D kernels): sampled cells against
+    # the plain double sum - corners, edges, interior points and every seam of the x kernels' CTAs (rows 4k and
+    # 4k + 3 of the forward kernel, 2k and 2k + 1 of the inverse one) - for the demag field and for all terms
     n = 4096
     cfg = config_c4(n)
     sim = mm.from_config(cfg)
@@ -181,19 +185,118 @@ def test_c4_full_size_sampled_cells(mm):
     assert "f2_ycol" in sim.profile_read()
     sim.profile(False)
     p = cfg["params"]
-    M = (4e-7 * np.pi * float(np.atleast_1d(p.Msat)[0])) * cfg["m0"].astype(np.float64)
-    cells = [(0, 0), (n - 1, n - 1), (0, n - 1), (2047, 2048), (255, 256), (1000, 3), (4095, 1777), (3071, 513)]
+    Ms, A = float(np.atleast_1d(p.Msat)[0]), float(np.atleast_1d(p.Aex)[0])
+    m = cfg["m0"].astype(np.float64)
+    M = (4e-7 * np.pi * Ms) * m
+    cells = [(0, 0), (n - 1, n - 1), (0, n - 1), (n - 1, 0), (2047, 2048), (255, 256), (1000, 3), (4095, 1777), (3071, 513)]
+    rng = np.random.default_rng(44)
+    for k in rng.integers(0, n // 4, size=14):           # CTA seams of both x kernels
+        cells += [(int(rng.integers(0, n)), 4 * int(k)), (int(rng.integers(0, n)), 4 * int(k) + 3),
+                  (int(rng.integers(0, n)), 4 * int(k) + 1), (int(rng.integers(0, n)), 4 * int(k) + 2)]
+    for k in (0, 255, 256, 1023, 1024, 4095):            # stripes of the register layout along x (thread t +- 1, t = 0, 255)
+        cells.append((k, int(rng.integers(0, n))))
+    assert len(cells) >= 64
     Br = _direct_sum_at(cells, M, cfg["cell"])
     scale = np.abs(B).max()
     for (ix, iy), br in zip(cells, Br):
         err = np.abs(B[:, iy, ix] - br).max() / scale
         assert err <= FIELD_TOL, ((ix, iy), err)
-    # properties that hold at any size: the full field (exchange of random m ~ 10 T dominates) stays
-    # finite everywhere and the step keeps |m| = 1
+    # all terms at the same cells: demag (above) + exchange (Eq. 6, Neumann edges) + Zeeman, written out per cell
+    Ball = sim.b_eff(MM_ALL).astype(np.float64).reshape(3, n, n)
+    dx, dy = cfg["cell"][0], cfg["cell"][1]
+    mm_ = m[:, 0]
+    worst = 0.0
+    for (ix, iy), br in zip(cells, Br):
+        ex = np.zeros(3)
+        for (jx, jy, d) in ((ix + 1, iy, dx), (ix - 1, iy, dx), (ix, iy + 1, dy), (ix, iy - 1, dy)):
+            if 0 <= jx < n and 0 <= jy < n:
+                ex += 2 * A / Ms / (d * d) * (mm_[:, jy, jx] - mm_[:, iy, ix])
+        want = br + ex + np.asarray(p.B_ext, dtype=np.float64)
+        worst = max(worst, np.abs(Ball[:, iy, ix] - want).max())
+    assert worst <= FIELD_TOL * np.abs(Ball).max(), worst
+    # properties that hold at any size: the step keeps |m| = 1 and everything stays finite
     sim.set_solver(fix_dt=cfg["fix_dt"])
     sim.steps(2)
-    m = sim.get_m().reshape(3, -1)
-    assert np.isfinite(m).all() and abs(np.linalg.norm(m, axis=0) - 1).max() < 1e-6
+    mg = sim.get_m().reshape(3, -1)
+    assert np.isfinite(mg).all() and abs(np.linalg.norm(mg, axis=0) - 1).max() < 1e-6
+
+
+def _direct_sum_at_3d(cells, M, cell):
+    """Eq. 3 (L121-L123) written out for single destination cells of an open 3D box: the sum over ALL source
+    cells with the oracle's tensor K = -N evaluated on the (|dx|, |dy|, |dz|) octant (in z slabs) and the
+    parity of each component restored by sign factors."""
+    from oracle.demag_tensor import tensor
+    _, nz, ny, nx = M.shape
+    keys = ("xx", "yy", "zz", "xy", "xz", "yz")
+    K = {k: np.empty((nz, ny, nx)) for k in keys}
+    X = (np.arange(nx) * cell[0])[None, None, :]
+    Y = (np.arange(ny) * cell[1])[None, :, None]
+    for z0 in range(0, nz, 8):
+        Z = (np.arange(z0, min(nz, z0 + 8)) * cell[2])[:, None, None]
+        T = tensor(X + 0 * Y + 0 * Z, Y + 0 * X + 0 * Z, Z + 0 * X + 0 * Y, cell)
+        for k in keys:
+            K[k][z0:z0 + Z.shape[0]] = -T[k]
+    comps = (("xx", "xy", "xz"), ("xy", "yy", "yz"), ("xz", "yz", "zz"))
+    par = dict(xx=(0, 0, 0), yy=(0, 0, 0), zz=(0, 0, 0), xy=(1, 1, 0), xz=(1, 0, 1), yz=(0, 1, 1))
+    out = []
+    for (ix, iy, iz) in cells:
+        dxs, dys, dzs = ix - np.arange(nx), iy - np.arange(ny), iz - np.arange(nz)
+        sel = np.ix_(np.abs(dzs), np.abs(dys), np.abs(dxs))
+        sg = (np.where(dxs < 0, -1.0, 1.0)[None, None, :], np.where(dys < 0, -1.0, 1.0)[None, :, None],
+              np.where(dzs < 0, -1.0, 1.0)[:, None, None])
+        b = np.zeros(3)
+        for i in range(3):
+            for j in range(3):
+                k = comps[i][j]
+                kk = K[k][sel]
+                for a in range(3):
+                    if par[k][a]:
+                        kk = kk * sg[a]
+                b[i] += (kk * M[j]).sum()
+        out.append(b)
+    return np.array(out)
+
+
+def test_c5_cubes_at_the_benchmarked_sizes(mm):
+    # BASELINE.json config 5 at the sizes the sweep times: 128^3 open and with PBC (4,4,0) against the oracle's
+    # own FFT field everywhere; 256^3 open (16.8 M cells) on sampled cells against the plain triple sum
+    for pbc in (False, True):
+        cfg = config_c5(128, pbc=pbc)
+        sim = mm.from_config(cfg)
+        ref = _ref_from(cfg, "fft")
+        _field_check(sim, ref, (MM_DEMAG, MM_ALL))
+        del sim, ref
+    n = 256
+    cfg = config_c5(n)
+    sim = mm.from_config(cfg)
+    B = sim.b_eff(MM_DEMAG).astype(np.float64)
+    Ms = float(np.atleast_1d(cfg["params"].Msat)[0])
+    M = (4e-7 * np.pi * Ms) * cfg["m0"].astype(np.float64)
+    cells = [(0, 0, 0), (n - 1, n - 1, n - 1), (n - 1, 0, 17), (127, 128, 128), (3, 200, 255), (64, 31, 1)]
+    Br = _direct_sum_at_3d(cells, M, cfg["cell"])
+    scale = np.abs(B).max()
+    for (ix, iy, iz), br in zip(cells, Br):
+        err = np.abs(B[:, iz, iy, ix] - br).max() / scale
+        assert err <= FIELD_TOL, ((ix, iy, iz), err)
+
+
+def test_direct_sum_helpers_agree_with_the_oracle_field():
+    # the sampled-cell sums used at full size, checked against the oracle's own field on small boxes
+    cfg = _rand_cfg((20, 12, 5), (2e-9, 3e-9, 4e-9), nreg=1, seed=3)
+    ref = _ref_from(cfg, "fft")
+    Br = ref.b_eff(MM_DEMAG)
+    M = (4e-7 * np.pi * cfg["params"].Msat[0]) * ref.m
+    cells = [(0, 0, 0), (19, 11, 4), (7, 3, 2), (19, 0, 1)]
+    got = _direct_sum_at_3d(cells, M, cfg["cell"])
+    for (ix, iy, iz), b in zip(cells, got):
+        assert np.abs(b - Br[:, iz, iy, ix]).max() < 1e-10 * np.abs(Br).max()
+    cfg = _rand_cfg((24, 10, 1), (4e-9, 3e-9, 2e-9), nreg=1, seed=4)
+    ref = _ref_from(cfg, "fft")
+    Br = ref.b_eff(MM_DEMAG)
+    M = (4e-7 * np.pi * cfg["params"].Msat[0]) * ref.m
+    got = _direct_sum_at([(0, 0), (23, 9), (11, 4)], M, cfg["cell"])
+    for (ix, iy), b in zip([(0, 0), (23, 9), (11, 4)], got):
+        assert np.abs(b - Br[:, 0, iy, ix]).max() < 1e-10 * np.abs(Br).max()
 
 
 def test_uniform_m_has_no_exchange_field_and_film_limit(mm):
@@ -350,7 +453,52 @@ def test_c3_reduced_adaptive_steps(mm):
     assert np.abs(m - ref.m).max() < 5e-3 and np.abs(sim.avg_m() - ref.avg_m()).max() < 1e-3
 
 
+@pytest.mark.skipif(not os.environ.get("MM_SLOW_TESTS"), reason="about 20 min of fp64 oracle steps; set MM_SLOW_TESTS=1 "
+                    "(run once per round under gpurun, log kept under profiles/)")
+def test_c3_as_stated_full_size_100_adaptive_steps(mm):
+    # BASELINE.json config 3 as stated: 128 x 128 x 32 cells, 64 Voronoi grains, random m, 100 adaptive RK45
+    # attempts on the GPU, then the oracle runs to the same physical time (reading #10)
+    cfg = config_c3()
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    sim.steps(cfg["nsteps"])
+    st = sim.stats()
+    assert st["steps"] + st["rejected"] == cfg["nsteps"]
+    ref.run(sim.t)
+    m = sim.get_m().astype(np.float64)
+    dm, davg = np.abs(m - ref.m).max(), np.abs(sim.avg_m() - ref.avg_m()).max()
+    print("C3 as stated: t = %.4e s, GPU steps %d (+%d rejected), oracle steps %d (+%d), max|dm| = %.3e, |d<m>| = %.3e"
+          % (sim.t, st["steps"], st["rejected"], ref.n_steps, ref.n_rejected, dm, davg))
+    assert davg <= 1e-3 and dm < 5e-3
+
+
 # --------------------------------------------------------------------------- boundary behaviour
+def test_failed_step_leaves_the_handle_usable(mm):
+    # a step that fails with MM_EDT (rejected at dt_min) must not poison the diagnostics: fields, torque and
+    # energy of the unchanged magnetisation still come out right, and clearing the error resumes stepping
+    cfg = _rand_cfg((32, 16, 1), (4e-9, 4e-9, 3e-9), nreg=2, seed=23)
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    sim.set_solver(max_err=1e-12, dt_init=2e-13, dt_min=2e-13)
+    with pytest.raises(mm.MMError) as e:
+        sim.step()
+    assert e.value.code == mm.MM_EDT
+    with pytest.raises(mm.MMError) as e:
+        sim.steps(3)                                     # still refused, still no-ops
+    assert e.value.code == mm.MM_EDT
+    assert np.abs(sim.get_m() - ref.m).max() < 1e-6      # nothing moved
+    _field_check(sim, ref, (MM_DEMAG, MM_ALL))
+    tq = sim.torque().astype(np.float64)
+    tr = ref.torque(ref.m) / ref.p.gamma_LL
+    assert np.abs(tq - tr).max() <= FIELD_TOL * np.abs(tr).max()
+    assert abs(sim.energy() - ref.energy()) <= 1e-5 * abs(ref.energy())
+    sim.set_solver(fix_dt=1e-13); ref.set_solver(fix_dt=1e-13)       # clears the error
+    sim.steps(5)
+    for _ in range(5):
+        ref.step()
+    assert np.abs(sim.get_m() - ref.m).max() < 2e-5 and abs(sim.t - 5e-13) < 1e-24
+
+
 def test_error_codes_and_state(mm):
     sim = mm.Sim((8, 4, 1), (2e-9, 2e-9, 2e-9))
     with pytest.raises(mm.MMError) as e:
