@@ -9,8 +9,8 @@ namespace {
 // per length: the radix plan (T threads and 16 points per thread for one pair of transforms) and
 // the CTA size NT; a CTA holds G = NT / T FFT groups and therefore 2G rows in the x kernels
 template <int N> struct PlanFor;
-// (NTF: the forward x kernel, whose transposed store wants at least 4 rows = 32-byte pieces)
-template <> struct PlanFor<4096> { using P = rf::Plan<4096, 256, 16, 16, 16>; static constexpr int NT = 256, NTF = 512, NTI = 256; };
+// (NTF: CTA size of the forward x kernel, four rows per FFT group; NTI: of the inverse one, two rows per group)
+template <> struct PlanFor<4096> { using P = rf::Plan<4096, 256, 16, 16, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
 template <> struct PlanFor<2048> { using P = rf::Plan<2048, 128, 16, 8, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
 template <> struct PlanFor<1024> { using P = rf::Plan<1024, 64, 16, 4, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
 template <> struct PlanFor<512> { using P = rf::Plan<512, 32, 16, 2, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
@@ -35,8 +35,9 @@ std::vector<float2> plan_table() {
 }
 
 // 3-D TMA view of spec: floats along y innermost (2 per bin), then kx, then component; one box =
-// {rows * 2 floats, K2_KB bins, 1}. Returns false if the driver entry point is unavailable.
-bool make_spec_map(mm_sim* s, int rows, CUtensorMap* out) {
+// {rows * 2 floats, kb bins, 1}. The view starts at column kx0 and walks every kstep-th column (nk of them).
+// Returns false if the driver entry point is unavailable.
+bool make_spec_map(mm_sim* s, int rows, CUtensorMap* out, int kb = K2_KB, int kx0 = 0, int kstep = 1, int nk = -1) {
   typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -48,11 +49,12 @@ bool make_spec_map(mm_sim* s, int rows, CUtensorMap* out) {
     return false;
   }
   const Fast2DArgs& a = s->f2;
-  const cuuint64_t dims[3] = {(cuuint64_t)2 * a.Ny, (cuuint64_t)a.Cx, 3};
-  const cuuint64_t strides[2] = {(cuuint64_t)a.Ny * sizeof(float2), (cuuint64_t)a.cstride * sizeof(float2)};
-  const cuuint32_t box[3] = {(cuuint32_t)(2 * rows), (cuuint32_t)K2_KB, 1};
+  if (nk < 0) nk = a.Cx;
+  const cuuint64_t dims[3] = {(cuuint64_t)2 * a.Ny, (cuuint64_t)nk, 3};
+  const cuuint64_t strides[2] = {(cuuint64_t)kstep * a.Ny * sizeof(float2), (cuuint64_t)a.cstride * sizeof(float2)};
+  const cuuint32_t box[3] = {(cuuint32_t)(2 * rows), (cuuint32_t)kb, 1};
   const cuuint32_t estr[3] = {1, 1, 1};
-  return ((EncodeFn)fn)(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)a.spec, dims, strides, box, estr,
+  return ((EncodeFn)fn)(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)(a.spec + (size_t)kx0 * a.Ny), dims, strides, box, estr,
                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
@@ -92,14 +94,11 @@ int axis_tables(mm_sim* s, int N, float2** fwd, float2** rev, float2** half) {
 template <int N>
 int x_attrs(mm_sim* s) {
   using F = PlanFor<N>;
-  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd<typename F::P, F::NTF, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   (int)k2_smem<typename F::P, F::NTF>()));
-  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd<typename F::P, F::NTF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   (int)k2_smem<typename F::P, F::NTF>()));
-  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd_tma<typename F::P, F::NTF, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   (int)k2_tma_store_smem<typename F::P, F::NTF>()));
-  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd_tma<typename F::P, F::NTF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   (int)k2_tma_store_smem<typename F::P, F::NTF>()));
+  const int fb = (int)k2_fwd_smem<typename F::P, F::NTF>();
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd4<typename F::P, F::NTF, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fb));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd4<typename F::P, F::NTF, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fb));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd4<typename F::P, F::NTF, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fb));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd4<typename F::P, F::NTF, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fb));
   CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv<typename F::P, F::NTI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    (int)k2_smem<typename F::P, F::NTI>()));
   CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv_tma<typename F::P, F::NTI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -117,18 +116,20 @@ int y_attrs(mm_sim* s) {
 template <int N>
 void launch_x(mm_sim* s, bool inverse, int role) {
   using F = PlanFor<N>;
-  constexpr int GF = F::NTF / F::P::T, GI = F::NTI / F::P::T;
-  const dim3 gf(s->g.Ny / (2 * GF), 3);
+  constexpr int GI = F::NTI / F::P::T;
+  constexpr int ROWS = K2Fwd<typename F::P, F::NTF>::ROWS;
   const bool ragged = s->f2.nxp < s->f2.Nx;
   const bool tma_on = s->f2_tma && !s->f2_no_tma;
-  if (!inverse && tma_on) {
-    const size_t b = k2_tma_store_smem<typename F::P, F::NTF>();
-    if (ragged) k2_xfwd_tma<typename F::P, F::NTF, true><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd);
-    else k2_xfwd_tma<typename F::P, F::NTF, false><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd);
-  } else if (!inverse) {
-    const size_t b = k2_smem<typename F::P, F::NTF>();
-    if (ragged) k2_xfwd<typename F::P, F::NTF, true><<<gf, F::NTF, b, s->stream>>>(s->f2, role);
-    else k2_xfwd<typename F::P, F::NTF, false><<<gf, F::NTF, b, s->stream>>>(s->f2, role);
+  if (!inverse) {
+    const dim3 gf((s->g.Ny + ROWS - 1) / ROWS, 3);
+    const size_t b = k2_fwd_smem<typename F::P, F::NTF>();
+    if (tma_on) {
+      if (ragged) k2_xfwd4<typename F::P, F::NTF, true, true><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd, s->f2_map_fwd_odd);
+      else k2_xfwd4<typename F::P, F::NTF, false, true><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd, s->f2_map_fwd_odd);
+    } else {
+      if (ragged) k2_xfwd4<typename F::P, F::NTF, true, false><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd, s->f2_map_fwd_odd);
+      else k2_xfwd4<typename F::P, F::NTF, false, false><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd, s->f2_map_fwd_odd);
+    }
   }
   else if (tma_on)
     k2_xinv_tma<typename F::P, F::NTI><<<dim3(s->g.Ny / (2 * GI), 3), F::NTI, k2_tma_smem<typename F::P, F::NTI>(), s->stream>>>(s->f2, role, s->f2_map_inv);
@@ -145,16 +146,22 @@ void launch_y(mm_sim* s) {
 }
 
 template <int N> constexpr int rows_inv_of() { return 2 * (PlanFor<N>::NTI / PlanFor<N>::P::T); }
-template <int N> constexpr int rows_of() { return 2 * (PlanFor<N>::NTF / PlanFor<N>::P::T); }   // NTF >= NT
-int rows_per_cta(int N) {
+int rows_per_cta(int N) {      // rows of one CTA of the x inverse kernel (the forward kernel pads its last CTA with zero rows)
   switch (N) {
-    case 4096: return rows_of<4096>();
-    case 2048: return rows_of<2048>();
-    case 1024: return rows_of<1024>();
-    case 512: return rows_of<512>();
-    case 256: return rows_of<256>();
+    case 4096: return rows_inv_of<4096>();
+    case 2048: return rows_inv_of<2048>();
+    case 1024: return rows_inv_of<1024>();
+    case 512: return rows_inv_of<512>();
+    case 256: return rows_inv_of<256>();
   }
   return 0;
+}
+
+template <int N>
+bool make_fwd_maps(mm_sim* s) {
+  using F = K2Fwd<typename PlanFor<N>::P, PlanFor<N>::NTF>;
+  return make_spec_map(s, F::ROWS, &s->f2_map_fwd, F::KB, 0, 2, N / 2 + 1) &&
+         make_spec_map(s, F::ROWS, &s->f2_map_fwd_odd, F::KB, 1, 2, N / 2);
 }
 
 }  // namespace
@@ -216,7 +223,11 @@ int mm_fast2d_init(mm_sim* s) {
 #define RI(N) rows_inv = rows_inv_of<N>()
   F2_SWITCH(a.Nx, RI)
 #undef RI
-  s->f2_tma = make_spec_map(s, rows_inv, &s->f2_map_inv) && make_spec_map(s, rows_per_cta(a.Nx), &s->f2_map_fwd);
+  bool fwd_ok = false;
+#define FM(N) fwd_ok = make_fwd_maps<N>(s)
+  F2_SWITCH(a.Nx, FM)
+#undef FM
+  s->f2_tma = make_spec_map(s, rows_inv, &s->f2_map_inv) && fwd_ok;
   return MM_OK;
 }
 

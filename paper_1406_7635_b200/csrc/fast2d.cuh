@@ -45,76 +45,6 @@ __device__ __forceinline__ float4 separate(float2 z, float2 zm) {
   return make_float4(0.5f * (z.x + zm.x), 0.5f * (z.y - zm.y), 0.5f * (z.y + zm.y), 0.5f * (zm.x - z.x));
 }
 
-// ---------------------------------------------------------------------------------- K_A
-// RAGGED: the film is narrower than the transform (nxp < N): columns beyond are zero fill
-template <class P, int NT, bool RAGGED>
-__global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd(Fast2DArgs a, int src_role) {
-  if (a.st->skip) return;
-  constexpr int N = P::N, T = P::T, E = P::E, G = NT / T, GP = K2Shape<P, NT>::GP;
-  extern __shared__ float4 smem4[];
-  __shared__ float bsat_s[MM_MAX_REGIONS];
-  const int tid = threadIdx.x, gid = tid / T, t = tid % T;
-  float4* xb = smem4 + (size_t)gid * GP;
-  const int c = blockIdx.y, r0 = blockIdx.x * 2 * G;
-  const float* __restrict__ src = a.st->ptr[src_role] + (size_t)c * a.ncell;
-  const uint8_t* __restrict__ reg = a.regions;
-  const bool uniform = a.luts->nregions == 1;       // one region: B_sat is a constant
-  const float b0 = a.luts->Bsat[0];
-  if (!uniform) {
-    for (int i = tid; i < MM_MAX_REGIONS; i += NT) bsat_s[i] = a.luts->Bsat[i];
-    __syncthreads();
-  }
-  {
-    const size_t rowA = (size_t)(r0 + 2 * gid) * a.nxp;      // physical row pitch; n >= nxp is zero fill
-    rf::C2 v[E];
-    const float2 wt = __ldg(&a.twox[t]);      // w_2N^t; the other points follow from constants
-#pragma unroll
-    for (int e = 0; e < E; ++e) {
-      const int n = rf::slot_index<P, P::RA>(t, e);
-      float2 z = make_float2(0.f, 0.f);
-      if (!RAGGED || n < a.nxp) {
-        const size_t iA = rowA + n, iB = iA + a.nxp;
-        const float sa = uniform ? b0 : bsat_s[reg[iA]], sb = uniform ? b0 : bsat_s[reg[iB]];
-        z = make_float2(src[iA] * sa, src[iB] * sb);            // M = B_sat m (L121)
-      }
-      const float2 zw = rf::cmul_tw1<-1>(z, rf::half_twiddle(wt, e));
-      v[e] = {make_float2(z.x, zw.x), make_float2(z.y, zw.y)};
-    }
-    rf::fft<P, -1, NT>(v, xb, t, gid, a.twx);
-    rf::group_sync<T, NT>(gid);
-#pragma unroll
-    for (int e = 0; e < E; ++e) xb[rf::slot_index<P, P::RLAST>(t, e)] = stage_pack(v[e]);
-  }
-  __syncthreads();
-  // separate the two real rows of every pair and store transposed: lane 0 holds bin kx = 2k,
-  // lane 1 bin kx = 2k + 1 of the padded transform; stored kx = 0 .. N
-  float2* __restrict__ out = a.spec + (size_t)c * a.cstride;
-  // (N/2) G items (k, p) over NT = G N/16 threads: exactly 8 per thread; all shared-memory reads first
-  constexpr int IT = (N / 2) * G / NT;
-  static_assert(IT * NT == (N / 2) * G, "items must divide evenly");
-  float4 u[IT]; float2 zm0[IT], zm1[IT];
-#pragma unroll
-  for (int it = 0; it < IT; ++it) {
-    const int w = tid + it * NT, p = w % G, k = w / G;
-    const float4* st = smem4 + (size_t)p * GP;
-    const float2* st2 = reinterpret_cast<const float2*>(st);
-    u[it] = st[k];
-    zm0[it] = st2[2 * ((N - k) & (N - 1))];
-    zm1[it] = st2[2 * (N - 1 - k) + 1];
-  }
-#pragma unroll
-  for (int it = 0; it < IT; ++it) {
-    const int w = tid + it * NT, p = w % G, k = w / G;
-    float2* o = out + (size_t)(2 * k) * a.Ny + r0 + 2 * p;
-    *reinterpret_cast<float4*>(o) = separate(make_float2(u[it].x, u[it].y), zm0[it]);
-    *reinterpret_cast<float4*>(o + a.Ny) = separate(make_float2(u[it].z, u[it].w), zm1[it]);
-  }
-  if (tid < G) {   // bin kx = N (k = N/2 of the even half): its own partner
-    const float2 z = reinterpret_cast<const float2*>(smem4 + (size_t)tid * GP)[2 * (N / 2)];
-    *reinterpret_cast<float4*>(out + (size_t)N * a.Ny + r0 + 2 * tid) = separate(z, z);
-  }
-}
-
 // ---------------------------------------------------------------------------------- K_C
 template <class P, int NT>
 __global__ void __launch_bounds__(NT, 512 / NT) k2_xinv(Fast2DArgs a, int dst_role) {
@@ -394,28 +324,44 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xinv_tma(Fast2DArgs a, int ds
   }
 }
 
-// ---------------------------------------------------------------------------------- K_A with TMA
-// Same computation as k2_xfwd; the separated spectra of the CTA's 2G rows leave as TMA boxes
-// {2G rows, KB bins}: the threads fill a ring of tiles in shared memory, one thread issues the tensor
-// stores, so the transposed 16G-byte pieces cost no LSU store wavefronts and the CTA does not wait
-// for them to drain.
-template <int G> struct K2StoreRing { static constexpr int NBUF = G >= 4 ? 3 : 4; };
+// ---------------------------------------------------------------------------------- K_A
+// x forward transform of FOUR rows per FFT group. Two real rows a, b form one complex line z = a + i b; the two
+// lanes of the packed engine carry two such lines (rows r, r+1 and r+2, r+3), and the even-bin and odd-bin
+// halves of the padded transform are two runs of the same group, one after the other:
+//     run E: FFT_N(z)          -> bins kx = 2k,     k = 0 .. N/2      (partner of bin 2k   is 2(N - k))
+//     run O: FFT_N(z w_2N^n)   -> bins kx = 2k + 1, k = 0 .. N/2 - 1  (partner of bin 2k+1 is 2(N-1-k) + 1)
+// After each run the spectra of a and b are separated (Hermitian symmetry) into tiles [bin][4G rows] and leave
+// TRANSPOSED, spec[c][kx][y], as TMA boxes {4G rows, KB bins} of a tensor map that walks every second column
+// (one map for the even, one for the odd columns): 32-byte pieces per group, written while the other run (or the
+// other CTA of the SM) computes. Compared with carrying the even/odd halves in the lanes (two rows per group) this
+// doubles the piece size at the same register count, needs no twiddle at all on the way in for run E and only
+// packed multiplies for run O. TMA = false: the same tiles are written with plain 32-byte stores.
 template <class P, int NT>
-constexpr size_t k2_tma_store_smem() {
-  return k2_smem<P, NT>() + (size_t)K2StoreRing<K2Shape<P, NT>::G>::NBUF * K2_KB * K2Shape<P, NT>::G * sizeof(float4) + 128;
+struct K2Fwd {
+  static constexpr int G = NT / P::T;
+  static constexpr int KB = (G >= 4 ? 512 / G : 256) < P::N / 2 ? (G >= 4 ? 512 / G : 256) : P::N / 2;   // bins per tile
+  static constexpr int NBUF = 3;                                                   // tiles in flight
+  static constexpr int TILE4 = KB * G * 2;                                         // float4 units per tile
+  static constexpr int NBE = (P::N / 2 + 1 + KB - 1) / KB, NBO = (P::N / 2 + KB - 1) / KB;
+  static constexpr int ROWS = 4 * G;
+};
+template <class P, int NT>
+constexpr size_t k2_fwd_smem() {
+  return k2_smem<P, NT>() + (size_t)K2Fwd<P, NT>::NBUF * K2Fwd<P, NT>::TILE4 * sizeof(float4) + 128;
 }
 
-template <class P, int NT, bool RAGGED>
-__global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd_tma(Fast2DArgs a, int src_role, const __grid_constant__ CUtensorMap map) {
+template <class P, int NT, bool RAGGED, bool TMA>
+__global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd4(Fast2DArgs a, int src_role, const __grid_constant__ CUtensorMap map_even,
+                                                         const __grid_constant__ CUtensorMap map_odd) {
   if (a.st->skip) return;
-  constexpr int N = P::N, T = P::T, E = P::E, G = NT / T, GP = K2Shape<P, NT>::GP;
-  constexpr int NB = (N + 1 + K2_KB - 1) / K2_KB, NBUF = K2StoreRing<G>::NBUF;
+  using F = K2Fwd<P, NT>;
+  constexpr int N = P::N, T = P::T, E = P::E, G = F::G, GP = K2Shape<P, NT>::GP, KB = F::KB, NBUF = F::NBUF;
   extern __shared__ __align__(128) float4 smem4[];
   __shared__ float bsat_s[MM_MAX_REGIONS];
   float4* tiles = smem4 + (size_t)G * GP + ((128 - ((size_t)G * GP * 16) % 128) % 128) / 16;   // 128-byte aligned
   const int tid = threadIdx.x, gid = tid / T, t = tid % T;
   float4* xb = smem4 + (size_t)gid * GP;
-  const int c = blockIdx.y, r0 = blockIdx.x * 2 * G;
+  const int c = blockIdx.y, r0 = blockIdx.x * F::ROWS;
   const float* __restrict__ src = a.st->ptr[src_role] + (size_t)c * a.ncell;
   const uint8_t* __restrict__ reg = a.regions;
   const bool uniform = a.luts->nregions == 1;       // one region: B_sat is a constant
@@ -429,52 +375,91 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd_tma(Fast2DArgs a, int sr
     int nb = (int)blockIdx.x + a.nsm * (512 / NT), nc = c;
     if (nb >= (int)gridDim.x) { nb -= gridDim.x; ++nc; }
     if (nc < 3 && nb < (int)gridDim.x) {
-      const float* nxt = a.st->ptr[src_role] + (size_t)nc * a.ncell + (size_t)nb * 2 * G * a.nxp;
-      for (int i = tid * 32; i < 2 * G * a.nxp; i += NT * 32) k2_prefetch_l2(nxt + i);
+      const float* nxt = a.st->ptr[src_role] + (size_t)nc * a.ncell + (size_t)nb * F::ROWS * a.nxp;
+      const long long lim = a.ncell - (long long)nb * F::ROWS * a.nxp;      // stay inside the component
+      for (int i = tid * 32; i < F::ROWS * a.nxp && i < lim; i += NT * 32) k2_prefetch_l2(nxt + i);
     }
   }
-  {
-    const size_t rowA = (size_t)(r0 + 2 * gid) * a.nxp;      // physical row pitch; n >= nxp is zero fill
-    rf::C2 v[E];
-    const float2 wt = __ldg(&a.twox[t]);      // w_2N^t; the other points follow from constants
-#pragma unroll
-    for (int e = 0; e < E; ++e) {
-      const int n = rf::slot_index<P, P::RA>(t, e);
-      float2 z = make_float2(0.f, 0.f);
-      if (!RAGGED || n < a.nxp) {
-        const size_t iA = rowA + n, iB = iA + a.nxp;
-        const float sa = uniform ? b0 : bsat_s[reg[iA]], sb = uniform ? b0 : bsat_s[reg[iB]];
-        z = make_float2(src[iA] * sa, src[iB] * sb);            // M = B_sat m (L121)
-      }
-      const float2 zw = rf::cmul_tw1<-1>(z, rf::half_twiddle(wt, e));
-      v[e] = {make_float2(z.x, zw.x), make_float2(z.y, zw.y)};
-    }
-    rf::fft<P, -1, NT>(v, xb, t, gid, a.twx);
-    rf::group_sync<T, NT>(gid);
-#pragma unroll
-    for (int e = 0; e < E; ++e) xb[rf::slot_index<P, P::RLAST>(t, e)] = stage_pack(v[e]);
-  }
-  __syncthreads();
-  // separate the two real rows of every pair (lane 0 of unit k = bin kx = 2k, lane 1 = bin 2k + 1)
-  // into tiles [bin][pair] and hand them to TMA; stored bins kx = 0 .. N (rows beyond are clipped)
+  const int row = r0 + 4 * gid;                       // first of the group's four rows
+  const float2 wt = __ldg(&a.twox[t]);                // w_2N^t; the other points follow from constants
+  int store_seq = 0;                                   // tiles handed to TMA so far (ring position)
 #pragma unroll 1
-  for (int j = 0; j < NB; ++j) {
-    float4* tile = tiles + (size_t)(j % NBUF) * K2_KB * G;
-    for (int i = tid; i < K2_KB * G; i += NT) {
-      const int p = i % G, kx = j * K2_KB + i / G;
-      if (kx > N) continue;
-      const float2* st2 = reinterpret_cast<const float2*>(smem4 + (size_t)p * GP);
-      const int k = kx >> 1, h = kx & 1;
-      const int km = h ? N - 1 - k : (N - k) & (N - 1);
-      tile[i] = separate(st2[2 * k + h], st2[2 * km + h]);
+  for (int run = 0; run < 2; ++run) {
+    {
+      rf::C2 v[E];
+#pragma unroll
+      for (int e = 0; e < E; ++e) {
+        const int n = rf::slot_index<P, P::RA>(t, e);
+        float z[4] = {0.f, 0.f, 0.f, 0.f};
+        if (!RAGGED || n < a.nxp) {
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            if (row + q < a.nyp) {                    // rows beyond the film: zero fill
+              const size_t i = (size_t)(row + q) * a.nxp + n;
+              z[q] = src[i] * (uniform ? b0 : bsat_s[reg[i]]);               // M = B_sat m (L121)
+            }
+          }
+        }
+        v[e] = {make_float2(z[0], z[2]), make_float2(z[1], z[3])};          // lanes: rows (r, r+1) and (r+2, r+3)
+      }
+      if (run == 1) {
+        // z w_2N^n, n = t + (N/16) e: first the constant part exp(-i pi e / 16), then w_2N^t for all sixteen
+        constexpr float C[16] = {1.f, 0.98078528040323043f, 0.92387953251128674f, 0.83146961230254524f, 0.70710678118654752f,
+                                 0.55557023301960218f, 0.38268343236508977f, 0.19509032201612825f, 0.f, -0.19509032201612825f,
+                                 -0.38268343236508977f, -0.55557023301960218f, -0.70710678118654752f, -0.83146961230254524f,
+                                 -0.92387953251128674f, -0.98078528040323043f};
+        constexpr float S[16] = {0.f, 0.19509032201612825f, 0.38268343236508977f, 0.55557023301960218f, 0.70710678118654752f,
+                                 0.83146961230254524f, 0.92387953251128674f, 0.98078528040323043f, 1.f, 0.98078528040323043f,
+                                 0.92387953251128674f, 0.83146961230254524f, 0.70710678118654752f, 0.55557023301960218f,
+                                 0.38268343236508977f, 0.19509032201612825f};
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+          if (e == 4) v[e] = rf::rot45<-1>(v[e]);
+          else if (e == 8) v[e] = rf::rot90<-1>(v[e]);
+          else if (e == 12) v[e] = rf::rot135<-1>(v[e]);
+          else if (e != 0) v[e] = rf::rotcs<-1>(v[e], C[e], S[e]);
+          v[e] = rf::cmul_tw<-1>(v[e], wt);
+        }
+      }
+      rf::fft<P, -1, NT>(v, xb, t, gid, a.twx);
+      rf::group_sync<T, NT>(gid);
+#pragma unroll
+      for (int e = 0; e < E; ++e) xb[rf::slot_index<P, P::RLAST>(t, e)] = stage_pack(v[e]);
     }
-    tma::fence_proxy_async();
-    if (tid == 0) tma::store_wait_read<NBUF - 2>();     // the tile of iteration j + 1 is free again
     __syncthreads();
-    if (tid == 0) {
-      tma::store_3d(&map, 2 * r0, j * K2_KB, c, tile);
-      tma::store_commit();
+    // separate the two real rows of each line: unit k of group p holds Z[k] of its two lines; tile[bin][p] =
+    // (A0, B0, A1, B1) = the 32 bytes of rows r .. r+3 at this bin
+    const int nbox = run == 0 ? F::NBE : F::NBO, nbin = run == 0 ? N / 2 + 1 : N / 2;
+#pragma unroll 1
+    for (int j = 0; j < nbox; ++j, ++store_seq) {
+      float4* tile = tiles + (size_t)(store_seq % NBUF) * F::TILE4;
+      for (int i = tid; i < KB * G; i += NT) {
+        const int p = i % G, k = j * KB + i / G;
+        if (k >= nbin) continue;
+        const float4* st = smem4 + (size_t)p * GP;
+        const int km = run == 0 ? ((N - k) & (N - 1)) : N - 1 - k;
+        const float4 u = st[k], um = st[km];
+        const float4 o0 = separate(make_float2(u.x, u.y), make_float2(um.x, um.y));
+        const float4 o1 = separate(make_float2(u.z, u.w), make_float2(um.z, um.w));
+        if (TMA) {
+          tile[2 * i] = o0; tile[2 * i + 1] = o1;
+        } else {
+          const int kx = 2 * k + run;
+          float4* o = reinterpret_cast<float4*>(a.spec + (size_t)c * a.cstride + (size_t)kx * a.Ny + r0 + 4 * p);
+          o[0] = o0; o[1] = o1;
+        }
+      }
+      if (TMA) {
+        tma::fence_proxy_async();
+        if (tid == 0) tma::store_wait_read<NBUF - 2>();     // the tile of the next iteration is free again
+        __syncthreads();
+        if (tid == 0) {
+          tma::store_3d(run == 0 ? &map_even : &map_odd, 2 * r0, j * KB, c, tile);
+          tma::store_commit();
+        }
+      }
     }
+    if (!TMA) __syncthreads();                              // xb is overwritten by the next run
   }
-  if (tid == 0) tma::store_wait_read<0>();               // shared memory must outlive the reads
+  if (TMA && tid == 0) tma::store_wait_read<0>();           // shared memory must outlive the reads
 }

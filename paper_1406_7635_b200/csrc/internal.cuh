@@ -40,7 +40,8 @@ struct mm_sim {
   ConvArgs conv;
   float* Kt = nullptr;         // kernel spectrum in the fast 2D layout
   Fast2DArgs f2;
-  CUtensorMap f2_map_inv, f2_map_fwd;   // TMA views of spec for the x kernels (boxes of 2G rows x 256 bins)
+  CUtensorMap f2_map_inv, f2_map_fwd, f2_map_fwd_odd;   // TMA views of spec for the x kernels (inverse: boxes of 2G rows x 256
+                                                        // bins; forward: 4G rows x KB bins of the even resp. odd columns)
   bool f2_no_tma = false;      // mm_set_option(MM_OPT_NO_TMA)
   bool f2_tma = false;         // tensor maps valid: the x kernels move their transposed pieces with TMA
   bool fast2d = false;         // fast 2D path available for this box

@@ -541,3 +541,98 @@ def test_zeeman_energy_is_minus_M_dot_B_times_volume():
         swing = max(swing, abs(sim.energy(terms=MM_ZEEMAN) - ez0))
         assert abs(sim.energy(terms=MM_ANIS | MM_ZEEMAN) - e0) < 1e-6 * abs(e0)
     assert swing > 0.5 * abs(e0)                         # energy really is traded between the two terms
+
+
+# ------------------------------------------------------------------ Dzyaloshinskii-Moriya exchange (Eq. 10-17)
+def _dmi_sim(grid, cell, pbc, D, A=16e-12, Ms=1100e3, Ku1=0.0, alpha=0.5):
+    sim = RefSim(grid, cell, pbc)
+    sim.set_params(Params.uniform(1, Msat=Ms, Aex=A, alpha=alpha, Ku1=Ku1, anisU=(0, 0, 1)))
+    sim.set_dmi(D)
+    sim.set_terms(MM_EXCH | MM_ANIS)                       # no demag: closed forms below
+    return sim
+
+
+def test_dmi_energy_density_eq16_equals_eq17_and_field_is_minus_dE_dM():
+    # periodic box (no boundary terms): (i) -1/2 M . B_DM (Eq. 17) equals D [m_z div m - (m . grad) m_z] (Eq. 16)
+    # cell by cell when both use the central differences of L246; (ii) the total exchange + DM field is
+    # -dE/dM of the summed energy (finite differences on single cells)
+    D, A, Ms = 1.3e-3, 16e-12, 1100e3
+    cell = (2e-9, 3e-9, 1e-9)
+    sim = _dmi_sim((8, 6, 1), cell, (1, 1, 0), D, A, Ms)
+    m = _rand_m(71, sim.shape)
+    sim.set_m(m)
+    Bdm = sim.b_exch(sim.m) - fld.b_exchange(sim.m, sim.regions, sim.L, sim.cell, sim.pbc)
+    dx = lambda f: (np.roll(f, -1, axis=2) - np.roll(f, 1, axis=2)) / (2 * cell[0])
+    dy = lambda f: (np.roll(f, -1, axis=1) - np.roll(f, 1, axis=1)) / (2 * cell[1])
+    mx, my, mz = sim.m
+    eq16 = D * (mz * (dx(mx) + dy(my)) - (mx * dx(mz) + my * dy(mz)))
+    eq17 = -0.5 * Ms * (sim.m * Bdm).sum(axis=0)
+    assert np.allclose(eq16, eq17, rtol=1e-12, atol=1e-9 * np.abs(eq16).max())
+    V = cell[0] * cell[1] * cell[2]
+    B = sim.b_exch(sim.m)
+    h = 1e-6
+    for (c, iy, ix) in ((0, 2, 3), (1, 0, 7), (2, 5, 0)):
+        mp = sim.m.copy(); mp[c, 0, iy, ix] += h
+        mn = sim.m.copy(); mn[c, 0, iy, ix] -= h
+        dE = (sim.energy(mp, MM_EXCH) - sim.energy(mn, MM_EXCH)) / (2 * h)
+        assert np.isclose(B[c, 0, iy, ix], -dE / (Ms * V), rtol=1e-6)
+
+
+def test_dmi_cycloid_energy_and_chirality():
+    # Neel cycloid m = (s sin kx, 0, cos kx) on a periodic chain: Eq. 16 gives the energy density s D k' with
+    # k' = sin(k dx)/dx the central-difference wave number; D > 0 favours s = -1 (m turns from +z towards -x)
+    n, dx_, D, A, Ms = 64, 1e-9, 2e-3, 16e-12, 1100e3
+    sim = _dmi_sim((n, 1, 1), (dx_, dx_, dx_), (1, 0, 0), D, A, Ms)
+    k = 2 * np.pi * 3 / (n * dx_)
+    x = np.arange(n) * dx_
+    for s_ in (+1, -1):
+        m = np.zeros((3, 1, 1, n)); m[0, 0, 0] = s_ * np.sin(k * x); m[2, 0, 0] = np.cos(k * x)
+        sim.set_m(m)
+        e_ex = (2 * A / dx_ ** 2) * (1 - np.cos(k * dx_))                       # Eq. 6 + 8 (spiral identity)
+        want = (e_ex + s_ * D * np.sin(k * dx_) / dx_) * n * dx_ ** 3
+        assert np.isclose(sim.energy(terms=MM_EXCH), want, rtol=1e-12)
+
+
+def test_dmi_boundary_conditions_tilt_the_edge_magnetisation():
+    # Eq. 11-13 with the exchange field under the same boundary conditions (L248): for m = (sin th, 0, cos th)
+    # the energy density is A th'^2 + K sin^2 th + D th', so th'' = sin th cos th / xi^2 (xi^2 = A/K), first
+    # integral th' = -sin th / xi, and the boundary condition th' = -D/2A fixes the edge tilt
+    #     sin th_edge = D / (2 sqrt(A K)),   tan(th/2) = tan(th_edge/2) exp(-x/xi)  from the left edge,
+    # with the opposite sign of m_x at the right edge. A chain of 0.25 nm cells, xi = 5.66 nm, relaxed.
+    n, dx_, D, A, K, Ms = 240, 0.25e-9, 1e-3, 16e-12, 0.5e6, 1100e3
+    sim = _dmi_sim((n, 1, 1), (dx_, 1e-9, 1e-9), (0, 0, 0), D, A, Ms, Ku1=K)
+    m = np.zeros((3, 1, 1, n)); m[2] = 1.0
+    sim.set_m(m)
+    sim.relax()
+    assert sim.max_torque() < 1e-5
+    xi = np.sqrt(A / K)
+    th_e = np.arcsin(D / (2 * np.sqrt(A * K)))
+    x = (np.arange(n) + 0.5) * dx_                                             # cell centres from the left edge
+    th = 2 * np.arctan(np.tan(th_e / 2) * np.exp(-x / xi))
+    mx = sim.m[0, 0, 0]
+    assert abs(np.sin(th_e) - 0.17678) < 1e-5
+    assert np.abs(mx[:n // 2] - np.sin(th[:n // 2])).max() < 0.01 * np.sin(th_e)
+    assert np.abs(mx[::-1][:n // 2] + np.sin(th[:n // 2])).max() < 0.01 * np.sin(th_e)
+    assert np.abs(sim.m[1]).max() < 1e-9
+
+
+def test_dmi_off_reduces_to_plain_exchange_and_vacuum_is_a_boundary():
+    # D = 0: the boundary conditions vanish and Eq. 6 is recovered exactly; a vacuum neighbour (Msat = 0) is a
+    # missing neighbour (geometry, L53): the cell next to it sees the same virtual neighbour as at the box edge
+    rng = np.random.default_rng(3)
+    sim = RefSim((7, 5, 2), (2e-9, 3e-9, 1e-9))
+    p = Params.uniform(2, Msat=np.array([1100e3, 0.0]), Aex=16e-12, alpha=0.5)
+    sim.set_params(p)
+    reg = np.zeros(sim.shape, dtype=np.int64); reg[:, :, 5:] = 1              # columns x >= 5 are empty
+    sim.set_regions(reg)
+    sim.set_m(_rand_m(5, sim.shape))
+    B0 = fld.b_exchange(sim.m, sim.regions, sim.L, sim.cell, sim.pbc)
+    Bz = fld.b_exchange_dmi(sim.m, sim.regions, sim.L, sim.cell, sim.pbc, p.Msat, p.Aex, np.zeros(2))
+    assert np.allclose(Bz, B0, rtol=0, atol=1e-12 * np.abs(B0).max())
+    # the same film cut out of a 5-column box: identical field in the magnetic cells when D != 0
+    sim.set_dmi(1.5e-3)
+    small = RefSim((5, 5, 2), (2e-9, 3e-9, 1e-9))
+    small.set_params(Params.uniform(1, Msat=1100e3, Aex=16e-12, alpha=0.5))
+    small.set_m(sim.m[:, :, :, :5]); small.set_dmi(1.5e-3)
+    assert np.allclose(sim.b_exch(sim.m)[:, :, :, :5], small.b_exch(small.m), rtol=1e-13)
+    assert np.abs(sim.b_exch(sim.m)[:, :, :, 5:]).max() == 0.0
