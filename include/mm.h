@@ -154,6 +154,15 @@ int mm_set_slonczewski(mm_sim* sim, double jz, double pol, double lambda, double
  * torque is evaluated (a later mm_set_params takes effect). j = 0 switches the term off. */
 int mm_set_zhang_li(mm_sim* sim, const double j[3], double xi);
 
+/* Interfacial Dzyaloshinskii-Moriya exchange (Eq. 10-17), part of the exchange term MM_EXCH (the paper's
+ * E_exch(DM)):  B_DM = (2D/Msat) (dm_z/dx, dm_z/dy, -dm_x/dx - dm_y/dy), central differences (L246), with the boundary
+ * conditions of Eq. 11-15: a missing neighbour (outside an open box, or a cell with Msat = 0) is replaced by
+ * m + (dm/di)|_dV Delta_i n, dm_z/dx = (D/2A) m_x, dm_x/dx = dm_y/dy = -(D/2A) m_z, dm_z/dy = (D/2A) m_y, others 0;
+ * with D != 0 the same virtual neighbours enter the Heisenberg exchange field (L248). D [J/m^2]: n = 1 value for
+ * the whole box or n = nregions values (host pointer); D and D/2A are those of the cell's own region (DESIGN.md
+ * #20). All zeros (or n = 0) switch the term off. Needs mm_set_params first; energies include Eq. 17. */
+int mm_set_dmi(mm_sim* sim, const double* D, int n);
+
 /* Precession term of Eq. 2 on (default) or off: off leaves tau = -gamma alpha/(1+alpha^2) m x (m x B),
  * "so that the effective field points towards decreasing energy" (relax(), L388). */
 int mm_set_precession(mm_sim* sim, int on);

@@ -70,6 +70,7 @@ _SIGNATURES = {
     "mm_torque": (C.c_int, [C.c_void_p, C.c_void_p]),
     "mm_set_solver_kind": (C.c_int, [C.c_void_p, C.c_int]),
     "mm_set_precession": (C.c_int, [C.c_void_p, C.c_int]),
+    "mm_set_dmi": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.c_int]),
     "mm_set_zhang_li": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.c_double]),
     "mm_set_slonczewski": (C.c_int, [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_double, C.POINTER(C.c_double)]),
     "mm_set_temperature": (C.c_int, [C.c_void_p, C.c_double, C.c_ulonglong]),
@@ -243,6 +244,12 @@ class Sim:
     def set_zhang_li(self, j, xi):
         v = (C.c_double * 3)(*[float(x) for x in j])
         _check(lib().mm_set_zhang_li(self._h, v, float(xi)), self._h)
+
+    def set_dmi(self, D):
+        """Dzyaloshinskii-Moriya strength [J/m^2]: a scalar or one value per region."""
+        d = np.atleast_1d(np.asarray(D, dtype=np.float64))
+        v = (C.c_double * len(d))(*d.tolist())
+        _check(lib().mm_set_dmi(self._h, v, len(d)), self._h)
 
     def set_precession(self, on):
         _check(lib().mm_set_precession(self._h, 1 if on else 0), self._h)

@@ -6,6 +6,7 @@
 #include "../../include/mm.h"
 
 #define MM_THERMAL 16u   /* internal term bit: thermal field of the current step (never part of MM_ALL) */
+#define MM_DMI_ON 32u    /* internal term bit: a Dzyaloshinskii-Moriya strength is set (exchange part takes the boundary-condition path) */
 #define MM_TRI_ENTRIES (MM_MAX_REGIONS * (MM_MAX_REGIONS + 1) / 2)
 
 // ---- buffer roles: every kernel fetches its array pointers from DevState::ptr[role], so that the
@@ -55,6 +56,8 @@ struct Luts {
   float bext[4];
   int nregions;
   int has_uniaxial, has_cubic;
+  float dmi[MM_MAX_REGIONS];    // 2 D / Msat [T m]            (Eq. 10)
+  float dmi_bc[MM_MAX_REGIONS]; // D / (2 Aex) [1/m]: boundary derivative of Eq. 11-13
   float exch[MM_TRI_ENTRIES];   // 2 * L[i,j] [T m^2], lower triangular i(i+1)/2 + j, i >= j (Eq. 9)
 };
 
@@ -75,6 +78,7 @@ struct Geometry {
   int Hy, Hz;    // Py/2 + 1, Pz/2 + 1: extent of the symmetric kernel spectrum
   int pbc[3];
   float inv_dx2, inv_dy2, inv_dz2;
+  float dx, dy;  // cell edges [m] (central differences and boundary conditions of the DM term)
   long long N;   // cells
 };
 

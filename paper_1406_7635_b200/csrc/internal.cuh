@@ -60,6 +60,9 @@ struct mm_sim {
   bool zl_on = false;          // Zhang-Li torque enabled (mm_set_zhang_li)
   double zl_j[3] = {};         // current density [A/m^2] and non-adiabaticity as passed; the kernel arguments are
   double zl_xi = 0.0;          // formed at launch time from the gamma_LL in force (mm_set_params may change it)
+  bool dmi_on = false;         // a Dzyaloshinskii-Moriya strength is set (mm_set_dmi): exchange takes the boundary-condition path
+  int dmi_n = 0;               // entries of hD in use: 0 (off), 1 (uniform) or nregions
+  double hD[MM_MAX_REGIONS] = {}, hMsat[MM_MAX_REGIONS] = {}, hAex[MM_MAX_REGIONS] = {};   // host copies for the DM tables
   bool stt_on = false;         // Slonczewski torque enabled (mm_set_slonczewski)
   float stt[7] = {};           // pref, pol, lam2, eps_prime, mp[3]  (SttArgs of local_rk.cuh)
   int nregions = 1;

@@ -26,6 +26,57 @@ __device__ __forceinline__ float mm_eta(unsigned long long seed, int comp, unsig
   return (float)(sqrt(-2.0 * log(1.0 - u1)) * cospi(2.0 * u2));
 }
 
+// Heisenberg + Dzyaloshinskii-Moriya exchange field of ONE cell with the boundary conditions of Eq. 11-15
+// (PAPER.md L215-L257): B_DM = (2D/Msat)(dm_z/dx, dm_z/dy, -dm_x/dx - dm_y/dy) by central differences (L246);
+// a missing neighbour - outside an open box or a vacuum cell (Msat = 0) - is the virtual
+// m + (dm/di)|_dV Delta_i n, and with D != 0 the same virtual neighbour enters Eq. 6 (L248).
+// Adds to (bx, by, bz). Used by the local kernels and the energy kernel when a DM strength is set.
+__device__ __forceinline__ void exch_dmi_cell(const Geometry& g, const uint8_t* __restrict__ regions, const Luts* __restrict__ lut,
+                                              const float* __restrict__ m, long long i, int x, int y, int z, int r, float mx,
+                                              float my, float mz, float& bx, float& by, float& bz) {
+  const long long N = g.N;
+  const float bc = lut->dmi_bc[r], cD = lut->dmi[r], own = __ldg(&lut->exch[tri_index(r, r)]);
+  float ex = 0.f, ey = 0.f, ez = 0.f;
+  // neighbour at sign = +-1 along axis (0 = x, 1 = y, 2 = z): (nx, ny, nz) and its exchange contribution
+  auto nbr = [&](bool inside, long long j, int axis, float sgn, float d, float w, float& nx, float& ny, float& nz) {
+    const int rj = inside ? (int)regions[j] : r;
+    if (inside && lut->live[rj] > 0.f) {
+      nx = m[j]; ny = m[N + j]; nz = m[2 * N + j];
+      w *= __ldg(&lut->exch[tri_index(r, rj)]);
+    } else {
+      const float s = sgn * d * bc;
+      nx = mx; ny = my; nz = mz;
+      if (axis == 0) { nx = mx - s * mz; nz = mz + s * mx; }
+      else if (axis == 1) { ny = my - s * mz; nz = mz + s * my; }
+      w *= own;
+    }
+    ex += w * (nx - mx); ey += w * (ny - my); ez += w * (nz - mz);
+  };
+  float px, py, pz, qx, qy, qz;
+  if (g.Nx > 1) {
+    const bool up = x + 1 < g.Nx || g.pbc[0], dn = x > 0 || g.pbc[0];
+    nbr(up, x + 1 < g.Nx ? i + 1 : i + 1 - g.Nx, 0, 1.f, g.dx, g.inv_dx2, px, py, pz);
+    nbr(dn, x > 0 ? i - 1 : i - 1 + g.Nx, 0, -1.f, g.dx, g.inv_dx2, qx, qy, qz);
+    const float h = cD / (2.f * g.dx);
+    bx += h * (pz - qz); bz -= h * (px - qx);
+  }
+  if (g.Ny > 1) {
+    const long long s = g.Nx;
+    const bool up = y + 1 < g.Ny || g.pbc[1], dn = y > 0 || g.pbc[1];
+    nbr(up, y + 1 < g.Ny ? i + s : i + s - s * g.Ny, 1, 1.f, g.dy, g.inv_dy2, px, py, pz);
+    nbr(dn, y > 0 ? i - s : i - s + s * g.Ny, 1, -1.f, g.dy, g.inv_dy2, qx, qy, qz);
+    const float h = cD / (2.f * g.dy);
+    by += h * (pz - qz); bz -= h * (py - qy);
+  }
+  if (g.Nz > 1) {
+    const long long s = (long long)g.Nx * g.Ny;
+    const bool up = z + 1 < g.Nz || g.pbc[2], dn = z > 0 || g.pbc[2];
+    nbr(up, z + 1 < g.Nz ? i + s : i + s - s * g.Nz, 2, 1.f, 0.f, g.inv_dz2, px, py, pz);
+    nbr(dn, z > 0 ? i - s : i - s + s * g.Nz, 2, -1.f, 0.f, g.inv_dz2, qx, qy, qz);
+  }
+  bx += ex; by += ey; bz += ez;
+}
+
 // B_eff = [B_demag] + B_exch (Eq. 6 / Eq. 9) + B_anis (Eq. 18, 21) + B_ext, then either stored as the
 // field (out_torque = 0) or turned into the torque over gamma (Eq. 2, sign reading DESIGN.md #5).
 // One thread per cell; x fastest so every global access of a warp is one contiguous segment.
@@ -45,7 +96,9 @@ __global__ void k_local(Geometry g, const uint8_t* __restrict__ regions, const L
   const float mx = m[i], my = m[N + i], mz = m[2 * N + i];
   float bx = 0.f, by = 0.f, bz = 0.f;
   if (mask & MM_DEMAG) { bx = bd[i]; by = bd[N + i]; bz = bd[2 * N + i]; }
-  if (mask & MM_EXCH) {
+  if ((mask & MM_EXCH) && (mask & MM_DMI_ON)) {
+    if (lut->live[r] > 0.f) exch_dmi_cell(g, regions, lut, m, i, x, y, z, r, mx, my, mz, bx, by, bz);
+  } else if (mask & MM_EXCH) {
     float ex = 0.f, ey = 0.f, ez = 0.f;
     auto nb = [&](long long j, float w) {
       float a = w * __ldg(&lut->exch[tri_index(r, regions[j])]);
@@ -119,7 +172,9 @@ struct ErrCoef { float e[7]; };            // b(high) - b(low) of the embedded p
 //          stencil is reading. Saves re-reading k_i and one launch per stage.
 // FUSE = 2: last stage of a step: the error norm max || sum_j e_j k_j || (L372) is reduced here.
 // grid = (Nx/4 / blockDim.x, Ny, Nz)
-template <bool UNIFORM, bool THERMAL, int FUSE>
+// DMI = a Dzyaloshinskii-Moriya strength is set: the exchange part runs cell by cell through exch_dmi_cell
+//       (boundary conditions, virtual neighbours); instantiated apart, the hot path does not pay for it.
+template <bool UNIFORM, bool THERMAL, int FUSE, bool DMI = false>
 __global__ void __launch_bounds__(128) k_local4(Geometry g, const uint8_t* __restrict__ regions, const Luts* __restrict__ lut,
                                                 DevState* st, int m_role, int bd_role, int dst_role, unsigned mask,
                                                 int out_torque, StageCoef sc, ErrCoef ec, int ynext_role) {
@@ -150,7 +205,14 @@ __global__ void __launch_bounds__(128) k_local4(Geometry g, const uint8_t* __res
     const uchar4 q = *reinterpret_cast<const uchar4*>(regions + i);
     r[0] = q.x; r[1] = q.y; r[2] = q.z; r[3] = q.w;
   }
-  if (mask & MM_EXCH) {
+  if (DMI && (mask & MM_EXCH)) {
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      const int rl = UNIFORM ? 0 : r[l];
+      if (lut->live[rl] > 0.f)
+        exch_dmi_cell(g, regions, lut, m, i + l, x + l, y, z, rl, mc[0][l], mc[1][l], mc[2][l], b[0][l], b[1][l], b[2][l]);
+    }
+  } else if (mask & MM_EXCH) {
     const float a0 = lut->exch[0];
     // a whole neighbour row segment (y or z direction): j = index of its first cell
     auto nb_row = [&](long long j, float w) {
@@ -481,7 +543,11 @@ __global__ void k_energy(Geometry g, const uint8_t* __restrict__ regions, const 
     const float mx = m[i], my = m[N + i], mz = m[2 * N + i];
     float e = 0.f;                                      // sum of weight * m . B  [T]
     if (mask & MM_DEMAG) e += 0.5f * (mx * bd[i] + my * bd[N + i] + mz * bd[2 * N + i]);
-    if (mask & MM_EXCH) {
+    if ((mask & MM_EXCH) && (mask & MM_DMI_ON)) {       // Eq. 8 + Eq. 17: -1/2 M . (B_exch + B_DM)
+      float ex = 0.f, ey = 0.f, ez = 0.f;
+      if (lut->live[r] > 0.f) exch_dmi_cell(g, regions, lut, m, i, x, y, z, r, mx, my, mz, ex, ey, ez);
+      e += 0.5f * (mx * ex + my * ey + mz * ez);
+    } else if (mask & MM_EXCH) {
       float ex = 0.f, ey = 0.f, ez = 0.f;
       auto nb = [&](long long j, float w) {
         float a = w * __ldg(&lut->exch[tri_index(r, regions[j])]);

@@ -3,6 +3,7 @@
 // the host and there is no CPU fallback.
 #include <algorithm>
 #include <cmath>
+#include <cstddef>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -210,16 +211,20 @@ void launch_local(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_
   ErrCoef ec = {};
   if (scp) sc = *scp;
   if (ecp) ec = *ecp;
+  if (s->dmi_on) mask |= MM_DMI_ON;
   if (local4_ok(s)) {
     const int q = g.Nx / 4, bt = q >= 128 ? 128 : (q >= 64 ? 64 : 32);
     const dim3 grid((q + bt - 1) / bt, g.Ny, g.Nz);
     const bool th = (mask & MM_THERMAL) != 0;
-#define MM_LOCAL4(U, T, F) k_local4<U, T, F><<<grid, bt, 0, s->stream>>>(g, s->regions, s->luts, s->dstate, src_role, R_B, dst_role, mask, out_torque, sc, ec, ynext)
-    if (s->nregions == 1) {
-      if (th) MM_LOCAL4(true, true, 0); else if (fuse == 1) MM_LOCAL4(true, false, 1); else if (fuse == 2) MM_LOCAL4(true, false, 2); else MM_LOCAL4(true, false, 0);
-    } else {
-      if (th) MM_LOCAL4(false, true, 0); else if (fuse == 1) MM_LOCAL4(false, false, 1); else if (fuse == 2) MM_LOCAL4(false, false, 2); else MM_LOCAL4(false, false, 0);
-    }
+#define MM_LOCAL4(U, T, F, D) k_local4<U, T, F, D><<<grid, bt, 0, s->stream>>>(g, s->regions, s->luts, s->dstate, src_role, R_B, dst_role, mask, out_torque, sc, ec, ynext)
+#define MM_LOCAL4_PICK(U, D)                                                                                            \
+    do {                                                                                                                \
+      if (th) MM_LOCAL4(U, true, 0, D); else if (fuse == 1) MM_LOCAL4(U, false, 1, D);                                   \
+      else if (fuse == 2) MM_LOCAL4(U, false, 2, D); else MM_LOCAL4(U, false, 0, D);                                    \
+    } while (0)
+    if (s->nregions == 1) { if (s->dmi_on) MM_LOCAL4_PICK(true, true); else MM_LOCAL4_PICK(true, false); }
+    else { if (s->dmi_on) MM_LOCAL4_PICK(false, true); else MM_LOCAL4_PICK(false, false); }
+#undef MM_LOCAL4_PICK
 #undef MM_LOCAL4
     return;
   }
@@ -437,6 +442,7 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
     g.Py = 2 * mm_fast2d_length(Ny);
   }
   g.pbc[0] = pbc_x > 0; g.pbc[1] = pbc_y > 0; g.pbc[2] = pbc_z > 0;
+  g.dx = (float)dx; g.dy = (float)dy;
   g.inv_dx2 = (float)(1.0 / (dx * dx)); g.inv_dy2 = (float)(1.0 / (dy * dy)); g.inv_dz2 = (float)(1.0 / (dz * dz));
   auto bail = [&](int code, const char* msg) {
     g_create_error = msg;
@@ -537,6 +543,7 @@ int mm_set_params(mm_sim* s, const mm_params* p) {
   if (!s || !p) return mm_fail(s, MM_EINVAL, "null argument");
   const int n = p->nregions;
   if (n < 1 || n > MM_MAX_REGIONS) return mm_fail(s, MM_EINVAL, "nregions out of range");
+  if (s->dmi_n > 1 && s->dmi_n != n) return mm_fail(s, MM_EINVAL, "the DM table of mm_set_dmi has another number of regions");
   for (int r = 0; r < n; ++r) {
     if (!(p->Msat[r] >= 0) || !(p->Aex[r] >= 0) || !std::isfinite(p->Msat[r]) || !std::isfinite(p->Aex[r]) ||
         !std::isfinite(p->alpha[r]) || !std::isfinite(p->Ku1[r]) || !std::isfinite(p->Ku2[r]) ||
@@ -563,6 +570,12 @@ int mm_set_params(mm_sim* s, const mm_params* p) {
     const double Ms = p->Msat[r], iMs = Ms > 0 ? 1.0 / Ms : 0.0;
     q[r] = Ms > 0 ? p->Aex[r] / Ms : 0.0;
     L->Bsat[r] = (float)(mu0 * Ms);
+    s->hMsat[r] = Ms; s->hAex[r] = p->Aex[r];
+    {   // Dzyaloshinskii-Moriya tables (Eq. 10, Eq. 11-13), from the strength last given to mm_set_dmi
+      const double D = s->dmi_n == 0 ? 0.0 : s->hD[s->dmi_n == 1 ? 0 : r];
+      L->dmi[r] = Ms > 0 ? (float)(2.0 * D / Ms) : 0.f;
+      L->dmi_bc[r] = (Ms > 0 && p->Aex[r] > 0) ? (float)(D / (2.0 * p->Aex[r])) : 0.f;
+    }
     L->alpha[r] = (float)p->alpha[r];
     L->live[r] = Ms > 0 ? 1.f : 0.f;
     {   // Eq. 24 without T and dt: sqrt(2 mu0 alpha kB / (Bsat gamma dV))
@@ -662,6 +675,32 @@ int mm_set_zhang_li(mm_sim* s, const double j[3], double xi) {
   for (int a = 0; a < 3; ++a) s->zl_j[a] = j[a];
   s->zl_xi = xi;
   s->zl_on = true;
+  return MM_OK;
+}
+
+int mm_set_dmi(mm_sim* s, const double* D, int n) {
+  if (!s) return MM_EINVAL;
+  if (!s->have_params) return mm_fail(s, MM_ESTATE, "mm_set_params must precede mm_set_dmi");
+  if (n < 0 || (n > 1 && n != s->nregions) || (n > 0 && !D)) return mm_fail(s, MM_EINVAL, "DM table: one value or one per region");
+  bool any = false;
+  for (int r = 0; r < n; ++r) {
+    if (!std::isfinite(D[r])) return mm_fail(s, MM_EINVAL, "non-finite DM strength");
+    s->hD[r] = D[r];
+    any = any || D[r] != 0.0;
+  }
+  s->dmi_n = any ? n : 0;
+  s->dmi_on = any;
+  std::vector<float> c(MM_MAX_REGIONS, 0.f), bc(MM_MAX_REGIONS, 0.f);
+  for (int r = 0; r < s->nregions && any; ++r) {
+    const double Dr = s->hD[n == 1 ? 0 : r], Ms = s->hMsat[r], A = s->hAex[r];
+    c[r] = Ms > 0 ? (float)(2.0 * Dr / Ms) : 0.f;
+    bc[r] = (Ms > 0 && A > 0) ? (float)(Dr / (2.0 * A)) : 0.f;
+  }
+  char* base = reinterpret_cast<char*>(s->luts);
+  CUDA_TRY(s, cudaMemcpyAsync(base + offsetof(Luts, dmi), c.data(), sizeof(float) * MM_MAX_REGIONS, cudaMemcpyHostToDevice, s->stream));
+  CUDA_TRY(s, cudaMemcpyAsync(base + offsetof(Luts, dmi_bc), bc.data(), sizeof(float) * MM_MAX_REGIONS, cudaMemcpyHostToDevice, s->stream));
+  CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+  s->have_k1 = false; s->graph_dirty = true;
   return MM_OK;
 }
 
@@ -842,7 +881,7 @@ int mm_energy(mm_sim* s, unsigned mask, double* joules) {
   clear_skip(s);
   if (mask & MM_DEMAG) launch_demag(s, R_M);
   CUDA_TRY(s, cudaMemsetAsync(s->scratch3, 0, 3 * sizeof(double), s->stream));
-  { Launch l(s, KK_OTHER); k_energy<<<s->nsm * 8, 256, 0, s->stream>>>(s->g, s->regions, s->luts, s->dstate, R_M, R_B, mask, s->scratch3); }
+  { Launch l(s, KK_OTHER); k_energy<<<s->nsm * 8, 256, 0, s->stream>>>(s->g, s->regions, s->luts, s->dstate, R_M, R_B, mask | (s->dmi_on ? MM_DMI_ON : 0u), s->scratch3); }
   CUDA_TRY(s, cudaGetLastError());
   double e = 0.0;
   if ((rc = copy_out(s, &e, s->scratch3, sizeof(double)))) return rc;

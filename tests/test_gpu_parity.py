@@ -814,3 +814,79 @@ def test_zhang_li_torque_and_advection(mm):
     sim.run(t)
     m = sim.get_m()
     assert np.abs(m[0, 0, 0] - np.cos(k * x - w * t)).max() < 2e-5 and np.abs(m[2]).max() < 1e-5
+
+
+# --------------------------------------------------------------------------- Dzyaloshinskii-Moriya exchange
+def test_dmi_field_energy_and_trajectory(mm):
+    # Eq. 10-17 (L215-L257): exchange + DM field with the boundary conditions on open edges, periodic axes and next
+    # to vacuum cells; per-region D; energies (Eq. 8 + Eq. 17); a short trajectory
+    for grid, cell, pbc, nreg in (((48, 20, 1), (2e-9, 3e-9, 1e-9), (0, 0, 0), 3), ((16, 12, 4), (2e-9, 2e-9, 1e-9), (2, 0, 0), 2),
+                                  ((30, 9, 2), (1e-9, 2e-9, 1e-9), (0, 0, 0), 3)):      # Nx % 4 != 0: one cell per thread
+        cfg = _rand_cfg(grid, cell, pbc=pbc, nreg=nreg, anis=True, seed=29)
+        if nreg == 3:
+            cfg["params"].Msat[2] = 0.0                      # region 2 is vacuum: its neighbours see a boundary
+        D = np.array([1.2e-3, -0.7e-3, 0.9e-3])[:nreg]
+        sim = mm.from_config(cfg)
+        ref = _ref_from(cfg, "fft")
+        sim.set_dmi(D); ref.set_dmi(D)
+        _field_check(sim, ref, (MM_EXCH, MM_ALL))
+        B1 = sim.b_eff(MM_EXCH).copy()
+        sim.set_dmi(0.0)
+        assert np.abs(sim.b_eff(MM_EXCH) - B1).max() > 1e-3 * np.abs(B1).max()       # the term was really there
+        sim.set_dmi(D)
+        scale = abs(ref.energy(terms=MM_EXCH)) + abs(ref.energy(terms=MM_DEMAG))
+        assert abs(sim.energy(MM_EXCH) - ref.energy(terms=MM_EXCH)) <= 2e-6 * scale
+        assert abs(sim.energy(MM_ALL) - ref.energy(terms=MM_ALL)) <= 4e-6 * scale
+        tq = sim.torque().astype(np.float64)
+        tr = ref.torque(ref.m) / ref.p.gamma_LL
+        assert np.abs(tq - tr).max() <= FIELD_TOL * np.abs(tr).max()
+        sim.set_solver(fix_dt=2e-14); ref.set_solver(fix_dt=2e-14)
+        sim.steps(25)
+        for _ in range(25):
+            ref.step()
+        assert np.abs(sim.get_m() - ref.m).max() < 5e-5
+
+
+def test_dmi_edge_tilt_closed_form(mm):
+    # the closed form the oracle is pinned with (boundary conditions Eq. 11-13): sin(theta_edge) = D / (2 sqrt(A K))
+    n, dx_, D, A, K, Ms = 240, 0.25e-9, 1e-3, 16e-12, 0.5e6, 1100e3
+    p = Params.uniform(1, Msat=Ms, Aex=A, alpha=0.5, Ku1=K, anisU=(0, 0, 1))
+    m0 = np.zeros((3, 1, 4, n), dtype=np.float32); m0[2] = 1.0
+    sim = mm.from_config(dict(grid=(n, 4, 1), cell=(dx_, 1e-9, 1e-9), pbc=(0, 1, 0), regions=None, params=p, m0=m0))
+    sim.set_terms(MM_EXCH | MM_ANIS)
+    sim.set_dmi(D)
+    sim.relax()
+    xi, th_e = np.sqrt(A / K), np.arcsin(D / (2 * np.sqrt(A * K)))
+    x = (np.arange(n) + 0.5) * dx_
+    th = 2 * np.arctan(np.tan(th_e / 2) * np.exp(-x / xi))
+    mx = sim.get_m()[0, 0, 1].astype(np.float64)
+    assert np.abs(mx[:n // 2] - np.sin(th[:n // 2])).max() < 0.01 * np.sin(th_e)
+    assert np.abs(mx[::-1][:n // 2] + np.sin(th[:n // 2])).max() < 0.01 * np.sin(th_e)
+
+
+def test_fig6_dmi_turns_a_bloch_wall_into_a_neel_wall(mm):
+    # The paper's DMI verification (Fig. 6, script L726-L745): 250 nm wide, 0.6 nm thick Co/Pt film, Msat 1100e3,
+    # Aex 16e-12, Ku1 1.27e6 along z, a down-up domain pair; relax at growing D. At D = 0 magnetostatics favour the
+    # Bloch wall (moment along the wall, y); the DM term favours the Neel wall (moment across it, x) and wins
+    # beyond a threshold of the order of 0.1 mJ/m^2 (the figure's x axis ends at 0.3 mJ/m^2, L743).
+    n = 128
+    c = 250e-9 / n
+    p = Params.uniform(1, Msat=1100e3, Aex=16e-12, alpha=3.0, Ku1=1.27e6, anisU=(0, 0, 1))
+    m0 = np.zeros((3, 1, n, n), dtype=np.float32)
+    m0[2, :, :, :n // 2] = -1.0; m0[2, :, :, n // 2:] = 1.0
+    m0[0, :, :, n // 2 - 1:n // 2 + 1] = 1.0; m0[1, :, :, n // 2 - 1:n // 2 + 1] = 1.0      # wall between Bloch and Neel
+    m0[2, :, :, n // 2 - 1:n // 2 + 1] = 0.0
+    sim = mm.from_config(dict(grid=(n, n, 1), cell=(c, c, 0.6e-9), pbc=(0, 0, 0), regions=None, params=p, m0=m0))
+    wall = []
+    for D in (0.0, 0.05e-3, 0.10e-3, 0.20e-3, 0.30e-3):
+        sim.set_dmi(D)
+        sim.relax()
+        m = sim.get_m()[:, 0, n // 4:3 * n // 4, :]          # away from the film's y edges
+        w = np.abs(m[2]) < 0.5                                # the wall cells
+        wall.append((float(m[0][w].mean()), float(m[1][w].mean())))
+    (x0, y0), (x4, y4) = wall[0], wall[-1]
+    assert abs(y0) > 0.8 and abs(x0) < 0.1, wall              # Bloch at D = 0
+    assert x4 > 0.8 and abs(y4) < 0.1, wall                   # Neel at 0.3 mJ/m^2, m_x > 0 for D > 0 (Eq. 16: cycloid energy s D k')
+    xs = [a for a, _ in wall]
+    assert all(b >= a - 1e-3 for a, b in zip(xs, xs[1:])), wall       # |m_x| grows monotonically with D
+    assert 0.05 < wall[2][0] < 0.99 or wall[1][0] > 0.05, wall       # the transition is gradual around 0.1 mJ/m^2
