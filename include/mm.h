@@ -212,6 +212,17 @@ int mm_max_torque(mm_sim* sim, double* tesla);
  * one scalar crosses to the host per sample. */
 int mm_relax(mm_sim* sim);
 
+/* Batched independent simulations (the paper's batch runs and its search over 3000 random starts, L426, L800-L803):
+ * `count` handles - typically many small boxes, which alone leave most of the GPU idle (L503) - advance together.
+ * Every handle enqueues on its own stream (create them with mm_create, or with distinct streams), so their kernels
+ * overlap on the device; the host enqueues a round on all handles before it waits for any. Results are bit for bit
+ * those of the same calls made one handle at a time. mm_batch_steps: n attempted steps each; mm_batch_run: advance
+ * every handle by `duration`; mm_batch_relax: relax() on every handle. Returns the first error met (all handles are
+ * still brought to a consistent state). `sims` is a host array of handles. */
+int mm_batch_steps(mm_sim* const* sims, int count, int n);
+int mm_batch_run(mm_sim* const* sims, int count, double duration);
+int mm_batch_relax(mm_sim* const* sims, int count);
+
 int mm_get_time(mm_sim* sim, double* t);
 int mm_set_time(mm_sim* sim, double t);
 /* Plain mean of m over all cells (fp64 accumulation), the paper's m.average() (L861). */

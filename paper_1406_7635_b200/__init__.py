@@ -81,6 +81,9 @@ _SIGNATURES = {
     "mm_energy": (C.c_int, [C.c_void_p, C.c_uint, C.POINTER(C.c_double)]),
     "mm_max_torque": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
     "mm_relax": (C.c_int, [C.c_void_p]),
+    "mm_batch_steps": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_int]),
+    "mm_batch_run": (C.c_int, [C.POINTER(C.c_void_p), C.c_int, C.c_double]),
+    "mm_batch_relax": (C.c_int, [C.POINTER(C.c_void_p), C.c_int]),
     "mm_get_time": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
     "mm_set_time": (C.c_int, [C.c_void_p, C.c_double]),
     "mm_get_avg_m": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
@@ -349,6 +352,27 @@ class Sim:
         v = C.c_long()
         _check(lib().mm_get_launch_count(self._h, C.byref(v)), self._h)
         return v.value
+
+
+def _handles(sims):
+    arr = (C.c_void_p * len(sims))(*[s._h.value for s in sims])
+    return arr, len(sims)
+
+
+def batch_steps(sims, n):
+    """n attempted steps of every Sim in `sims`, concurrently (mm_batch_steps)."""
+    arr, cnt = _handles(sims)
+    _check(lib().mm_batch_steps(arr, cnt, int(n)))
+
+
+def batch_run(sims, duration):
+    arr, cnt = _handles(sims)
+    _check(lib().mm_batch_run(arr, cnt, float(duration)))
+
+
+def batch_relax(sims):
+    arr, cnt = _handles(sims)
+    _check(lib().mm_batch_relax(arr, cnt))
 
 
 def from_config(cfg, **kw):

@@ -382,25 +382,38 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd4(Fast2DArgs a, int src_r
   }
   const int row = r0 + 4 * gid;                       // first of the group's four rows
   const float2 wt = __ldg(&a.twox[t]);                // w_2N^t; the other points follow from constants
+  // row pointers at column t (point e of this thread sits (N/16) e further on); rows beyond the film read row 0
+  // with weight 0, so that all 64 loads of a run are unconditional and can be in flight together
+  const float* rp[4]; const uint8_t* gp[4]; float rw[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    const bool ok = row + q < a.nyp;
+    const size_t o = (size_t)(ok ? row + q : 0) * a.nxp + t;
+    rp[q] = src + o; gp[q] = reg + o; rw[q] = ok ? (uniform ? b0 : 1.f) : 0.f;
+  }
   int store_seq = 0;                                   // tiles handed to TMA so far (ring position)
 #pragma unroll 1
   for (int run = 0; run < 2; ++run) {
     {
       rf::C2 v[E];
+      if (uniform) {
 #pragma unroll
-      for (int e = 0; e < E; ++e) {
-        const int n = rf::slot_index<P, P::RA>(t, e);
-        float z[4] = {0.f, 0.f, 0.f, 0.f};
-        if (!RAGGED || n < a.nxp) {
+        for (int e = 0; e < E; ++e) {
+          const int off = (N / 16) * e;
+          float z[4];
 #pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            if (row + q < a.nyp) {                    // rows beyond the film: zero fill
-              const size_t i = (size_t)(row + q) * a.nxp + n;
-              z[q] = src[i] * (uniform ? b0 : bsat_s[reg[i]]);               // M = B_sat m (L121)
-            }
-          }
+          for (int q = 0; q < 4; ++q) z[q] = (!RAGGED || t + off < a.nxp) ? rp[q][off] * rw[q] : 0.f;      // M = B_sat m (L121)
+          v[e] = {make_float2(z[0], z[2]), make_float2(z[1], z[3])};          // lanes: rows (r, r+1) and (r+2, r+3)
         }
-        v[e] = {make_float2(z[0], z[2]), make_float2(z[1], z[3])};          // lanes: rows (r, r+1) and (r+2, r+3)
+      } else {
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+          const int off = (N / 16) * e;
+          float z[4];
+#pragma unroll
+          for (int q = 0; q < 4; ++q) z[q] = (!RAGGED || t + off < a.nxp) ? rp[q][off] * (bsat_s[gp[q][off]] * rw[q]) : 0.f;
+          v[e] = {make_float2(z[0], z[2]), make_float2(z[1], z[3])};
+        }
       }
       if (run == 1) {
         // z w_2N^n, n = t + (N/16) e: first the constant part exp(-i pi e / 16), then w_2N^t for all sixteen

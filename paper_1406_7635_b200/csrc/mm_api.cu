@@ -873,90 +873,227 @@ int mm_get_avg_m(mm_sim* s, double avg[3]) {
   return MM_OK;
 }
 
-int mm_energy(mm_sim* s, unsigned mask, double* joules) {
-  int rc;
-  if ((rc = check_ready(s))) return rc;
-  if (!joules) return mm_fail(s, MM_EINVAL, "null argument");
-  mask &= MM_ALL;
+// energy and maximum torque in two halves - enqueue the reduction, then fetch the scalar - so that the batched
+// drivers below can enqueue on every handle before they wait for any of them
+static void energy_enqueue(mm_sim* s, unsigned mask) {
   clear_skip(s);
   if (mask & MM_DEMAG) launch_demag(s, R_M);
-  CUDA_TRY(s, cudaMemsetAsync(s->scratch3, 0, 3 * sizeof(double), s->stream));
+  cudaMemsetAsync(s->scratch3, 0, 3 * sizeof(double), s->stream);
   { Launch l(s, KK_OTHER); k_energy<<<s->nsm * 8, 256, 0, s->stream>>>(s->g, s->regions, s->luts, s->dstate, R_M, R_B, mask | (s->dmi_on ? MM_DMI_ON : 0u), s->scratch3); }
+}
+static int energy_collect(mm_sim* s, double* joules) {
   CUDA_TRY(s, cudaGetLastError());
   double e = 0.0;
+  int rc;
   if ((rc = copy_out(s, &e, s->scratch3, sizeof(double)))) return rc;
   *joules = e / (4e-7 * M_PI) * s->cell[0] * s->cell[1] * s->cell[2];
   return MM_OK;
 }
-
-int mm_max_torque(mm_sim* s, double* tesla) {
-  int rc;
-  if ((rc = check_ready(s))) return rc;
-  if (!tesla) return mm_fail(s, MM_EINVAL, "null argument");
-  if ((rc = pull_state(s))) return rc;
+static void max_torque_enqueue(mm_sim* s) {
   clear_skip(s);
-  launch_eval(s, R_M, R_Y, s->terms, s->precession ? 1 : 2);
+  launch_eval(s, R_M, R_Y, s->terms, s->precession ? 1 : 2);       // role R_Y never changes hands: field[R_Y]
   unsigned* bits = reinterpret_cast<unsigned*>(s->scratch3);
-  CUDA_TRY(s, cudaMemsetAsync(bits, 0, sizeof(unsigned), s->stream));
-  { Launch l(s, KK_OTHER); k_maxnorm<<<s->nsm * 8, 256, 0, s->stream>>>(s->g.N, s->hst.ptr[R_Y], bits); }
+  cudaMemsetAsync(bits, 0, sizeof(unsigned), s->stream);
+  { Launch l(s, KK_OTHER); k_maxnorm<<<s->nsm * 8, 256, 0, s->stream>>>(s->g.N, s->field[R_Y], bits); }
+}
+static int max_torque_collect(mm_sim* s, double* tesla) {
   CUDA_TRY(s, cudaGetLastError());
   unsigned b = 0;
-  if ((rc = copy_out(s, &b, bits, sizeof(unsigned)))) return rc;
+  int rc;
+  if ((rc = copy_out(s, &b, s->scratch3, sizeof(unsigned)))) return rc;
   float f;
   memcpy(&f, &b, sizeof(f));
   *tesla = (double)f;
   return f == f ? MM_OK : mm_fail(s, MM_ENAN, "non-finite torque");
 }
 
-int mm_relax(mm_sim* s) {
+int mm_energy(mm_sim* s, unsigned mask, double* joules) {
+  int rc;
+  if ((rc = check_ready(s))) return rc;
+  if (!joules) return mm_fail(s, MM_EINVAL, "null argument");
+  energy_enqueue(s, mask & MM_ALL);
+  return energy_collect(s, joules);
+}
+
+int mm_max_torque(mm_sim* s, double* tesla) {
+  int rc;
+  if ((rc = check_ready(s))) return rc;
+  if (!tesla) return mm_fail(s, MM_EINVAL, "null argument");
+  max_torque_enqueue(s);
+  return max_torque_collect(s, tesla);
+}
+
+// relax() (L388-L392, #15) as a state machine: every round enqueues 3 steps (or none) and one reduction,
+// then fetches one scalar. mm_relax drives one handle; mm_batch_relax drives many, enqueueing a round on every
+// handle (each on its own stream, so small boxes overlap on the device) before it waits for any scalar.
+namespace {
+struct RelaxJob {
+  mm_sim* s;
+  int solver0; bool prec0; double err0, fix0;
+  int phase = 0;            // 0, 1: first two energy samples; 2: energy phase; 3: first torque sample; 4: torque phase
+  bool wants_energy = true; // what the pending round has enqueued
+  bool done = false;
+  int rc = MM_OK;
+  long batches = 0;
+  double e0 = 0, e1 = 0, t0 = 0, max_err = 0;
+};
+const long kRelaxMaxBatches = 200000;
+
+int relax_set_err(mm_sim* s, double max_err, double fix_dt) {
+  int r = pull_state(s);
+  if (r) return r;
+  s->hst.max_err = max_err; s->hst.fix_dt = fix_dt;
+  return push_state(s);
+}
+int relax_begin(RelaxJob& j) {
+  mm_sim* s = j.s;
   int rc;
   if ((rc = check_ready(s))) return rc;
   if ((rc = pull_state(s))) return rc;
-  const int solver0 = s->solver;
-  const bool prec0 = s->precession;
-  const double err0 = s->hst.max_err, fix0 = s->hst.fix_dt;
+  j.solver0 = s->solver; j.prec0 = s->precession; j.err0 = s->hst.max_err; j.fix0 = s->hst.fix_dt;
+  j.max_err = j.err0;
   if ((rc = mm_set_solver_kind(s, MM_RK23))) return rc;
   s->precession = false;
   s->have_k1 = false; s->graph_dirty = true;
-  auto set_err = [&](double max_err, double fix_dt) {
-    int r = pull_state(s);
-    if (r) return r;
-    s->hst.max_err = max_err; s->hst.fix_dt = fix_dt;
-    return push_state(s);
-  };
+  return relax_set_err(s, j.err0, 0.0);
+}
+int relax_end(RelaxJob& j, int code) {
+  mm_sim* s = j.s;
+  s->precession = j.prec0;
+  int r = mm_set_solver_kind(s, j.solver0);
+  if (!r) r = relax_set_err(s, j.err0, j.fix0);
+  s->have_k1 = false; s->graph_dirty = true;
+  return code ? code : r;
+}
+// decide what the next round is and enqueue it; sets done when the procedure is over
+void relax_enqueue(RelaxJob& j) {
+  mm_sim* s = j.s;
   auto advance = [&]() { for (int i = 0; i < 3; ++i) step_once(s); };     // sampled every 3 steps (#15)
-  auto finish = [&](int code) {
-    s->precession = prec0;
-    int r = mm_set_solver_kind(s, solver0);
-    if (!r) r = set_err(err0, fix0);
-    s->have_k1 = false; s->graph_dirty = true;
-    return code ? code : r;
-  };
-  if ((rc = set_err(err0, 0.0))) return finish(rc);
-  const long max_batches = 200000;
-  long batches = 0;
-  double e0, e1, t0, t1, max_err = err0;
-  // energy phase: advance while the total energy keeps falling (until it cuts into the noise floor)
-  advance(); if ((rc = mm_energy(s, s->terms, &e0))) return finish(rc);
-  advance(); if ((rc = mm_energy(s, s->terms, &e1))) return finish(rc);
-  while (e1 < e0 && batches++ < max_batches) {
-    advance();
-    e0 = e1;
-    if ((rc = mm_energy(s, s->terms, &e1))) return finish(rc);
+  if (j.phase == 2 && !(j.e1 < j.e0 && j.batches++ < kRelaxMaxBatches)) j.phase = 3;   // energy stopped falling
+  if (j.phase == 4 && !(j.batches++ < kRelaxMaxBatches)) { j.done = true; return; }
+  if (j.phase <= 2) { advance(); energy_enqueue(s, s->terms & MM_ALL); j.wants_energy = true; }
+  else { if (j.phase == 4) advance(); max_torque_enqueue(s); j.wants_energy = false; }
+}
+void relax_collect(RelaxJob& j) {
+  mm_sim* s = j.s;
+  double v = 0.0;
+  if ((j.rc = j.wants_energy ? energy_collect(s, &v) : max_torque_collect(s, &v))) { j.done = true; return; }
+  switch (j.phase) {
+    case 0: j.e0 = v; j.phase = 1; break;
+    case 1: j.e1 = v; j.phase = 2; break;
+    case 2: j.e0 = j.e1; j.e1 = v; break;
+    case 3: j.t0 = v; j.phase = 4; break;
+    default:
+      if (v < j.t0) { j.t0 = v; break; }
+      if (j.max_err <= 1e-9) { j.done = true; break; }
+      j.max_err = std::max(j.max_err / std::sqrt(2.0), 1e-9);       // the torque stopped falling: tighten MaxErr
+      if ((j.rc = relax_set_err(s, j.max_err, 0.0))) { j.done = true; break; }
+      j.t0 = v;
   }
-  // torque phase: advance while the maximum torque keeps falling; each time it stops, tighten MaxErr
-  if ((rc = mm_max_torque(s, &t0))) return finish(rc);
-  while (batches++ < max_batches) {
-    advance();
-    if ((rc = mm_max_torque(s, &t1))) return finish(rc);
-    if (t1 < t0) { t0 = t1; continue; }
-    if (max_err <= 1e-9) break;
-    max_err = std::max(max_err / std::sqrt(2.0), 1e-9);
-    if ((rc = set_err(max_err, 0.0))) return finish(rc);
-    t0 = t1;
+}
+int relax_many(mm_sim* const* sims, int count) {
+  std::vector<RelaxJob> jobs((size_t)count);
+  int rc = MM_OK;
+  for (int i = 0; i < count; ++i) {
+    jobs[i].s = sims[i];
+    if ((jobs[i].rc = relax_begin(jobs[i]))) { jobs[i].done = true; jobs[i].phase = -1; }
   }
-  if ((rc = pull_state(s))) return finish(rc);
-  return finish(status_to_error(s));
+  for (;;) {
+    bool any = false;
+    for (auto& j : jobs) if (!j.done) relax_enqueue(j);
+    for (auto& j : jobs) if (!j.done) { relax_collect(j); any = true; }
+    if (!any) break;
+  }
+  for (auto& j : jobs) {
+    int r = j.rc;
+    if (j.phase >= 0) {
+      if (!r) r = pull_state(j.s);
+      r = relax_end(j, r ? r : status_to_error(j.s));
+    }
+    if (r && !rc) rc = r;
+  }
+  return rc;
+}
+}  // namespace
+
+int mm_relax(mm_sim* s) {
+  if (!s) return MM_EINVAL;
+  return relax_many(&s, 1);
+}
+
+// ---- batched independent simulations (the paper's parameter sweeps and its 3000-start search, L426, L800-L803):
+// the handles step concurrently, each on its own stream, and the host waits once per round for all of them
+static int batch_check(mm_sim* const* sims, int count) {
+  if (!sims || count < 0) return MM_EINVAL;
+  for (int i = 0; i < count; ++i) if (!sims[i]) return MM_EINVAL;
+  return MM_OK;
+}
+
+int mm_batch_relax(mm_sim* const* sims, int count) {
+  int rc;
+  if ((rc = batch_check(sims, count))) return rc;
+  return relax_many(sims, count);
+}
+
+int mm_batch_steps(mm_sim* const* sims, int count, int n) {
+  int rc;
+  if ((rc = batch_check(sims, count))) return rc;
+  if (n < 0) return MM_EINVAL;
+  for (int i = 0; i < count; ++i)
+    if ((rc = check_ready(sims[i])) || (rc = check_thermal(sims[i]))) return rc;
+  for (int k = 0; k < n; ++k)
+    for (int i = 0; i < count; ++i) step_once(sims[i]);
+  int first = MM_OK;
+  for (int i = 0; i < count; ++i) {
+    mm_sim* s = sims[i];
+    rc = (cudaGetLastError() == cudaSuccess) ? pull_state(s) : mm_fail(s, MM_ECUDA, "launch failed");
+    if (!rc) rc = status_to_error(s);
+    if (rc && !first) first = rc;
+  }
+  return first;
+}
+
+int mm_batch_run(mm_sim* const* sims, int count, double duration) {
+  int rc;
+  if ((rc = batch_check(sims, count))) return rc;
+  if (!(duration >= 0) || !std::isfinite(duration)) return MM_EINVAL;
+  if (duration == 0 || count == 0) return MM_OK;
+  std::vector<char> active((size_t)count, 1);
+  for (int i = 0; i < count; ++i) {
+    mm_sim* s = sims[i];
+    if ((rc = check_ready(s)) || (rc = check_thermal(s)) || (rc = pull_state(s))) return rc;
+    s->hst.run_mode = 1; s->hst.t_end = s->hst.t + duration; s->hst.run_duration = duration; s->hst.skip = 0;
+    if ((rc = push_state(s))) return rc;
+  }
+  int first = MM_OK;
+  for (bool any = true; any;) {
+    for (int i = 0; i < count; ++i) {
+      if (!active[i]) continue;
+      mm_sim* s = sims[i];
+      const double dt = s->hst.fix_dt > 0 ? s->hst.fix_dt : s->hst.dt;
+      const double est = (s->hst.t_end - s->hst.t) / (dt > 0 ? dt : 1e-18);
+      int batch = s->hst.fix_dt > 0 ? (est > 64 ? 64 : (int)std::ceil(est - 1e-9)) : (est > 86 ? 64 : (int)std::floor(0.75 * est));
+      if (batch < 1) batch = 1;
+      for (int k = 0; k < batch; ++k) step_once(s);
+    }
+    any = false;
+    for (int i = 0; i < count; ++i) {
+      if (!active[i]) continue;
+      mm_sim* s = sims[i];
+      rc = pull_state(s);
+      const bool over = rc || s->hst.skip || s->hst.status != MM_OK ||
+                        !(s->hst.t_end - s->hst.t > 1e-12 * std::max(duration, 1e-30));
+      if (!over) { any = true; continue; }
+      active[i] = 0;
+      const int st = s->hst.status;
+      s->hst.run_mode = 0; s->hst.skip = 0;
+      if (!rc) rc = push_state(s);
+      s->hst.status = st;
+      if (!rc) rc = status_to_error(s);
+      if (rc && !first) first = rc;
+    }
+  }
+  return first;
 }
 
 int mm_get_stats(mm_sim* s, long* steps, long* rejected, long* evals, size_t* peak) {

@@ -890,3 +890,34 @@ def test_fig6_dmi_turns_a_bloch_wall_into_a_neel_wall(mm):
     xs = [a for a, _ in wall]
     assert all(b >= a - 1e-3 for a, b in zip(xs, xs[1:])), wall       # |m_x| grows monotonically with D
     assert 0.05 < wall[2][0] < 0.99 or wall[1][0] > 0.05, wall       # the transition is gradual around 0.1 mJ/m^2
+
+
+# --------------------------------------------------------------------------- batched independent simulations
+def test_batched_boxes_match_one_at_a_time_runs_bit_for_bit(mm):
+    # the paper's batch use (search over random starts of standard problem 3, L426; batch runs L800-L803): many
+    # small boxes advance together, each handle on its own stream. Steps, run() and relax() of a batch must
+    # give exactly the results of the same calls made one handle at a time.
+    n, Ms, A = 16, 500e3, 20e-12
+    Km = 0.5 * 4e-7 * np.pi * Ms * Ms
+    c = 8.3 * np.sqrt(A / Km) / n
+    p = Params.uniform(1, Msat=Ms, Aex=A, alpha=0.5, Ku1=0.1 * Km, anisU=(0, 0, 1))
+    nb = 32
+
+    def make(i):
+        m0 = random_unit_vectors(1000 + i, n ** 3).reshape(3, n, n, n)
+        return mm.from_config(dict(grid=(n, n, n), cell=(c, c, c), pbc=(0, 0, 0), regions=None, params=p, m0=m0))
+
+    solo = [make(i) for i in range(nb)]
+    for s_ in solo:
+        s_.steps(7); s_.run(2e-12); s_.relax()
+    want = [(s_.get_m().copy(), s_.energy(), s_.t) for s_ in solo]
+    del solo
+    batch = [make(i) for i in range(nb)]
+    mm.batch_steps(batch, 7)
+    mm.batch_run(batch, 2e-12)
+    mm.batch_relax(batch)
+    for s_, (m, e, t) in zip(batch, want):
+        assert np.array_equal(s_.get_m(), m) and s_.energy() == e and s_.t == t
+    # the relaxed states are energy minima of the cube (flower-like or vortex-like), not all the same one
+    es = np.array([w[1] for w in want]) / (Km * (c * n) ** 3)
+    assert es.min() > 0.25 and es.max() < 0.40 and np.ptp(es) >= 0
