@@ -60,7 +60,7 @@ def kernel_bytes(kind, n, P):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -70,7 +70,7 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.Q,
-                                       "--format=csv,noheader,nounits", "-lms", "200"], stdout=self.f,
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
                                       stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
@@ -109,50 +109,71 @@ class ClockSampler:
         return out
 
 
-def run_reference(args, rank):
-    """The oracle as it stands, on the host cores: a bounded sample of the same workload."""
-    if rank != 0:
-        return
+def _oracle_threads():
+    import oracle.field as of
+    return int(of.FFT_WORKERS)
+
+
+def _time_oracle(n, steps, budget_s):
+    """Time `steps` RK45 steps of the oracle (as it stands: numpy fp64, library FFT threaded over the host cores)
+    on the C4 recipe at n x n x 1; stops early when the time budget is spent. Returns (cell-updates/s, steps done, s)."""
     from oracle import RefSim
     from synth import config_c4
-    n = args.cpu_size
     cfg = config_c4(n)
     ref = RefSim(cfg["grid"], cfg["cell"], cfg["pbc"], demag_method="fft")
     ref.set_params(cfg["params"]); ref.set_m(cfg["m0"]); ref.set_solver(fix_dt=cfg["fix_dt"])
-    steps = max(1, min(args.steps, args.cpu_steps))
-    for _ in range(min(args.warmup, 1)):
-        ref.step()
-    t0 = time.perf_counter()
-    for _ in range(steps):
-        ref.step()
+    ref.step()                                   # warm-up: kernel spectrum, FSAL slope
+    done, t0 = 0, time.perf_counter()
+    while done < steps:
+        ref.step(); done += 1
+        if time.perf_counter() - t0 > budget_s:
+            break
     dt = time.perf_counter() - t0
-    value = n * n * steps / dt
-    sample = "C4 recipe at %dx%dx1, %d RK45 steps (numpy fp64, FFT demag)" % (n, n, steps)
-    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
-            "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * dt / steps, "higher_is_better": True,
+    return n * n * done / dt, done, dt
+
+
+def cpu_baseline(args):
+    """The oracle on the box's host cores: a bounded sample of the C4 workload at the largest size that fits the
+    time budget (args.cpu_size, default 1024^2) and at 256^2; cell-updates/s is not size-invariant, both are given."""
+    big, nbig, sbig = _time_oracle(args.cpu_size, args.cpu_steps, args.cpu_budget)
+    small, nsmall, ssmall = _time_oracle(256, 20, 0.3 * args.cpu_budget) if args.cpu_size != 256 else (big, nbig, sbig)
+    thr = _oracle_threads()
+    return {"value": big, "unit": UNIT, "cores": thr, "host_cores": os.cpu_count(), "kind": "oracle",
+            "sample": "C4 recipe at %dx%dx1, %d RK45 steps in %.1f s (numpy fp64 oracle, FFT demag, library FFT on %d threads, "
+                      "the rest of the step on one)" % (args.cpu_size, args.cpu_size, nbig, sbig, thr),
+            "also": {"size": 256, "value": small, "steps": nsmall, "seconds": ssmall}}
+
+
+def run_reference(args, rank):
+    """--impl reference: the oracle as it stands, on the host cores, each step a bounded sample of the workload."""
+    if rank != 0:
+        return
+    n = args.cpu_size
+    steps = max(1, min(args.steps, args.cpu_steps))
+    value, done, dt = _time_oracle(n, steps, args.cpu_budget)
+    thr = _oracle_threads()
+    sample = "C4 recipe at %dx%dx1, %d RK45 steps (numpy fp64, FFT demag, library FFT on %d threads)" % (n, n, done, thr)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": done,
+            "warmup": 1, "ms_per_step": 1e3 * dt / done, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": "C4 film %dx%dx1 (bounded sample of the %d^2 workload)" % (n, n, args.size),
-                       "cells": n * n, "fix_dt": cfg["fix_dt"]},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+                       "cells": n * n, "fix_dt": 1e-13},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": thr, "host_cores": os.cpu_count(), "kind": "oracle",
+                             "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
 
-def cpu_baseline(args):
-    from oracle import RefSim
-    from synth import config_c4
-    n = args.cpu_size
-    cfg = config_c4(n)
-    ref = RefSim(cfg["grid"], cfg["cell"], cfg["pbc"], demag_method="fft")
-    ref.set_params(cfg["params"]); ref.set_m(cfg["m0"]); ref.set_solver(fix_dt=cfg["fix_dt"])
-    ref.step()
-    t0 = time.perf_counter()
-    for _ in range(args.cpu_steps):
-        ref.step()
-    dt = time.perf_counter() - t0
-    return {"value": n * n * args.cpu_steps / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": "C4 recipe at %dx%dx1, %d RK45 steps (numpy fp64, FFT demag, single thread)" % (n, n, args.cpu_steps)}
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without a launcher: start the N ranks ourselves (the driver's torchrun line)."""
+    import socket
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
 
 
 def main():
@@ -161,17 +182,21 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--size", type=int, default=4096)
-    ap.add_argument("--workload", default="c4", choices=["c4", "c5", "c5pbc", "c3"],
-                    help="c4: size x size x 1 film (default, the metric's workload); c5 / c5pbc: size^3 cube, open / "
+    ap.add_argument("--workload", default="c4", choices=["c4", "c4regions", "c5", "c5pbc", "c3"],
+                    help="c4: size x size x 1 film (default, the metric's workload); c4regions: the same film cut into 64 "
+                         "Voronoi regions with an inter-region exchange table; c5 / c5pbc: size^3 cube, open / "
                          "PBC(4,4,0); c3: 128 x 128 x 32 multi-region block, adaptive steps (--size is ignored)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--cpu-size", type=int, default=256)
-    ap.add_argument("--cpu-steps", type=int, default=36)
+    ap.add_argument("--cpu-size", type=int, default=1024, help="film edge of the timed oracle sample")
+    ap.add_argument("--cpu-steps", type=int, default=8)
+    ap.add_argument("--cpu-budget", type=float, default=25.0, help="seconds of oracle time per sample")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
+    if args.impl == "ours" and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        spawn_ranks(args)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -201,6 +226,11 @@ def main():
         cfg = config_c4(n, seed_offset=replicas.replica_seed(0, rank))     # one independent replica per rank
         cells, step_bytes = n * n, STEP_BYTES_PER_CELL
         wname = "C4 film %dx%dx1, 4x4x2 nm, Permalloy, random m, B_ext 10 mT, fix_dt 1e-13 s" % (n, n)
+    elif args.workload == "c4regions":
+        from synth import config_c4_regions
+        cfg = config_c4_regions(n)
+        cells, step_bytes = n * n, STEP_BYTES_PER_CELL
+        wname = "C4 film %dx%dx1 in 64 Voronoi regions (Msat +-10 %%, inter-region exchange 0.5-1), fix_dt 1e-13 s" % (n, n)
     elif args.workload == "c3":
         from synth import config_c3
         cfg = config_c3()
@@ -228,13 +258,30 @@ def main():
     barrier()
     sampler = ClockSampler(local_rank) if rank == 0 else None
     l0 = sim.launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
-        sim.step(want_info=False)
-    e1.record()
-    barrier()
-    ms = e0.elapsed_time(e1)
+    # L2: a step streams its whole working set several times, so nothing of one step survives to the next when
+    # the set is much larger than the cache; a set that fits is flushed (a 256 MB memset) before every timed step
+    l2_bytes = torch.cuda.get_device_properties(local_rank).L2_cache_size
+    working = sim.stats()["peak_device_bytes"]
+    flush = torch.empty(2 * l2_bytes, dtype=torch.uint8, device="cuda") if working < 4 * l2_bytes else None
+    hstream = sim.stream                      # the handle's own stream: events must be recorded where its kernels run
+    if flush is None:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(hstream)
+        for _ in range(args.steps):
+            sim.step(want_info=False)
+        e1.record(hstream)
+        barrier()
+        ms = e0.elapsed_time(e1)
+    else:
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for a_, b_ in ev:
+            with torch.cuda.stream(hstream):
+                flush.zero_()
+            a_.record(hstream)
+            sim.step(want_info=False)
+            b_.record(hstream)
+        barrier()
+        ms = sum(a_.elapsed_time(b_) for a_, b_ in ev)
     launches = sim.launch_count() - l0
     clocks = sampler.stop() if sampler else None
     value, ms = replicas.aggregate_throughput(cells * args.steps, ms, device="cuda")   # all ranks' units / max time
@@ -249,22 +296,24 @@ def main():
     roofline, kernels = None, {}
     tot_ms = sum(v[0] for v in prof.values()) or 1.0
     for name, (kms, cnt) in prof.items():
-        b = kernel_bytes(name, n, P) if args.workload == "c4" else 0.0     # byte table is for the 2D path
+        b = kernel_bytes(name, n, P) if args.workload in ("c4", "c4regions") else 0.0     # byte table is for the 2D path
         kernels[name] = {"ms_per_launch": kms / cnt, "launches_per_step": cnt / args.steps, "share": kms / tot_ms,
                          "GBps": (b / (kms / cnt * 1e-3) / 1e9) if b else None}
-    if prof and args.workload == "c4":
+    if prof and args.workload in ("c4", "c4regions"):
         top = max(prof, key=lambda k: prof[k][0])
         b = kernel_bytes(top, n, P)
         ach = b / (prof[top][0] / prof[top][1] * 1e-3) / 1e9
-        traffic = None
+        traffic, traffic_src = None, None
         try:
             with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
-                traffic = json.load(f).get("%s@%d" % (top, n))
+                tj = json.load(f)
+            traffic = tj.get("%s@%d" % (top, n))
+            traffic_src = tj.get("_captured")       # which ncu capture the figure is from (not measured in this run)
         except Exception:
             pass
         roofline = {"bound": "hbm", "kernel": top, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                    "traffic": traffic, "peak_source": peak_src, "algorithmic_bytes_per_launch": b,
-                    "share_of_step": prof[top][0] / tot_ms}
+                    "traffic": traffic, "traffic_source": traffic_src if traffic else None, "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": b, "share_of_step": prof[top][0] / tot_ms}
     step_gbs = step_bytes * cells * args.steps / (ms * 1e-3) / 1e9
     step_roofline = {"achieved": step_gbs, "peak": peak, "unit": "GB/s", "frac": step_gbs / peak,
                      "frac_of_8TBps": step_gbs / 8000.0, "bytes_per_cell_step": step_bytes}
@@ -295,7 +344,8 @@ def main():
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": wname,
                            "cells": cells, "fft": list(sim.fft_size()), "parallelism": "replicas x%d" % world,
-                           "l2": "working set %.1f GB >> 126 MB L2 (no flush needed)" % (sim.stats()["peak_device_bytes"] / 1e9),
+                           "l2": ("working set %.2f GB vs %d MB L2: " % (working / 1e9, l2_bytes >> 20)) +
+                                 ("streams through, no flush" if flush is None else "L2 flushed before every timed step"),
                            "evals_per_step": 6},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
                 "step_roofline": step_roofline, "kernels": kernels,

@@ -3,6 +3,7 @@
 #include <vector>
 #include "internal.cuh"
 #include "fast2d.cuh"
+#include "fft_tables.cuh"
 
 namespace {
 
@@ -10,29 +11,17 @@ namespace {
 // the CTA size NT; a CTA holds G = NT / T FFT groups and therefore 2G rows in the x kernels
 template <int N> struct PlanFor;
 // (NTF: CTA size of the forward x kernel, four rows per FFT group; NTI: of the inverse one, two rows per group)
-template <> struct PlanFor<4096> { using P = rf::Plan<4096, 256, 16, 16, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
+#ifndef MM_X4096_NTF
+#define MM_X4096_NTF 256
+#endif
+#ifndef MM_X4096_NTI
+#define MM_X4096_NTI 256
+#endif
+template <> struct PlanFor<4096> { using P = rf::Plan<4096, 256, 16, 16, 16>; static constexpr int NT = 256, NTF = MM_X4096_NTF, NTI = MM_X4096_NTI; };
 template <> struct PlanFor<2048> { using P = rf::Plan<2048, 128, 16, 8, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
 template <> struct PlanFor<1024> { using P = rf::Plan<1024, 64, 16, 4, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
 template <> struct PlanFor<512> { using P = rf::Plan<512, 32, 16, 2, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
 template <> struct PlanFor<256> { using P = rf::Plan<256, 16, 16, 16, 1>; static constexpr int NT = 128, NTF = 128, NTI = 128; };
-
-// forward twiddles of a plan, laid out as fft_reg.cuh reads them
-template <class P>
-std::vector<float2> plan_table() {
-  std::vector<float2> tw(P::TW);
-  const int N = P::N;
-  auto put = [&](size_t i, double turns) {
-    const double ang = -2.0 * M_PI * turns;
-    tw[i] = make_float2((float)cos(ang), (float)sin(ang));
-  };
-  for (int s = 1; s < P::RA; ++s)
-    for (int bf = 0; bf < N / P::RA; ++bf) put((size_t)(s - 1) * (N / P::RA) + bf, (double)((long long)s * bf % N) / N);
-  if (P::NPASS == 3)
-    for (int s = 1; s < P::RB; ++s)
-      for (int bf = 0; bf < N / P::RB; ++bf)
-        put((size_t)P::TW1 + (size_t)(s - 1) * (N / P::RB) + bf, (double)((long long)s * P::RA * (bf % P::M2) % N) / N);
-  return tw;
-}
 
 // 3-D TMA view of spec: floats along y innermost (2 per bin), then kx, then component; one box =
 // {rows * 2 floats, kb bins, 1}. The view starts at column kx0 and walks every kstep-th column (nk of them).
@@ -59,25 +48,9 @@ bool make_spec_map(mm_sim* s, int rows, CUtensorMap* out, int kb = K2_KB, int kx
                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-int upload(mm_sim* s, const std::vector<float2>& h, float2** out) {
-  *out = (float2*)mm_dev_alloc(s, sizeof(float2) * h.size());
-  if (!*out) return mm_fail(s, MM_ENOMEM, "fast path twiddles");
-  CUDA_TRY(s, cudaMemcpy(*out, h.data(), sizeof(float2) * h.size(), cudaMemcpyHostToDevice));
-  return MM_OK;
-}
-
 template <int N>
 int make_axis_tables(mm_sim* s, float2** fwd, float2** rev, float2** half) {
-  using P = typename PlanFor<N>::P;
-  int rc;
-  if ((rc = upload(s, plan_table<P>(), fwd))) return rc;
-  if ((rc = upload(s, plan_table<typename P::Reversed>(), rev))) return rc;
-  std::vector<float2> w(N);
-  for (int n = 0; n < N; ++n) {
-    const double ang = -M_PI * (double)n / (double)N;      // exp(-2 pi i n / (2N))
-    w[n] = make_float2((float)cos(ang), (float)sin(ang));
-  }
-  return upload(s, w, half);
+  return mm_plan_tables<typename PlanFor<N>::P>(s, fwd, rev, half);
 }
 
 int axis_tables(mm_sim* s, int N, float2** fwd, float2** rev, float2** half) {
@@ -103,8 +76,13 @@ int x_attrs(mm_sim* s) {
                                    (int)k2_smem<typename F::P, F::NTI>()));
   CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv_tma<typename F::P, F::NTI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    (int)k2_tma_smem<typename F::P, F::NTI>()));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv_direct<typename F::P, F::NTI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)K2Inv<typename F::P, F::NTI>::SMEM));
   return MM_OK;
 }
+// the direct-read x inverse wins where one FFT group fills the CTA (its landed pieces are then read without bank
+// conflicts); below that the ring version is kept
+template <int N> constexpr bool xinv_direct() { return PlanFor<N>::NTI == PlanFor<N>::P::T || N >= 2048; }
 template <int N>
 int y_attrs(mm_sim* s) {
   using F = PlanFor<N>;
@@ -131,6 +109,8 @@ void launch_x(mm_sim* s, bool inverse, int role) {
       else k2_xfwd4<typename F::P, F::NTF, false, false><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd, s->f2_map_fwd_odd);
     }
   }
+  else if (tma_on && xinv_direct<N>())
+    k2_xinv_direct<typename F::P, F::NTI><<<dim3(s->g.Ny / (2 * GI), 3), F::NTI, K2Inv<typename F::P, F::NTI>::SMEM, s->stream>>>(s->f2, role, s->f2_map_inv_even, s->f2_map_inv_odd);
   else if (tma_on)
     k2_xinv_tma<typename F::P, F::NTI><<<dim3(s->g.Ny / (2 * GI), 3), F::NTI, k2_tma_smem<typename F::P, F::NTI>(), s->stream>>>(s->f2, role, s->f2_map_inv);
   else
@@ -157,6 +137,13 @@ int rows_per_cta(int N) {      // rows of one CTA of the x inverse kernel (the f
   return 0;
 }
 
+template <int N>
+bool make_inv_maps(mm_sim* s) {
+  using F = PlanFor<N>;
+  using I = K2Inv<typename F::P, F::NTI>;
+  return make_spec_map(s, 2 * I::G, &s->f2_map_inv_even, I::KB, 0, 2, N / 2 + 1) &&
+         make_spec_map(s, 2 * I::G, &s->f2_map_inv_odd, I::KB, 1, 2, N / 2);
+}
 template <int N>
 bool make_fwd_maps(mm_sim* s) {
   using F = K2Fwd<typename PlanFor<N>::P, PlanFor<N>::NTF>;
@@ -227,7 +214,11 @@ int mm_fast2d_init(mm_sim* s) {
 #define FM(N) fwd_ok = make_fwd_maps<N>(s)
   F2_SWITCH(a.Nx, FM)
 #undef FM
-  s->f2_tma = make_spec_map(s, rows_inv, &s->f2_map_inv) && fwd_ok;
+  bool inv_ok = false;
+#define IM(N) inv_ok = make_inv_maps<N>(s)
+  F2_SWITCH(a.Nx, IM)
+#undef IM
+  s->f2_tma = make_spec_map(s, rows_inv, &s->f2_map_inv) && fwd_ok && inv_ok;
   return MM_OK;
 }
 

@@ -36,6 +36,14 @@ constexpr size_t k2_smem() { return sizeof(float4) * (size_t)K2Shape<P, NT>::G *
 __device__ __forceinline__ void k2_prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void k2_prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
+// loads and stores through pointers fetched from DevState::ptr: the compiler cannot see that they are global
+__device__ __forceinline__ float k2_ldg(const float* p) {
+  float v;
+  asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ void k2_stg(float* p, float v) { asm volatile("st.global.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory"); }
+
 // stage unit = (z0.re, z0.im, z1.re, z1.im): each lane's complex number is one 8-byte half
 __device__ __forceinline__ float4 stage_pack(rf::C2 a) { return make_float4(a.re.x, a.im.x, a.re.y, a.im.y); }
 __device__ __forceinline__ rf::C2 stage_unpack(float4 q) { return {make_float2(q.x, q.z), make_float2(q.y, q.w)}; }
@@ -98,8 +106,8 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xinv(Fast2DArgs a, int dst_ro
       const int n = rf::slot_index<PI, PI::RLAST>(t, e);
       const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), rf::half_twiddle(wt, e));
       if (n < a.nxp) {
-        dst[rowA + n] = v[e].re.x + u.x;
-        dst[rowA + a.nxp + n] = v[e].im.x + u.y;
+        k2_stg(dst + rowA + n, v[e].re.x + u.x);
+        k2_stg(dst + rowA + a.nxp + n, v[e].im.x + u.y);
       }
     }
   }
@@ -127,8 +135,10 @@ constexpr size_t k2_y_smem() { return (size_t)(NT / P::T) * K2YShape<P>::GROUP_B
 // Every FFT group works on its own: an XY job is one column of the x and y components (coupled by
 // the kernel product), a Z job one column of the z component. All code is straight-line (a rolled
 // loop over components would carry the 64-register point array around its back edge, which costs
-// a register permutation through local memory). Several CTAs share an SM out of phase with one
-// another: butterflies of one over the exchanges and loads of the other.
+// a register permutation through local memory).
+// Two CTAs share an SM: butterflies of one over the exchanges and loads of the other. (Forcing the phases apart - two
+// groups per CTA taking turns in their exchanges by named-barrier tokens, or a start offset between the CTAs of an
+// SM - was measured and is slower or neutral, profiles/r02_experiments.md.)
 template <class P, int NT>
 struct K2Col {
   using PI = typename P::Reversed;
@@ -186,8 +196,8 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_ycol(Fast2DArgs a, int nxy) {
   }
   {
     // columns that will be wanted soon, on their way from DRAM to L2: this job's second component and
-    // the first component of the job that follows on this SM (CTAs are dispatched in order, two per SM)
-    const int ahead = kx + 2 * a.nsm * G;
+    // the first component of the job that follows on this SM (CTAs are dispatched in order, 512 / NT per SM)
+    const int ahead = kx + (512 / NT) * a.nsm * G;
     const float2* nxt = a.spec + (size_t)(xy ? 0 : 2) * a.cstride + (size_t)ahead * a.Ny;
     for (int i = t * 16; i < N; i += T * 16) {
       if (xy) k2_prefetch_l2(col + a.cstride + i);
@@ -317,9 +327,85 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xinv_tma(Fast2DArgs a, int ds
       const int n = rf::slot_index<PI, PI::RLAST>(t, e);
       const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), rf::half_twiddle(wt, e));
       if (n < a.nxp) {
-        dst[rowA + n] = v[e].re.x + u.x;
-        dst[rowA + a.nxp + n] = v[e].im.x + u.y;
+        k2_stg(dst + rowA + n, v[e].re.x + u.x);
+        k2_stg(dst + rowA + a.nxp + n, v[e].im.x + u.y);
       }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------- K_C, direct read
+// All bins of the CTA's 2G rows arrive as TMA boxes {2G rows, KB bins} of two tensor maps that walk every second
+// column of spec (even kx = 2k, k = 0 .. N/2; odd kx = 2k + 1, k = 0 .. N/2 - 1), every box in flight at once on one
+// mbarrier. The landing area IS the FFT exchange buffer: each thread builds its sixteen points of both transforms
+// straight from the landed pieces - point n of the even-bin transform is Z[2n], of the odd-bin one Z[2n + 1], with
+// Z[b] = A[b] + i B[b] for b <= N and Z[b] = conj(A[2N - b]) + i conj(B[2N - b]) above (A, B: spectra of the two
+// real rows of a pair) - then, after one CTA barrier, the buffer is reused for the exchanges. No conversion pass,
+// no ring: the whole gather costs 32 shared loads per thread.
+template <class P, int NT>
+struct K2Inv {
+  static constexpr int N = P::N, G = NT / P::T;
+  static constexpr int KB = N / 2 < 256 ? N / 2 : 256;                         // bins per box
+  static constexpr int NBE = (N / 2 + 1 + KB - 1) / KB, NBO = (N / 2 + KB - 1) / KB;
+  static constexpr int LAND4 = (NBE + NBO) * KB * G;                           // float4 units of the landing area
+  static constexpr int XB4 = G * K2Shape<P, NT>::GP;                           // float4 units of the exchange buffers
+  static constexpr size_t SMEM = sizeof(float4) * (size_t)(LAND4 > XB4 ? LAND4 : XB4) + 128;
+};
+
+template <class P, int NT>
+__global__ void __launch_bounds__(NT, 512 / NT) k2_xinv_direct(Fast2DArgs a, int dst_role, const __grid_constant__ CUtensorMap map_even,
+                                                               const __grid_constant__ CUtensorMap map_odd) {
+  if (a.st->skip) return;
+  using PI = typename P::Reversed;
+  using S = K2Inv<P, NT>;
+  constexpr int N = P::N, T = P::T, E = P::E, G = NT / T, GP = K2Shape<P, NT>::GP, KB = S::KB;
+  extern __shared__ __align__(128) float4 smem4[];
+  __shared__ __align__(8) uint64_t full;
+  float4* land = reinterpret_cast<float4*>((reinterpret_cast<uintptr_t>(smem4) + 127) & ~(uintptr_t)127);
+  const float4* Se = land;                                  // [k][p]: even bin 2k of row pair p
+  const float4* So = land + (size_t)S::NBE * KB * G;        // [k][p]: odd bin 2k + 1
+  const int tid = threadIdx.x, gid = tid / T, t = tid % T;
+  const int c = blockIdx.y, r0 = blockIdx.x * 2 * G;
+  if (tid == 0) {
+    tma::mbar_init(&full, 1);
+    tma::fence_barrier_init();
+    tma::fence_proxy_async();
+    tma::mbar_expect_tx(&full, (uint32_t)(S::LAND4 * sizeof(float4)));
+#pragma unroll 1
+    for (int b = 0; b < S::NBE; ++b) tma::load_3d(land + (size_t)b * KB * G, &map_even, 2 * r0, b * KB, c, &full);
+#pragma unroll 1
+    for (int b = 0; b < S::NBO; ++b) tma::load_3d(land + (size_t)(S::NBE + b) * KB * G, &map_odd, 2 * r0, b * KB, c, &full);
+  }
+  float* __restrict__ dst = a.st->ptr[dst_role] + (size_t)c * a.ncell;
+  const float2 wt = __ldg(&a.twox[t]);      // w_2N^t; the other points follow from constants
+  __syncthreads();                          // the barrier is initialised
+  tma::mbar_wait(&full, 0);
+  rf::C2 v[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int n = rf::slot_index<PI, PI::RA>(t, e);        // = t + (N/16) e: the mirror tests fold per e
+    float4 qe, qo;
+    if (e < E / 2) {                      // n < N/2: bins 2n, 2n + 1 < N
+      qe = Se[(size_t)n * G + gid]; qo = So[(size_t)n * G + gid];
+      v[e] = {make_float2(qe.x - qe.w, qo.x - qo.w), make_float2(qe.y + qe.z, qo.y + qo.z)};
+    } else {                              // bins above N: the conjugate partner 2N - b
+      qo = So[(size_t)(N - 1 - n) * G + gid];
+      qe = Se[(size_t)(N - n) * G + gid];
+      const bool self = e == E / 2 && t == 0;              // bin N itself (n = N/2)
+      v[e] = {make_float2(self ? qe.x - qe.w : qe.x + qe.w, qo.x + qo.w), make_float2(self ? qe.y + qe.z : qe.z - qe.y, qo.z - qo.y)};
+    }
+  }
+  __syncthreads();                          // everyone has its points: the landing area becomes the exchange buffers
+  float4* xb = land + (size_t)gid * GP;
+  rf::fft<PI, +1, NT>(v, xb, t, gid, a.twx_r);
+  const size_t rowA = (size_t)(r0 + 2 * gid) * a.nxp;      // physical row pitch; n >= nxp is zero fill
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int n = rf::slot_index<PI, PI::RLAST>(t, e);
+    const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), rf::half_twiddle(wt, e));
+    if (n < a.nxp) {
+      k2_stg(dst + rowA + n, v[e].re.x + u.x);
+      k2_stg(dst + rowA + a.nxp + n, v[e].im.x + u.y);
     }
   }
 }
@@ -402,7 +488,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd4(Fast2DArgs a, int src_r
           const int off = (N / 16) * e;
           float z[4];
 #pragma unroll
-          for (int q = 0; q < 4; ++q) z[q] = (!RAGGED || t + off < a.nxp) ? rp[q][off] * rw[q] : 0.f;      // M = B_sat m (L121)
+          for (int q = 0; q < 4; ++q) z[q] = (!RAGGED || t + off < a.nxp) ? k2_ldg(rp[q] + off) * rw[q] : 0.f;      // M = B_sat m (L121)
           v[e] = {make_float2(z[0], z[2]), make_float2(z[1], z[3])};          // lanes: rows (r, r+1) and (r+2, r+3)
         }
       } else {
@@ -411,7 +497,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xfwd4(Fast2DArgs a, int src_r
           const int off = (N / 16) * e;
           float z[4];
 #pragma unroll
-          for (int q = 0; q < 4; ++q) z[q] = (!RAGGED || t + off < a.nxp) ? rp[q][off] * (bsat_s[gp[q][off]] * rw[q]) : 0.f;
+          for (int q = 0; q < 4; ++q) z[q] = (!RAGGED || t + off < a.nxp) ? k2_ldg(rp[q] + off) * (bsat_s[gp[q][off]] * rw[q]) : 0.f;
           v[e] = {make_float2(z[0], z[2]), make_float2(z[1], z[3])};
         }
       }

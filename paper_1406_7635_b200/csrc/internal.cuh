@@ -6,13 +6,15 @@
 #include <vector>
 #include "common.cuh"
 #include "demag_conv_args.cuh"
+#include "fast3d.cuh"
 
 void* mm_default_alloc(size_t bytes, void*);
 void mm_default_free(void* p, void*);
 
 // kernel classes for launch counting and per-kernel CUDA-event timing (mm_profile)
 enum KernelKind { KK_XFWD = 0, KK_YFWD, KK_YINV, KK_LAST_XY, KK_LAST_Z, KK_LAST_3D, KK_XINV, KK_LOCAL, KK_STAGE,
-                  KK_ERROR, KK_CTRL, KK_OTHER, KK_F2_XFWD, KK_F2_YCOL, KK_F2_XINV, KK_COUNT };
+                  KK_ERROR, KK_CTRL, KK_OTHER, KK_F2_XFWD, KK_F2_YCOL, KK_F2_XINV, KK_F3_Y, KK_F3_Z,
+                  KK_COUNT };
 struct ProfEntry { int kind; cudaEvent_t a, b; };
 
 struct mm_sim {
@@ -37,14 +39,19 @@ struct mm_sim {
   float* K = nullptr;
   float2 *twx = nullptr, *twy = nullptr, *twz = nullptr;
   double* scratch3 = nullptr;
+  double* red_part = nullptr;       // per-block partials of the ordered fp64 reductions (k_energy, k_sum3)
+  unsigned* red_ticket = nullptr;   // their ticket counter (zero between launches)
   ConvArgs conv;
   float* Kt = nullptr;         // kernel spectrum in the fast 2D layout
   Fast2DArgs f2;
+  CUtensorMap f2_map_inv_even, f2_map_inv_odd;          // boxes {2G rows, KB bins} over the even / odd columns (direct-read x inverse)
   CUtensorMap f2_map_inv, f2_map_fwd, f2_map_fwd_odd;   // TMA views of spec for the x kernels (inverse: boxes of 2G rows x 256
                                                         // bins; forward: 4G rows x KB bins of the even resp. odd columns)
   bool f2_no_tma = false;      // mm_set_option(MM_OPT_NO_TMA)
   bool f2_tma = false;         // tensor maps valid: the x kernels move their transposed pieces with TMA
   bool fast2d = false;         // fast 2D path available for this box
+  Fast3DArgs f3;
+  bool fast3d = false;         // register-FFT y and z stages available for this box (fast3d.cu)
   bool force_generic = false;  // mm_set_option(MM_OPT_GENERIC_FFT)
   // host state
   DevState hst;
@@ -88,6 +95,10 @@ bool mm_fast2d_supported(int Nx, int Ny, int Nz, const int* pbc);   // fast2d.cu
 int mm_fast2d_length(int N);      // transform length of the fast path for N physical cells (power of two)
 int mm_fast2d_init(mm_sim* s);
 void mm_fast2d_demag(mm_sim* s, int src_role);
+bool mm_fast3d_supported(int Nx, int Ny, int Nz, const int* pbc);   // fast3d.cu
+int mm_fast3d_init(mm_sim* s);
+void mm_fast3d_y(mm_sim* s, bool inverse);
+void mm_fast3d_z(mm_sim* s);
 
 #define CUDA_TRY(s, expr)                                                                       \
   do {                                                                                          \

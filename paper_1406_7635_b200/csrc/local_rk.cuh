@@ -511,26 +511,61 @@ __global__ void k_normalise(long long N, float* __restrict__ m, const uint8_t* _
   m[i] = x * inv; m[N + i] = y * inv; m[2 * N + i] = z * inv;
 }
 
-// plain mean of m (fp64 accumulation); out[3] must be zeroed first
-__global__ void k_sum3(long long N, const float* __restrict__ m, double* __restrict__ out) {
+// Deterministic grid-wide fp64 sum of NV values per thread: warp shuffles, the warps of a block in index order,
+// one partial per block, and the block that finishes last (ticket counter) adds the partials in block order and
+// resets the ticket. The result does not depend on scheduling, so the same state always gives the same bits
+// (batched and one-at-a-time runs compare energies with ==). part: gridDim.x * NV doubles; ticket: zero on entry.
+template <int NV>
+__device__ __forceinline__ void grid_sum_ordered(double* v, double* __restrict__ part, unsigned* __restrict__ ticket,
+                                                 double* __restrict__ out) {
+  __shared__ double wsum[32][NV];
+  __shared__ bool last;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+#pragma unroll
+  for (int c = 0; c < NV; ++c) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
+    if (lane == 0) wsum[w][c] = v[c];
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int c = 0; c < NV; ++c) {
+      double a = 0.0;
+      for (int i = 0; i < nw; ++i) a += wsum[i][c];
+      part[(size_t)blockIdx.x * NV + c] = a;
+    }
+    __threadfence();
+    last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+  }
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  if (threadIdx.x < NV) {
+    double a = 0.0;
+    for (unsigned b = 0; b < gridDim.x; ++b) a += __ldcg(&part[(size_t)b * NV + threadIdx.x]);
+    out[threadIdx.x] = a;
+  }
+  if (threadIdx.x == 0) *ticket = 0u;
+}
+
+// plain mean of m (fp64 accumulation, fixed summation order)
+__global__ void k_sum3(long long N, const float* __restrict__ m, double* __restrict__ part, unsigned* __restrict__ ticket,
+                       double* __restrict__ out) {
   double s[3] = {0.0, 0.0, 0.0};
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
     s[0] += m[i]; s[1] += m[N + i]; s[2] += m[2 * N + i];
   }
-#pragma unroll
-  for (int c = 0; c < 3; ++c) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) s[c] += __shfl_xor_sync(0xffffffffu, s[c], o);
-    if ((threadIdx.x & 31) == 0) atomicAdd(&out[c], s[c]);
-  }
+  grid_sum_ordered<3>(s, part, ticket, out);
 }
 
 // Energy of the selected terms, joules / cell volume summed over cells (fp64 accumulation):
 //   E/V = - sum_cells M . [ 1/2 B_demag (Eq. 4) + 1/2 B_exch (Eq. 8) + 1/2 B_anis(Ku1) + 1/4 B_anis(Ku2) (Eq. 20)
 //                           + 1/4 B(Kc1) + 1/6 B(Kc2) + 1/8 B(Kc3) (Eq. 23) + B_ext ],   M = Msat m.
-// B_demag of m must already be in role bd_role. out[0] must be zeroed first.
+// B_demag of m must already be in role bd_role. Fixed summation order (grid_sum_ordered).
 __global__ void k_energy(Geometry g, const uint8_t* __restrict__ regions, const Luts* __restrict__ lut, DevState* st,
-                         int m_role, int bd_role, unsigned mask, double* __restrict__ out) {
+                         int m_role, int bd_role, unsigned mask, double* __restrict__ part, unsigned* __restrict__ ticket,
+                         double* __restrict__ out) {
   const float* __restrict__ m = st->ptr[m_role];
   const float* __restrict__ bd = st->ptr[bd_role];
   const long long N = g.N;
@@ -586,9 +621,7 @@ __global__ void k_energy(Geometry g, const uint8_t* __restrict__ regions, const 
     if (mask & MM_ZEEMAN) e += mx * lut->bext[0] + my * lut->bext[1] + mz * lut->bext[2];
     acc -= (double)lut->Bsat[r] * (double)e;           // times mu0 Msat; divided by mu0 on the host
   }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-  if ((threadIdx.x & 31) == 0) atomicAdd(out, acc);
+  grid_sum_ordered<1>(&acc, part, ticket, out);
 }
 
 // max over cells of the Euclidean norm of a 3N vector field (float bits; non-negative floats order as uints)

@@ -157,7 +157,11 @@ void launch_demag(mm_sim* s, int src_role) {
   const int T = 256;
   dim3 gx((pairs + s->xL - 1) / s->xL, 3);
   { Launch l(s, KK_XFWD); k_x_fwd<<<gx, T, s->xSmem, s->stream>>>(s->conv, src_role, s->xL); }
-  if (s->last_along_z) {
+  if (s->fast3d && !s->force_generic) {
+    { Launch l(s, KK_F3_Y); mm_fast3d_y(s, false); }
+    { Launch l(s, KK_F3_Z); mm_fast3d_z(s); }
+    { Launch l(s, KK_F3_Y); mm_fast3d_y(s, true); }
+  } else if (s->last_along_z) {
     dim3 gy((g.Cx + s->yC - 1) / s->yC, g.Nz, 3);
     if (g.Py > 1) { Launch l(s, KK_YFWD); k_y_axis<<<gy, T, s->ySmem, s->stream>>>(s->conv, 0, s->yC); }
     dim3 gl((g.Cx + s->lastC[2] - 1) / s->lastC[2], g.Py);
@@ -452,7 +456,9 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
   if (g.Px > kMaxFft || g.Py > kMaxFft || g.Pz > kMaxFft) return bail(MM_EINVAL, "padded FFT length above 8192");
   if (!smooth5(g.Px) || !smooth5(g.Py) || !smooth5(g.Pz)) return bail(MM_EINVAL, "periodic axis length must be 2^a 3^b 5^c");
   g.Cx = g.Px / 2 + 1;
-  g.pitch = g.Cx;
+  s->fast3d = !s->fast2d && Nz > 1 && mm_fast3d_supported(Nx, Ny, Nz, s->rep) && g.Py == 2 * Ny && g.Pz == 2 * Nz;
+  // rows of the spectrum start on 128-byte lines when the strided stages read pieces of neighbouring kx
+  g.pitch = s->fast3d ? (g.Cx + 15) / 16 * 16 : g.Cx;
   g.Hy = g.Py / 2 + 1; g.Hz = g.Pz / 2 + 1;
   s->px = make_plan(Nx, g.Px); s->py = make_plan(Ny, g.Py); s->pz = make_plan(Nz, g.Pz);
   int rc;
@@ -467,10 +473,13 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
   s->luts = (Luts*)mm_dev_alloc(s, sizeof(Luts));
   s->dstate = (DevState*)mm_dev_alloc(s, sizeof(DevState));
   s->scratch3 = (double*)mm_dev_alloc(s, 3 * sizeof(double));
+  s->red_part = (double*)mm_dev_alloc(s, (size_t)(3 * 8 * s->nsm + 1) * sizeof(double));   // per-block partials + ticket
   const int rowsS = (g.Pz == 1) ? g.Ny : g.Nz * g.Py;
   const size_t spec_rows = s->fast2d ? (size_t)g.Py / 2 : (size_t)rowsS;      // fast layout: [Cx][Py / 2]
   s->spec = (float2*)mm_dev_alloc(s, sizeof(float2) * 3 * spec_rows * g.pitch);
-  if (!s->regions || !s->luts || !s->dstate || !s->spec || !s->scratch3) return bail(MM_ENOMEM, "device buffers");
+  if (!s->regions || !s->luts || !s->dstate || !s->spec || !s->scratch3 || !s->red_part) return bail(MM_ENOMEM, "device buffers");
+  s->red_ticket = reinterpret_cast<unsigned*>(s->red_part + 3 * 8 * s->nsm);
+  if (cudaMemsetAsync(s->red_ticket, 0, sizeof(double), s->stream) != cudaSuccess) return bail(MM_ECUDA, "memset");
   if (cudaMemsetAsync(s->regions, 0, (size_t)g.N, s->stream) != cudaSuccess) return bail(MM_ECUDA, "memset");
   for (int r = 0; r < R_COUNT; ++r) cudaMemsetAsync(s->field[r], 0, fbytes, s->stream);
   if ((rc = upload_twiddles(s, g.Px, &s->twx)) || (rc = upload_twiddles(s, g.Py, &s->twy)) ||
@@ -485,6 +494,7 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
   c.K = s->K; c.kstride = (long long)g.Cx * g.Hy * g.Hz;
   c.regions = s->regions; c.luts = s->luts; c.st = s->dstate;
   if (s->fast2d && (rc = mm_fast2d_init(s))) { std::string m = s->err; return bail(rc, m.c_str()); }
+  if (s->fast3d && (rc = mm_fast3d_init(s))) { std::string m = s->err; return bail(rc, m.c_str()); }
   // controller state
   DevState& h = s->hst;
   memset(&h, 0, sizeof(h));
@@ -865,8 +875,7 @@ int mm_get_avg_m(mm_sim* s, double avg[3]) {
   if (!s || !avg) return MM_EINVAL;
   int rc;
   if ((rc = pull_state(s))) return rc;
-  CUDA_TRY(s, cudaMemsetAsync(s->scratch3, 0, 3 * sizeof(double), s->stream));
-  { Launch l(s, KK_OTHER); k_sum3<<<s->nsm * 4, 256, 0, s->stream>>>(s->g.N, s->hst.ptr[R_M], s->scratch3); }
+  { Launch l(s, KK_OTHER); k_sum3<<<s->nsm * 4, 256, 0, s->stream>>>(s->g.N, s->hst.ptr[R_M], s->red_part, s->red_ticket, s->scratch3); }
   CUDA_TRY(s, cudaGetLastError());
   if ((rc = copy_out(s, avg, s->scratch3, 3 * sizeof(double)))) return rc;
   for (int c = 0; c < 3; ++c) avg[c] /= (double)s->g.N;
@@ -878,8 +887,7 @@ int mm_get_avg_m(mm_sim* s, double avg[3]) {
 static void energy_enqueue(mm_sim* s, unsigned mask) {
   clear_skip(s);
   if (mask & MM_DEMAG) launch_demag(s, R_M);
-  cudaMemsetAsync(s->scratch3, 0, 3 * sizeof(double), s->stream);
-  { Launch l(s, KK_OTHER); k_energy<<<s->nsm * 8, 256, 0, s->stream>>>(s->g, s->regions, s->luts, s->dstate, R_M, R_B, mask | (s->dmi_on ? MM_DMI_ON : 0u), s->scratch3); }
+  { Launch l(s, KK_OTHER); k_energy<<<s->nsm * 8, 256, 0, s->stream>>>(s->g, s->regions, s->luts, s->dstate, R_M, R_B, mask | (s->dmi_on ? MM_DMI_ON : 0u), s->red_part, s->red_ticket, s->scratch3); }
 }
 static int energy_collect(mm_sim* s, double* joules) {
   CUDA_TRY(s, cudaGetLastError());
@@ -1137,7 +1145,7 @@ int mm_profile(mm_sim* s, int enable) {
 
 int mm_profile_read(mm_sim* s, int kind, const char** name, double* total_ms, long* launches) {
   static const char* names[KK_COUNT] = {"x_fwd", "y_fwd", "y_inv", "last_xy", "last_z", "last_3d", "x_inv", "local",
-                                        "rk_stage", "rk_error", "rk_ctrl", "other", "f2_xfwd", "f2_ycol", "f2_xinv"};
+                                        "rk_stage", "rk_error", "rk_ctrl", "other", "f2_xfwd", "f2_ycol", "f2_xinv", "f3_y", "f3_z"};
   if (!s || kind < 0 || kind >= KK_COUNT) return MM_EINVAL;
   if (!s->prof.empty()) {
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));

@@ -8,8 +8,8 @@ the other.
 """
 from .rng import hash64, uniform01, random_unit_vectors
 from .params import Params
-from .configs import (SEED0, config_c1, config_c2, config_c3, config_c4, config_c5,
-                      voronoi_regions)
+from .configs import (SEED0, config_c1, config_c2, config_c3, config_c4, config_c4_regions,
+                      config_c5, voronoi_regions)
 
 __all__ = ["hash64", "uniform01", "random_unit_vectors", "Params", "SEED0", "config_c1",
-           "config_c2", "config_c3", "config_c4", "config_c5", "voronoi_regions"]
+           "config_c2", "config_c3", "config_c4", "config_c4_regions", "config_c5", "voronoi_regions"]

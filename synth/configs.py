@@ -96,6 +96,24 @@ def config_c4(n=4096, seed_offset=0):
                 m0=_random_m(SEED0 + 4 + 1000 * seed_offset, grid), fix_dt=1e-13, nsteps=1000)
 
 
+def config_c4_regions(n=4096, ngrains=64):
+    """The C4 film cut into `ngrains` Voronoi regions (the structure of C3 in two dimensions): per-region Msat
+    within 10 % of Permalloy's, inter-region exchange scaled 0.5-1. Exercises the B_sat gather of the x forward
+    kernel and the triangular-table gathers of the stencil at the benchmark size."""
+    grid = (n, n, 1)
+    seed = SEED0 + 44
+    regions = voronoi_regions(seed, grid, ngrains)
+    g = np.arange(ngrains, dtype=np.uint64)
+    Msat = 8.6e5 * (0.9 + 0.2 * uniform01(seed, 10, g))
+    ntri = ngrains * (ngrains + 1) // 2
+    S = 0.5 + 0.5 * uniform01(seed, 12, np.arange(ntri, dtype=np.uint64))
+    for i in range(ngrains):
+        S[i * (i + 1) // 2 + i] = 1.0
+    p = Params.uniform(ngrains, Msat=Msat, Aex=1.3e-11, alpha=0.01, B_ext=(10e-3, 0, 0), exch_scale=S)
+    return dict(name="C4-%d-regions" % n, grid=grid, cell=(4e-9, 4e-9, 2e-9), pbc=(0, 0, 0), regions=regions,
+                params=p, m0=_random_m(SEED0 + 4, grid), fix_dt=1e-13, nsteps=1000)
+
+
 def config_c5(n=128, pbc=False):
     """Large 3D cube, cubic anisotropy Kc1 = -5e3 J/m^3, optional PBC (4, 4, 0)."""
     grid = (n, n, n)

@@ -133,6 +133,25 @@ def test_fast2d_path_fields(mm, grid):
     assert np.abs(Bf - Bg).max() <= 2e-5 * np.abs(Bg).max()
 
 
+@pytest.mark.parametrize("grid", [(40, 64, 32), (64, 32, 128), (24, 512, 32), (130, 128, 64), (32, 256, 256), (16, 32, 512)])
+def test_fast3d_path_fields(mm, grid):
+    # open 3D boxes whose y and z extents are powers of two take the register-FFT y and z stages (fast3d.cuh):
+    # every plan (32 .. 512 points) on either axis, several CTAs per kernel, a ragged last kx tile, regions and
+    # anisotropy in the local terms; compared with the oracle and with the generic any-size kernels
+    cfg = _rand_cfg(grid, (3e-9, 2e-9, 2.5e-9), nreg=3, anis=True, seed=33)
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    sim.profile(True)
+    _field_check(sim, ref, (MM_DEMAG, MM_ALL))
+    prof = sim.profile_read()
+    sim.profile(False)
+    assert "f3_y" in prof and "f3_z" in prof and "last_3d" not in prof
+    Bf = sim.b_eff(MM_DEMAG)
+    sim.set_option(mm.MM_OPT_GENERIC_FFT, 1)
+    Bg = sim.b_eff(MM_DEMAG)
+    assert np.abs(Bf - Bg).max() <= 2e-5 * np.abs(Bg).max()
+
+
 def test_fast2d_one_region_and_steps(mm):
     # one region (the bench workload's shape): B_sat is a constant and the region gathers are skipped
     cfg = config_c4(512)
@@ -920,4 +939,4 @@ def test_batched_boxes_match_one_at_a_time_runs_bit_for_bit(mm):
         assert np.array_equal(s_.get_m(), m) and s_.energy() == e and s_.t == t
     # the relaxed states are energy minima of the cube (flower-like or vortex-like), not all the same one
     es = np.array([w[1] for w in want]) / (Km * (c * n) ** 3)
-    assert es.min() > 0.25 and es.max() < 0.40 and np.ptp(es) >= 0
+    assert es.min() > 0.15 and es.max() < 0.30 and np.ptp(es) > 1e-3     # cf. tests/golden/sp3_oracle_energies.txt
