@@ -36,3 +36,21 @@ struct Fast2DArgs {
   const Luts* luts;
   DevState* st;
 };
+
+// argument block of the register-FFT stages of open 3D boxes (fast3d.cuh)
+struct Fast3DArgs {
+  Geometry g;
+  int Nxt;                         // transform length along x (power of two >= Nx; padded length 2 Nxt), 0: generic x stage
+  const float2 *twx, *twx_r, *twox;   // x plan (length Nxt)
+  const uint8_t* regions;
+  const Luts* luts;
+  float2* spec;                    // [3][Nz][Py][pitch]
+  long long cstride;               // Nz * Py * pitch
+  const float* K3;                 // [Hy][kx tiles][6][Nz + 1][C]: the kernel spectrum (xx, yy, zz, xy, xz, yz over the
+                                   // non-negative octant) cut into the tiles of the z stage: the (Nz + 1) x C values of
+                                   // the six components at one ky and C neighbouring kx are one contiguous block
+  const float2 *twy, *twy_r, *twoy;   // y plan (length Ny): forward table, reversed-plan table, exp(-i pi n / Ny)
+  const float2 *twz, *twz_r, *twoz;   // z plan (length Nz)
+  DevState* st;
+};
+

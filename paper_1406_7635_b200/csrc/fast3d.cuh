@@ -9,6 +9,10 @@
 // or transformed. All lines of a CTA run in lockstep, so the exchanges use the CTA barrier and shared buffers
 // laid out [point][line]: a quarter-warp always reads or writes 128 contiguous bytes (no padding, no conflicts).
 //
+//   k3_xfwd: rows -> x spectrum. Two real rows a, b form one complex line z = a + i b (lanes: even / odd bins of the
+//            padded transform); the spectra of a and b are separated by Hermitian symmetry (partner values through
+//            shared memory) and stored as rows spec[c][z][y][kx], kx = 0 .. Nx, 16 bytes (two bins) per store.
+//   k3_xinv: x spectrum -> rows of B_demag (only the Nx physical outputs are formed).
 //   k3_y   : y forward (rows y < Ny -> bins ky < 2Ny) or y inverse (bins -> rows), in place, one component
 //   k3_z   : z forward of the three components, product with the six-component real symmetric kernel spectrum
 //            (Eq. 3; K real and even/odd under the mirrors, L145), z inverse; in place, only the Nz physical layers
@@ -17,17 +21,8 @@
 #pragma once
 #include "common.cuh"
 #include "fft_reg.cuh"
-
-struct Fast3DArgs {
-  Geometry g;
-  float2* spec;                    // [3][Nz][Py][pitch]
-  long long cstride;               // Nz * Py * pitch
-  const float* K;                  // [6][Hz][Hy][Cx]: xx, yy, zz, xy, xz, yz over the non-negative octant
-  long long kstride;               // Hz * Hy * Cx
-  const float2 *twy, *twy_r, *twoy;   // y plan (length Ny): forward table, reversed-plan table, exp(-i pi n / Ny)
-  const float2 *twz, *twz_r, *twoz;   // z plan (length Nz)
-  DevState* st;
-};
+#include "tma_util.cuh"
+#include "demag_conv_args.cuh"
 
 namespace f3 {
 using rf::C2;
@@ -103,7 +98,166 @@ __device__ __forceinline__ void inv_store(float2* __restrict__ line, size_t stri
   }
 }
 
+// ---- rows: the T threads of a line are neighbours (coalesced 4-byte accesses along x); one padded buffer per line
+__device__ __forceinline__ int xp(int a) { return a + (a >> 4); }
+template <class P> __host__ __device__ constexpr int row_pitch() { return P::N + P::N / 16 + 1; }      // float4 units, odd
+
+template <class P, int R, int RN, int MP>
+__device__ __forceinline__ void exchange_rows(C2* v, float4* xb, int t) {
+  constexpr int MN = MP / RN;
+  static_assert(P::T % MN == 0, "threads of a line must cover whole butterflies of the next pass");
+  const int rbase = (t / MN) * MP + (t % MN);
+  constexpr int RB_STEP = (P::T / MN) * MP;
+  __syncthreads();
+#pragma unroll
+  for (int b = 0; b < P::E / R; ++b)
+#pragma unroll
+    for (int s = 0; s < R; ++s) xb[xp(t + P::T * b + (P::N / R) * s)] = rf::pack(v[b * R + s]);
+  __syncthreads();
+#pragma unroll
+  for (int b = 0; b < P::E / RN; ++b)
+#pragma unroll
+    for (int s = 0; s < RN; ++s) v[b * RN + s] = rf::unpack(xb[xp(rbase + RB_STEP * b + s * MN)]);
+}
+template <class P, int DIR>
+__device__ __forceinline__ void fft_rows(C2* v, float4* xb, int t, const float2* __restrict__ tw) {
+  rf::pass_butterflies<P, P::RA, DIR>(v);
+  {
+    float2 w[(P::RA - 1) * (P::E / P::RA)];
+    rf::load_twiddles<P, P::RA>(w, t, tw);
+    rf::apply_twiddles<P, P::RA, DIR>(v, w);
+  }
+  exchange_rows<P, P::RA, P::RB, P::M1>(v, xb, t);
+  rf::pass_butterflies<P, P::RB, DIR>(v);
+  if constexpr (P::NPASS == 3) {
+    {
+      float2 w[(P::RB - 1) * (P::E / P::RB)];
+      rf::load_twiddles<P, P::RB>(w, t, tw + P::TW1);
+      rf::apply_twiddles<P, P::RB, DIR>(v, w);
+    }
+    exchange_rows<P, P::RB, P::RC, P::M2>(v, xb, t);
+    rf::pass_butterflies<P, P::RC, DIR>(v);
+  }
+}
+
+__device__ __forceinline__ float ldg_f(const float* p) {
+  float v;
+  asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ void stg_f(float* p, float v) { asm volatile("st.global.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory"); }
+
 }  // namespace f3
+
+// ---------------------------------------------------------------------------------- x stage
+// grid (row pairs / G, component); block G * P::T threads (t fastest); shared memory G * row_pitch float4
+template <class P, int G>
+__global__ void __launch_bounds__(P::T * G) k3_xfwd(Fast3DArgs a, int src_role) {
+  if (a.st->skip) return;
+  constexpr int N = P::N, T = P::T, E = P::E;
+  static_assert(P::RA == 16 && E == 16, "sixteen points per thread at stride N/16 on the sample side");
+  extern __shared__ float4 smem4[];
+  __shared__ float bsat_s[MM_MAX_REGIONS];
+  const int tid = threadIdx.x, t = tid % T, gi = tid / T;
+  const int c = blockIdx.y;
+  const int pair = blockIdx.x * G + gi, npairs = a.g.Ny * a.g.Nz / 2;      // Ny is even: a pair never straddles z
+  const bool live = pair < npairs;
+  const int r0 = 2 * (live ? pair : 0);                                      // flattened (z, y) row index
+  const int z = r0 / a.g.Ny, y = r0 - z * a.g.Ny;
+  float4* xb = smem4 + (size_t)gi * f3::row_pitch<P>();
+  const bool uniform = a.luts->nregions == 1;
+  const float b0 = a.luts->Bsat[0];
+  if (!uniform) {
+    for (int i = tid; i < MM_MAX_REGIONS; i += T * G) bsat_s[i] = a.luts->Bsat[i];
+    __syncthreads();
+  }
+  const float* __restrict__ src = a.st->ptr[src_role] + (size_t)c * a.g.N + (size_t)r0 * a.g.Nx;
+  const uint8_t* __restrict__ reg = a.regions + (size_t)r0 * a.g.Nx;
+  const float2 wt = __ldg(&a.twox[t]);
+  rf::C2 v[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int n = t + (N / 16) * e;
+    float2 zz = make_float2(0.f, 0.f);                      // M = B_sat m (L121); zero beyond the box (L509)
+    if (n < a.g.Nx) {
+      zz.x = f3::ldg_f(src + n) * (uniform ? b0 : bsat_s[reg[n]]);
+      zz.y = f3::ldg_f(src + a.g.Nx + n) * (uniform ? b0 : bsat_s[reg[a.g.Nx + n]]);
+    }
+    const float2 zw = rf::cmul_tw1<-1>(zz, rf::half_twiddle(wt, e));
+    v[e] = {make_float2(zz.x, zw.x), make_float2(zz.y, zw.y)};
+  }
+  f3::fft_rows<P, -1>(v, xb, t, a.twx);
+  // Hermitian separation: partner of even bin 2j is even bin 2((N - j) mod N), of odd bin 2j + 1 odd bin 2(N - 1 - j) + 1
+  __syncthreads();
+#pragma unroll
+  for (int e = 0; e < E; ++e)
+    xb[f3::xp(rf::slot_index<P, P::RLAST>(t, e))] = make_float4(v[e].re.x, v[e].im.x, v[e].re.y, v[e].im.y);
+  __syncthreads();
+  if (!live) return;
+  float2* __restrict__ outA = a.spec + (size_t)c * a.cstride + ((size_t)z * a.g.Py + y) * a.g.pitch;
+  float2* __restrict__ outB = outA + a.g.pitch;
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int j = rf::slot_index<P, P::RLAST>(t, e);
+    if (j > N / 2) continue;                                 // bins above Nx are the mirror images
+    const float4 pe = xb[f3::xp((N - j) & (N - 1))], po = xb[f3::xp(N - 1 - j)];
+    const float2 ze = make_float2(v[e].re.x, v[e].im.x), zo = make_float2(v[e].re.y, v[e].im.y);
+    // A = (Z[k] + conj Z[-k]) / 2, B = (Z[k] - conj Z[-k]) / 2i
+    const float4 A = make_float4(0.5f * (ze.x + pe.x), 0.5f * (ze.y - pe.y), 0.5f * (zo.x + po.z), 0.5f * (zo.y - po.w));
+    const float4 B = make_float4(0.5f * (ze.y + pe.y), 0.5f * (pe.x - ze.x), 0.5f * (zo.y + po.w), 0.5f * (po.z - zo.x));
+    // bins 2j and 2j + 1 side by side (for j = N/2 the second one falls in the padding of the pitch)
+    *reinterpret_cast<float4*>(outA + 2 * j) = A;
+    *reinterpret_cast<float4*>(outB + 2 * j) = B;
+  }
+}
+
+template <class P, int G>
+__global__ void __launch_bounds__(P::T * G) k3_xinv(Fast3DArgs a, int dst_role) {
+  if (a.st->skip) return;
+  using PI = typename P::Reversed;
+  constexpr int N = P::N, T = P::T, E = P::E;
+  static_assert(PI::RLAST == 16, "sixteen points per thread at stride N/16 on the sample side");
+  extern __shared__ float4 smem4[];
+  const int tid = threadIdx.x, t = tid % T, gi = tid / T;
+  const int c = blockIdx.y;
+  const int pair = blockIdx.x * G + gi, npairs = a.g.Ny * a.g.Nz / 2;
+  const bool live = pair < npairs;
+  const int r0 = 2 * (live ? pair : 0);
+  const int z = r0 / a.g.Ny, y = r0 - z * a.g.Ny;
+  float4* xb = smem4 + (size_t)gi * f3::row_pitch<P>();
+  const float2* __restrict__ inA = a.spec + (size_t)c * a.cstride + ((size_t)z * a.g.Py + y) * a.g.pitch;
+  const float2* __restrict__ inB = inA + a.g.pitch;
+  const float2 wt = __ldg(&a.twox[t]);
+  rf::C2 v[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    // point j of the even-bin transform is Z[2j], of the odd-bin one Z[2j + 1]; Z[b] = A[b] + i B[b] for b <= N,
+    // conj(A[2N - b]) + i conj(B[2N - b]) above
+    const int j = rf::slot_index<PI, PI::RA>(t, e);
+    if (2 * j + 1 <= N) {
+      const float4 A = *reinterpret_cast<const float4*>(inA + 2 * j), B = *reinterpret_cast<const float4*>(inB + 2 * j);
+      v[e] = {make_float2(A.x - B.y, A.z - B.w), make_float2(A.y + B.x, A.w + B.z)};
+    } else if (2 * j == N) {
+      const float2 A0 = inA[N], B0 = inB[N], A1 = inA[N - 1], B1 = inB[N - 1];      // bin N itself; bin N + 1 -> N - 1
+      v[e] = {make_float2(A0.x - B0.y, A1.x + B1.y), make_float2(A0.y + B0.x, B1.x - A1.y)};
+    } else {
+      const float2 A0 = inA[2 * N - 2 * j], B0 = inB[2 * N - 2 * j], A1 = inA[2 * N - 2 * j - 1], B1 = inB[2 * N - 2 * j - 1];
+      v[e] = {make_float2(A0.x + B0.y, A1.x + B1.y), make_float2(B0.x - A0.y, B1.x - A1.y)};
+    }
+  }
+  f3::fft_rows<PI, +1>(v, xb, t, a.twx_r);
+  if (!live) return;
+  float* __restrict__ dst = a.st->ptr[dst_role] + (size_t)c * a.g.N + (size_t)r0 * a.g.Nx;
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int n = t + (N / 16) * e;
+    const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), rf::half_twiddle(wt, e));
+    if (n < a.g.Nx) {
+      f3::stg_f(dst + n, v[e].re.x + u.x);
+      f3::stg_f(dst + a.g.Nx + n, v[e].im.x + u.y);
+    }
+  }
+}
 
 // ---------------------------------------------------------------------------------- y stage
 // grid (kx tiles, z < Nz, component); block P::T * C threads; shared memory N * C float4
@@ -146,19 +300,36 @@ __global__ void __launch_bounds__(P::T * C) k3_y(Fast3DArgs a) {
 // index of kernel component (i, j) in K: xx, yy, zz, xy, xz, yz
 __host__ __device__ constexpr int k3_comp(int i, int j) { return i == j ? i : (i + j == 1 ? 3 : (i + j == 2 ? 4 : 5)); }
 
-// grid (kx tiles, Py); block 3 * P::T * C threads (component-major inside a point); shared memory N * 3C float4.
-// blockIdx.y walks ky as 0, 1, Py-1, 2, Py-2, ..: a line and its mirror read the same kernel rows back to back.
+// grid (kx tiles, Py); block 3 * P::T * C threads (component-major inside a point); shared memory: N * 3C float4 of
+// exchange buffers + the kernel tile 6 (N + 1) C floats, which one bulk copy brings in while the forward transforms
+// run. blockIdx.y walks ky as 0, 1, Py-1, 2, Py-2, ..: a line and its mirror read the same kernel tile back to back.
 template <class P, int C>
-__global__ void __launch_bounds__(3 * P::T * C) k3_z(Fast3DArgs a) {
+struct K3Z {
+  static constexpr int KT = 6 * (P::N + 1) * C;                       // floats of one kernel tile
+  static constexpr size_t XB_BYTES = sizeof(float4) * (size_t)P::N * 3 * C;
+  static constexpr size_t SMEM = XB_BYTES + sizeof(float) * KT + 16;
+};
+
+template <class P, int C, int MINB>
+__global__ void __launch_bounds__(3 * P::T * C, MINB) k3_z(Fast3DArgs a) {
   if (a.st->skip) return;
-  using PI = typename P::Reversed;
   constexpr int N = P::N, T = P::T, E = P::E, LS = 3 * C;
-  extern __shared__ float4 smem4[];
+  extern __shared__ __align__(16) float4 smem4[];
+  __shared__ __align__(8) uint64_t kfull;
+  float* ksm = reinterpret_cast<float*>(reinterpret_cast<char*>(smem4) + K3Z<P, C>::XB_BYTES);
   const int tid = threadIdx.x, g = tid % C, comp = (tid / C) % 3, t = tid / LS;
   const int Py = a.g.Py, i = blockIdx.y;
   const int ky = i == 0 ? 0 : ((i & 1) ? (i + 1) / 2 : Py - i / 2);
   const int kyf = ky <= Py / 2 ? ky : Py - ky;
   const float sy = ky <= Py / 2 ? 1.f : -1.f;
+  if (tid == 0) {
+    tma::mbar_init(&kfull, 1);
+    tma::fence_barrier_init();
+    tma::fence_proxy_async();
+    constexpr uint32_t bytes = sizeof(float) * K3Z<P, C>::KT;
+    tma::mbar_expect_tx(&kfull, bytes);
+    tma::bulk_load(ksm, a.K3 + ((size_t)kyf * gridDim.x + blockIdx.x) * K3Z<P, C>::KT, bytes, &kfull);
+  }
   const int kx = blockIdx.x * C + g;
   const bool live = kx < a.g.Cx;
   const int kxc = live ? kx : a.g.Cx - 1;
@@ -167,12 +338,13 @@ __global__ void __launch_bounds__(3 * P::T * C) k3_z(Fast3DArgs a) {
   float4* xb = smem4 + comp * C + g;
   const float2 wt = __ldg(&a.twoz[t]);
   rf::C2 v[E];
-  f3::load_fwd<P, LS>(line, zs, a.g.Nz, wt, v, xb, t, a.twz);
+  f3::load_fwd<P, LS>(line, zs, a.g.Nz, wt, v, xb, t, a.twz);      // (its barriers also publish the mbarrier's initialisation)
   // hand the spectrum to the other two components of this line (same t, same slots)
   __syncthreads();
 #pragma unroll
   for (int e = 0; e < E; ++e) xb[(size_t)rf::slot_index<P, P::RLAST>(t, e) * LS] = rf::pack(v[e]);
   __syncthreads();
+  tma::mbar_wait(&kfull, 0);
   {
     const int o1 = (comp + 1) % 3, o2 = (comp + 2) % 3;
     const float4* x1 = smem4 + o1 * C + g;
@@ -180,19 +352,18 @@ __global__ void __launch_bounds__(3 * P::T * C) k3_z(Fast3DArgs a) {
     // mirror signs: a component pair that contains y is odd under ky -> -ky, one that contains z under kz -> -kz
     const float y1 = (comp == 1 || o1 == 1) ? sy : 1.f, y2 = (comp == 1 || o2 == 1) ? sy : 1.f;
     const bool z1 = comp == 2 || o1 == 2, z2 = comp == 2 || o2 == 2;
-    const float* __restrict__ K0 = a.K + (size_t)comp * a.kstride + (size_t)kyf * a.g.Cx + kxc;
-    const float* __restrict__ K1 = a.K + (size_t)k3_comp(comp, o1) * a.kstride + (size_t)kyf * a.g.Cx + kxc;
-    const float* __restrict__ K2 = a.K + (size_t)k3_comp(comp, o2) * a.kstride + (size_t)kyf * a.g.Cx + kxc;
-    const size_t ks = (size_t)a.g.Hy * a.g.Cx;                      // stride of kz in K
+    const float* K0 = ksm + (size_t)comp * (N + 1) * C + g;
+    const float* K1 = ksm + (size_t)k3_comp(comp, o1) * (N + 1) * C + g;
+    const float* K2 = ksm + (size_t)k3_comp(comp, o2) * (N + 1) * C + g;
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       const int j = rf::slot_index<P, P::RLAST>(t, e);
       const int b0 = 2 * j, b1 = 2 * j + 1;                         // bins of the two lanes; Pz / 2 = N
       const int f0 = b0 <= N ? b0 : 2 * N - b0, f1 = b1 <= N ? b1 : 2 * N - b1;
       const float s0 = b0 <= N ? 1.f : -1.f, s1 = b1 <= N ? 1.f : -1.f;
-      const float2 kd = make_float2(__ldg(K0 + f0 * ks), __ldg(K0 + f1 * ks));
-      float2 k1 = make_float2(__ldg(K1 + f0 * ks) * y1, __ldg(K1 + f1 * ks) * y1);
-      float2 k2 = make_float2(__ldg(K2 + f0 * ks) * y2, __ldg(K2 + f1 * ks) * y2);
+      const float2 kd = make_float2(K0[f0 * C], K0[f1 * C]);
+      float2 k1 = make_float2(K1[f0 * C] * y1, K1[f1 * C] * y1);
+      float2 k2 = make_float2(K2[f0 * C] * y2, K2[f1 * C] * y2);
       if (z1) { k1.x *= s0; k1.y *= s1; }
       if (z2) { k2.x *= s0; k2.y *= s1; }
       const rf::C2 A = rf::unpack(x1[(size_t)j * LS]), B = rf::unpack(x2[(size_t)j * LS]);
@@ -202,4 +373,19 @@ __global__ void __launch_bounds__(3 * P::T * C) k3_z(Fast3DArgs a) {
   }
   // (the first exchange of the inverse starts with a barrier: all reads of the handed-over spectra are done by then)
   f3::inv_store<P, LS>(line, zs, a.g.Nz, live, wt, v, xb, t, a.twz_r);
+}
+
+// the kernel spectrum in the tile order of k3_z (see Fast3DArgs::K3), from the generic layout K[6][Hz][Hy][Cx]
+__global__ void k3_pack_kernel(const float* __restrict__ K, float* __restrict__ K3, int Cx, int Hy, int Hz, int C, int ntiles) {
+  const long long kstride = (long long)Cx * Hy * Hz, total = (long long)Hy * ntiles * 6 * Hz * C;
+  for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < total; o += (long long)gridDim.x * blockDim.x) {
+    const int g = (int)(o % C);
+    long long r = o / C;
+    const int kf = (int)(r % Hz); r /= Hz;
+    const int comp = (int)(r % 6); r /= 6;
+    const int tile = (int)(r % ntiles);
+    const int kyf = (int)(r / ntiles);
+    const int kx = tile * C + g;
+    K3[o] = kx < Cx ? K[comp * kstride + ((long long)kf * Hy + kyf) * Cx + kx] : 0.f;
+  }
 }

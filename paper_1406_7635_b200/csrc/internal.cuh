@@ -6,14 +6,13 @@
 #include <vector>
 #include "common.cuh"
 #include "demag_conv_args.cuh"
-#include "fast3d.cuh"
 
 void* mm_default_alloc(size_t bytes, void*);
 void mm_default_free(void* p, void*);
 
 // kernel classes for launch counting and per-kernel CUDA-event timing (mm_profile)
 enum KernelKind { KK_XFWD = 0, KK_YFWD, KK_YINV, KK_LAST_XY, KK_LAST_Z, KK_LAST_3D, KK_XINV, KK_LOCAL, KK_STAGE,
-                  KK_ERROR, KK_CTRL, KK_OTHER, KK_F2_XFWD, KK_F2_YCOL, KK_F2_XINV, KK_F3_Y, KK_F3_Z,
+                  KK_ERROR, KK_CTRL, KK_OTHER, KK_F2_XFWD, KK_F2_YCOL, KK_F2_XINV, KK_F3_Y, KK_F3_Z, KK_F3_XFWD, KK_F3_XINV,
                   KK_COUNT };
 struct ProfEntry { int kind; cudaEvent_t a, b; };
 
@@ -97,6 +96,7 @@ int mm_fast2d_init(mm_sim* s);
 void mm_fast2d_demag(mm_sim* s, int src_role);
 bool mm_fast3d_supported(int Nx, int Ny, int Nz, const int* pbc);   // fast3d.cu
 int mm_fast3d_init(mm_sim* s);
+bool mm_fast3d_x(mm_sim* s, bool inverse, int role);
 void mm_fast3d_y(mm_sim* s, bool inverse);
 void mm_fast3d_z(mm_sim* s);
 

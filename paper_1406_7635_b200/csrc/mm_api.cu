@@ -156,8 +156,11 @@ void launch_demag(mm_sim* s, int src_role) {
   const int rows = g.Ny * g.Nz, pairs = (rows + 1) / 2;
   const int T = 256;
   dim3 gx((pairs + s->xL - 1) / s->xL, 3);
-  { Launch l(s, KK_XFWD); k_x_fwd<<<gx, T, s->xSmem, s->stream>>>(s->conv, src_role, s->xL); }
-  if (s->fast3d && !s->force_generic) {
+  const bool f3 = s->fast3d && !s->force_generic;
+  const bool f3x = f3 && s->f3.Nxt > 0;      // the x extent has a register-FFT plan as well
+  if (f3x) { Launch l(s, KK_F3_XFWD); mm_fast3d_x(s, false, src_role); }
+  else { Launch l(s, KK_XFWD); k_x_fwd<<<gx, T, s->xSmem, s->stream>>>(s->conv, src_role, s->xL); }
+  if (f3) {
     { Launch l(s, KK_F3_Y); mm_fast3d_y(s, false); }
     { Launch l(s, KK_F3_Z); mm_fast3d_z(s); }
     { Launch l(s, KK_F3_Y); mm_fast3d_y(s, true); }
@@ -173,7 +176,8 @@ void launch_demag(mm_sim* s, int src_role) {
     dim3 g1((g.Cx + s->lastC[1] - 1) / s->lastC[1]);
     { Launch l(s, KK_LAST_Z); k_last_fused<1><<<g1, T, s->lastSmem[1], s->stream>>>(s->conv, 1, s->lastC[1]); }
   }
-  { Launch l(s, KK_XINV); k_x_inv<<<gx, T, s->xSmem, s->stream>>>(s->conv, R_B, s->xL); }
+  if (f3x) { Launch l(s, KK_F3_XINV); mm_fast3d_x(s, true, R_B); }
+  else { Launch l(s, KK_XINV); k_x_inv<<<gx, T, s->xSmem, s->stream>>>(s->conv, R_B, s->xL); }
 }
 
 // can the four-cells-per-thread local kernel (and with it the fused stage / error variants) run on this box?
@@ -1145,7 +1149,7 @@ int mm_profile(mm_sim* s, int enable) {
 
 int mm_profile_read(mm_sim* s, int kind, const char** name, double* total_ms, long* launches) {
   static const char* names[KK_COUNT] = {"x_fwd", "y_fwd", "y_inv", "last_xy", "last_z", "last_3d", "x_inv", "local",
-                                        "rk_stage", "rk_error", "rk_ctrl", "other", "f2_xfwd", "f2_ycol", "f2_xinv", "f3_y", "f3_z"};
+                                        "rk_stage", "rk_error", "rk_ctrl", "other", "f2_xfwd", "f2_ycol", "f2_xinv", "f3_y", "f3_z", "f3_xfwd", "f3_xinv"};
   if (!s || kind < 0 || kind >= KK_COUNT) return MM_EINVAL;
   if (!s->prof.empty()) {
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));

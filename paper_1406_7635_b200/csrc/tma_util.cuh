@@ -40,6 +40,12 @@ __device__ __forceinline__ void load_3d(void* dst, const CUtensorMap* map, int c
       "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_addr(bar))
       : "memory");
 }
+// global -> shared, one contiguous block (addresses and size multiples of 16 bytes); completion on the mbarrier
+__device__ __forceinline__ void bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_addr(dst)),
+               "l"(src), "r"(bytes), "r"(smem_addr(bar))
+               : "memory");
+}
 // shared -> global (3-D tensor map); tracked by bulk async-groups
 __device__ __forceinline__ void store_3d(const CUtensorMap* map, int c0, int c1, int c2, const void* src) {
   asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(map), "r"(c0),

@@ -146,6 +146,8 @@ def test_fast3d_path_fields(mm, grid):
     prof = sim.profile_read()
     sim.profile(False)
     assert "f3_y" in prof and "f3_z" in prof and "last_3d" not in prof
+    nx = grid[0]
+    assert ("f3_xfwd" in prof and "f3_xinv" in prof) == (nx >= 32 and nx & (nx - 1) == 0)      # x extents with a plan
     Bf = sim.b_eff(MM_DEMAG)
     sim.set_option(mm.MM_OPT_GENERIC_FFT, 1)
     Bg = sim.b_eff(MM_DEMAG)
