@@ -40,7 +40,7 @@ struct Fast2DArgs {
 // argument block of the register-FFT stages of open 3D boxes (fast3d.cuh)
 struct Fast3DArgs {
   Geometry g;
-  int Nxt;                         // transform length along x (power of two >= Nx; padded length 2 Nxt), 0: generic x stage
+  int mode[3];                     // per axis: 0 generic kernels, 1 open axis (padded x2, pruned), 2 periodic axis
   const float2 *twx, *twx_r, *twox;   // x plan (length Nxt)
   const uint8_t* regions;
   const Luts* luts;

@@ -28,6 +28,8 @@ int attrs_y(mm_sim* s) {
   using P = typename Plan3<N>::P;
   CUDA_TRY(s, cudaFuncSetAttribute(k3_y<P, cy<N>(), false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_y<N>()));
   CUDA_TRY(s, cudaFuncSetAttribute(k3_y<P, cy<N>(), true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_y<N>()));
+  CUDA_TRY(s, cudaFuncSetAttribute(k3_yp<P, cy<N>(), false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_y<N>()));
+  CUDA_TRY(s, cudaFuncSetAttribute(k3_yp<P, cy<N>(), true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_y<N>()));
   return MM_OK;
 }
 template <int N>
@@ -51,6 +53,12 @@ template <int N>
 void launch_y(mm_sim* s, bool inverse) {
   using P = typename Plan3<N>::P;
   constexpr int C = cy<N>();
+  if (s->f3.mode[1] == 2) {                                   // periodic: two neighbouring columns per line group
+    const dim3 grid(((s->g.Cx + 1) / 2 + C - 1) / C, s->g.Nz, 3);
+    if (inverse) k3_yp<P, C, true><<<grid, P::T * C, smem_y<N>(), s->stream>>>(s->f3);
+    else k3_yp<P, C, false><<<grid, P::T * C, smem_y<N>(), s->stream>>>(s->f3);
+    return;
+  }
   const dim3 grid((s->g.Cx + C - 1) / C, s->g.Nz, 3);
   if (inverse) k3_y<P, C, true><<<grid, P::T * C, smem_y<N>(), s->stream>>>(s->f3);
   else k3_y<P, C, false><<<grid, P::T * C, smem_y<N>(), s->stream>>>(s->f3);
@@ -70,16 +78,24 @@ int attrs_x(mm_sim* s) {
   using P = typename Plan3<N>::P;
   CUDA_TRY(s, cudaFuncSetAttribute(k3_xfwd<P, gx<N>()>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_x<N>()));
   CUDA_TRY(s, cudaFuncSetAttribute(k3_xinv<P, gx<N>()>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_x<N>()));
+  CUDA_TRY(s, cudaFuncSetAttribute(k3_xfwd_p<P, gx<N>()>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_x<N>()));
+  CUDA_TRY(s, cudaFuncSetAttribute(k3_xinv_p<P, gx<N>()>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_x<N>()));
   return MM_OK;
 }
 template <int N>
 void launch_x(mm_sim* s, bool inverse, int role) {
   using P = typename Plan3<N>::P;
   constexpr int G = gx<N>();
-  const int npairs = s->g.Ny * s->g.Nz / 2;
-  const dim3 grid((npairs + G - 1) / G, 3);
-  if (inverse) k3_xinv<P, G><<<grid, P::T * G, smem_x<N>(), s->stream>>>(s->f3, role);
-  else k3_xfwd<P, G><<<grid, P::T * G, smem_x<N>(), s->stream>>>(s->f3, role);
+  const bool periodic = s->f3.mode[0] == 2;
+  const int nlines = s->g.Ny * s->g.Nz / (periodic ? 4 : 2);      // row pairs, or row quadruples on a periodic axis
+  const dim3 grid((nlines + G - 1) / G, 3);
+  if (periodic) {
+    if (inverse) k3_xinv_p<P, G><<<grid, P::T * G, smem_x<N>(), s->stream>>>(s->f3, role);
+    else k3_xfwd_p<P, G><<<grid, P::T * G, smem_x<N>(), s->stream>>>(s->f3, role);
+  } else {
+    if (inverse) k3_xinv<P, G><<<grid, P::T * G, smem_x<N>(), s->stream>>>(s->f3, role);
+    else k3_xfwd<P, G><<<grid, P::T * G, smem_x<N>(), s->stream>>>(s->f3, role);
+  }
 }
 
 bool pow2_in_range(int n) { return n >= 32 && n <= 512 && (n & (n - 1)) == 0; }
@@ -95,58 +111,70 @@ bool pow2_in_range(int n) { return n >= 32 && n <= 512 && (n & (n - 1)) == 0; }
     case 512: { CALL(512); break; }     \
   }
 
-// open boxes whose y and z extents are powers of two from 32 to 512 cells (the padded length of such an axis is
-// exactly twice its extent); the x stage stays with the generic kernels
-bool mm_fast3d_supported(int Nx, int Ny, int Nz, const int* pbc) {
-  (void)Nx;
-  return !pbc[0] && !pbc[1] && !pbc[2] && pow2_in_range(Ny) && pow2_in_range(Nz);
+// Which stages of a 3D box run on the register engine: an axis qualifies if its extent is a power of two from 32 to
+// 512 cells and it is either open (its padded length is then exactly twice the extent) or periodic (not padded;
+// x and y only - the rows of a periodic x axis are taken four at a time). The other stages keep the generic kernels;
+// all of them share the layout spec[c][z][ky][kx].
+void mm_fast3d_modes(const Geometry& g, int* mode) {
+  const int N[3] = {g.Nx, g.Ny, g.Nz}, P[3] = {g.Px, g.Py, g.Pz};
+  for (int a = 0; a < 3; ++a) {
+    mode[a] = 0;
+    if (!pow2_in_range(N[a])) continue;
+    if (!g.pbc[a] && P[a] == 2 * N[a]) mode[a] = 1;
+    else if (g.pbc[a] && P[a] == N[a] && a < 2) mode[a] = 2;
+  }
+  if (mode[0] == 2 && g.Ny % 4 != 0) mode[0] = 0;
+  if (g.Ny % 2 != 0) mode[0] = 0;
+  if (g.Nz == 1) mode[0] = mode[1] = mode[2] = 0;           // one-layer films: fast2d.cu or the generic kernels
 }
 
 int mm_fast3d_init(mm_sim* s) {
   const Geometry& g = s->g;
-  if (g.Py != 2 * g.Ny || g.Pz != 2 * g.Nz) { s->fast3d = false; return MM_OK; }
   Fast3DArgs& a = s->f3;
   a.g = g;
+  mm_fast3d_modes(g, a.mode);
   a.spec = s->spec;
   a.cstride = (long long)g.Nz * g.Py * g.pitch;
   a.st = s->dstate;
   a.regions = s->regions; a.luts = s->luts;
-  a.Nxt = (pow2_in_range(g.Nx) && g.Px == 2 * g.Nx) ? g.Nx : 0;
   float2 *f, *r, *h;
   int rc = MM_OK;
 #define TY(N) rc = mm_plan_tables<Plan3<N>::P>(s, &f, &r, &h)
-  if (a.Nxt) {
-    F3_SWITCH(a.Nxt, TY)
-    if (rc) return rc;
-    a.twx = f; a.twx_r = r; a.twox = h;
 #define AX(N) rc = attrs_x<N>(s)
-    F3_SWITCH(a.Nxt, AX)
-#undef AX
-    if (rc) return rc;
-  }
-  F3_SWITCH(g.Ny, TY)
-  if (rc) return rc;
-  a.twy = f; a.twy_r = r; a.twoy = h;
-  F3_SWITCH(g.Nz, TY)
-  if (rc) return rc;
-  a.twz = f; a.twz_r = r; a.twoz = h;
-#undef TY
 #define AY(N) rc = attrs_y<N>(s)
 #define AZ(N) rc = attrs_z<N>(s)
-  F3_SWITCH(g.Ny, AY)
-  if (rc) return rc;
-  F3_SWITCH(g.Nz, AZ)
+  if (a.mode[0]) {
+    F3_SWITCH(g.Nx, TY)
+    if (rc) return rc;
+    a.twx = f; a.twx_r = r; a.twox = h;
+    F3_SWITCH(g.Nx, AX)
+    if (rc) return rc;
+  }
+  if (a.mode[1]) {
+    F3_SWITCH(g.Ny, TY)
+    if (rc) return rc;
+    a.twy = f; a.twy_r = r; a.twoy = h;
+    F3_SWITCH(g.Ny, AY)
+    if (rc) return rc;
+  }
+  if (a.mode[2]) {
+    F3_SWITCH(g.Nz, TY)
+    if (rc) return rc;
+    a.twz = f; a.twz_r = r; a.twoz = h;
+    F3_SWITCH(g.Nz, AZ)
+    if (rc) return rc;
+  }
+#undef TY
+#undef AX
 #undef AY
 #undef AZ
-  return rc;
+  return MM_OK;
 }
 
-bool mm_fast3d_x(mm_sim* s, bool inverse, int role) {      // false: this box keeps the generic x stage
-  if (!s->f3.Nxt) return false;
+void mm_fast3d_x(mm_sim* s, bool inverse, int role) {
 #define LX(N) launch_x<N>(s, inverse, role)
-  F3_SWITCH(s->f3.Nxt, LX)
+  F3_SWITCH(s->g.Nx, LX)
 #undef LX
-  return true;
 }
 void mm_fast3d_y(mm_sim* s, bool inverse) {
 #define LY(N) launch_y<N>(s, inverse)

@@ -22,6 +22,7 @@
 #include "common.cuh"
 #include "fft_reg.cuh"
 #include "tma_util.cuh"
+#include <type_traits>
 #include "demag_conv_args.cuh"
 
 namespace f3 {
@@ -293,6 +294,131 @@ __global__ void __launch_bounds__(P::T * C) k3_y(Fast3DArgs a) {
       v[e] = {make_float2(lo.x, hi.x), make_float2(lo.y, hi.y)};
     }
     f3::inv_store<P, C>(line, ps, a.g.Ny, live, wt, v, xb, t, a.twy_r);
+  }
+}
+
+// ---------------------------------------------------------------------------------- periodic axes
+// A periodic axis is not padded (the images are folded into the kernel): a plain N-point
+// transform per line. The two lanes of the packed engine then carry two different lines.
+//
+// y stage, periodic: lanes = the lines at kx and kx + 1 (one 16-byte access per point). grid (kx pair tiles, z, c)
+template <class P, int C, bool INV>
+__global__ void __launch_bounds__(P::T * C) k3_yp(Fast3DArgs a) {
+  if (a.st->skip) return;
+  using PL = typename std::conditional<INV, typename P::Reversed, P>::type;
+  constexpr int T = P::T, E = P::E;
+  extern __shared__ float4 smem4[];
+  const int tid = threadIdx.x, g = tid % C, t = tid / C;
+  const int kx = 2 * (blockIdx.x * C + g);
+  const bool live = kx < a.g.Cx;                          // (kx + 1 may be a padding column of the pitch: harmless)
+  const size_t ps = (size_t)a.g.pitch;
+  float2* __restrict__ line = a.spec + (size_t)blockIdx.z * a.cstride + (size_t)blockIdx.y * a.g.Py * ps + (live ? kx : 0);
+  rf::C2 v[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const float4 q = *reinterpret_cast<const float4*>(line + (size_t)rf::slot_index<PL, PL::RA>(t, e) * ps);
+    v[e] = {make_float2(q.x, q.z), make_float2(q.y, q.w)};
+  }
+  f3::fft<PL, INV ? +1 : -1, C>(v, smem4 + g, t, INV ? a.twy_r : a.twy);
+  if (live) {
+#pragma unroll
+    for (int e = 0; e < E; ++e)
+      *reinterpret_cast<float4*>(line + (size_t)rf::slot_index<PL, PL::RLAST>(t, e) * ps) =
+          make_float4(v[e].re.x, v[e].im.x, v[e].re.y, v[e].im.y);
+  }
+}
+
+// x stage, periodic: four real rows per line group - lanes = the complex lines (r, r+1) and (r+2, r+3); N-point
+// transform, Hermitian separation (partner of bin j is bin (N - j) mod N), bins 0 .. N/2 stored.
+template <class P, int G>
+__global__ void __launch_bounds__(P::T * G) k3_xfwd_p(Fast3DArgs a, int src_role) {
+  if (a.st->skip) return;
+  constexpr int N = P::N, T = P::T, E = P::E;
+  extern __shared__ float4 smem4[];
+  __shared__ float bsat_s[MM_MAX_REGIONS];
+  const int tid = threadIdx.x, t = tid % T, gi = tid / T;
+  const int c = blockIdx.y;
+  const int quad = blockIdx.x * G + gi, nquads = a.g.Ny * a.g.Nz / 4;       // Ny is a multiple of 4
+  const bool live = quad < nquads;
+  const int r0 = 4 * (live ? quad : 0);
+  const int z = r0 / a.g.Ny, y = r0 - z * a.g.Ny;
+  float4* xb = smem4 + (size_t)gi * f3::row_pitch<P>();
+  const bool uniform = a.luts->nregions == 1;
+  const float b0 = a.luts->Bsat[0];
+  if (!uniform) {
+    for (int i = tid; i < MM_MAX_REGIONS; i += T * G) bsat_s[i] = a.luts->Bsat[i];
+    __syncthreads();
+  }
+  const int nx = a.g.Nx;
+  const float* __restrict__ src = a.st->ptr[src_role] + (size_t)c * a.g.N + (size_t)r0 * nx;
+  const uint8_t* __restrict__ reg = a.regions + (size_t)r0 * nx;
+  rf::C2 v[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int n = rf::slot_index<P, P::RA>(t, e);
+    float q[4];
+#pragma unroll
+    for (int r = 0; r < 4; ++r) q[r] = f3::ldg_f(src + (size_t)r * nx + n) * (uniform ? b0 : bsat_s[reg[(size_t)r * nx + n]]);
+    v[e] = {make_float2(q[0], q[2]), make_float2(q[1], q[3])};
+  }
+  f3::fft_rows<P, -1>(v, xb, t, a.twx);
+  __syncthreads();
+#pragma unroll
+  for (int e = 0; e < E; ++e)
+    xb[f3::xp(rf::slot_index<P, P::RLAST>(t, e))] = make_float4(v[e].re.x, v[e].im.x, v[e].re.y, v[e].im.y);
+  __syncthreads();
+  if (!live) return;
+  float2* __restrict__ out = a.spec + (size_t)c * a.cstride + ((size_t)z * a.g.Py + y) * a.g.pitch;
+  const size_t ps = (size_t)a.g.pitch;
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int j = rf::slot_index<P, P::RLAST>(t, e);
+    if (j > N / 2) continue;
+    const float4 p = xb[f3::xp((N - j) & (N - 1))];
+    const float2 z0 = make_float2(v[e].re.x, v[e].im.x), z1 = make_float2(v[e].re.y, v[e].im.y);
+    out[j] = make_float2(0.5f * (z0.x + p.x), 0.5f * (z0.y - p.y));
+    out[ps + j] = make_float2(0.5f * (z0.y + p.y), 0.5f * (p.x - z0.x));
+    out[2 * ps + j] = make_float2(0.5f * (z1.x + p.z), 0.5f * (z1.y - p.w));
+    out[3 * ps + j] = make_float2(0.5f * (z1.y + p.w), 0.5f * (p.z - z1.x));
+  }
+}
+
+template <class P, int G>
+__global__ void __launch_bounds__(P::T * G) k3_xinv_p(Fast3DArgs a, int dst_role) {
+  if (a.st->skip) return;
+  using PI = typename P::Reversed;
+  constexpr int N = P::N, T = P::T, E = P::E;
+  extern __shared__ float4 smem4[];
+  const int tid = threadIdx.x, t = tid % T, gi = tid / T;
+  const int c = blockIdx.y;
+  const int quad = blockIdx.x * G + gi, nquads = a.g.Ny * a.g.Nz / 4;
+  const bool live = quad < nquads;
+  const int r0 = 4 * (live ? quad : 0);
+  const int z = r0 / a.g.Ny, y = r0 - z * a.g.Ny;
+  float4* xb = smem4 + (size_t)gi * f3::row_pitch<P>();
+  const float2* __restrict__ in = a.spec + (size_t)c * a.cstride + ((size_t)z * a.g.Py + y) * a.g.pitch;
+  const size_t ps = (size_t)a.g.pitch;
+  rf::C2 v[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int j = rf::slot_index<PI, PI::RA>(t, e);
+    const bool dir = j <= N / 2;                            // Z[j] = A[j] + i B[j]; above N/2: conj(A[N-j]) + i conj(B[N-j])
+    const int k = dir ? j : N - j;
+    const float2 A0 = in[k], B0 = in[ps + k], A1 = in[2 * ps + k], B1 = in[3 * ps + k];
+    if (dir) v[e] = {make_float2(A0.x - B0.y, A1.x - B1.y), make_float2(A0.y + B0.x, A1.y + B1.x)};
+    else v[e] = {make_float2(A0.x + B0.y, A1.x + B1.y), make_float2(B0.x - A0.y, B1.x - A1.y)};
+  }
+  f3::fft_rows<PI, +1>(v, xb, t, a.twx_r);
+  if (!live) return;
+  const int nx = a.g.Nx;
+  float* __restrict__ dst = a.st->ptr[dst_role] + (size_t)c * a.g.N + (size_t)r0 * nx;
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const int n = rf::slot_index<PI, PI::RLAST>(t, e);
+    f3::stg_f(dst + n, v[e].re.x);
+    f3::stg_f(dst + nx + n, v[e].im.x);
+    f3::stg_f(dst + 2 * (size_t)nx + n, v[e].re.y);
+    f3::stg_f(dst + 3 * (size_t)nx + n, v[e].im.y);
   }
 }
 

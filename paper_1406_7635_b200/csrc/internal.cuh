@@ -50,7 +50,7 @@ struct mm_sim {
   bool f2_tma = false;         // tensor maps valid: the x kernels move their transposed pieces with TMA
   bool fast2d = false;         // fast 2D path available for this box
   Fast3DArgs f3;
-  bool fast3d = false;         // register-FFT y and z stages available for this box (fast3d.cu)
+  bool fast3d = false;         // some stage of this 3D box runs on the register engine (fast3d.cu, f3.mode)
   bool force_generic = false;  // mm_set_option(MM_OPT_GENERIC_FFT)
   // host state
   DevState hst;
@@ -94,9 +94,9 @@ bool mm_fast2d_supported(int Nx, int Ny, int Nz, const int* pbc);   // fast2d.cu
 int mm_fast2d_length(int N);      // transform length of the fast path for N physical cells (power of two)
 int mm_fast2d_init(mm_sim* s);
 void mm_fast2d_demag(mm_sim* s, int src_role);
-bool mm_fast3d_supported(int Nx, int Ny, int Nz, const int* pbc);   // fast3d.cu
+void mm_fast3d_modes(const Geometry& g, int* mode);   // fast3d.cu: per axis 0 generic, 1 open, 2 periodic
 int mm_fast3d_init(mm_sim* s);
-bool mm_fast3d_x(mm_sim* s, bool inverse, int role);
+void mm_fast3d_x(mm_sim* s, bool inverse, int role);
 void mm_fast3d_y(mm_sim* s, bool inverse);
 void mm_fast3d_z(mm_sim* s);
 

@@ -157,19 +157,18 @@ void launch_demag(mm_sim* s, int src_role) {
   const int T = 256;
   dim3 gx((pairs + s->xL - 1) / s->xL, 3);
   const bool f3 = s->fast3d && !s->force_generic;
-  const bool f3x = f3 && s->f3.Nxt > 0;      // the x extent has a register-FFT plan as well
+  const bool f3x = f3 && s->f3.mode[0], f3y = f3 && s->f3.mode[1], f3z = f3 && s->f3.mode[2];      // stage by stage
   if (f3x) { Launch l(s, KK_F3_XFWD); mm_fast3d_x(s, false, src_role); }
   else { Launch l(s, KK_XFWD); k_x_fwd<<<gx, T, s->xSmem, s->stream>>>(s->conv, src_role, s->xL); }
-  if (f3) {
-    { Launch l(s, KK_F3_Y); mm_fast3d_y(s, false); }
-    { Launch l(s, KK_F3_Z); mm_fast3d_z(s); }
-    { Launch l(s, KK_F3_Y); mm_fast3d_y(s, true); }
-  } else if (s->last_along_z) {
+  if (s->last_along_z) {
     dim3 gy((g.Cx + s->yC - 1) / s->yC, g.Nz, 3);
-    if (g.Py > 1) { Launch l(s, KK_YFWD); k_y_axis<<<gy, T, s->ySmem, s->stream>>>(s->conv, 0, s->yC); }
+    if (f3y) { Launch l(s, KK_F3_Y); mm_fast3d_y(s, false); }
+    else if (g.Py > 1) { Launch l(s, KK_YFWD); k_y_axis<<<gy, T, s->ySmem, s->stream>>>(s->conv, 0, s->yC); }
     dim3 gl((g.Cx + s->lastC[2] - 1) / s->lastC[2], g.Py);
-    { Launch l(s, KK_LAST_3D); k_last_fused<3><<<gl, T, s->lastSmem[2], s->stream>>>(s->conv, 2, s->lastC[2]); }
-    if (g.Py > 1) { Launch l(s, KK_YINV); k_y_axis<<<gy, T, s->ySmem, s->stream>>>(s->conv, 1, s->yC); }
+    if (f3z) { Launch l(s, KK_F3_Z); mm_fast3d_z(s); }
+    else { Launch l(s, KK_LAST_3D); k_last_fused<3><<<gl, T, s->lastSmem[2], s->stream>>>(s->conv, 2, s->lastC[2]); }
+    if (f3y) { Launch l(s, KK_F3_Y); mm_fast3d_y(s, true); }
+    else if (g.Py > 1) { Launch l(s, KK_YINV); k_y_axis<<<gy, T, s->ySmem, s->stream>>>(s->conv, 1, s->yC); }
   } else {
     dim3 g0((g.Cx + s->lastC[0] - 1) / s->lastC[0]);
     { Launch l(s, KK_LAST_XY); k_last_fused<2><<<g0, T, s->lastSmem[0], s->stream>>>(s->conv, 0, s->lastC[0]); }
@@ -460,7 +459,11 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
   if (g.Px > kMaxFft || g.Py > kMaxFft || g.Pz > kMaxFft) return bail(MM_EINVAL, "padded FFT length above 8192");
   if (!smooth5(g.Px) || !smooth5(g.Py) || !smooth5(g.Pz)) return bail(MM_EINVAL, "periodic axis length must be 2^a 3^b 5^c");
   g.Cx = g.Px / 2 + 1;
-  s->fast3d = !s->fast2d && Nz > 1 && mm_fast3d_supported(Nx, Ny, Nz, s->rep) && g.Py == 2 * Ny && g.Pz == 2 * Nz;
+  {
+    int mode[3];
+    mm_fast3d_modes(g, mode);
+    s->fast3d = !s->fast2d && (mode[0] || mode[1] || mode[2]);
+  }
   // rows of the spectrum start on 128-byte lines when the strided stages read pieces of neighbouring kx
   g.pitch = s->fast3d ? (g.Cx + 15) / 16 * 16 : g.Cx;
   g.Hy = g.Py / 2 + 1; g.Hz = g.Pz / 2 + 1;

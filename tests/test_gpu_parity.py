@@ -154,6 +154,30 @@ def test_fast3d_path_fields(mm, grid):
     assert np.abs(Bf - Bg).max() <= 2e-5 * np.abs(Bg).max()
 
 
+@pytest.mark.parametrize("grid,pbc,kinds", [
+    ((64, 64, 32), (2, 2, 0), ("f3_xfwd", "f3_y", "f3_z", "f3_xinv")),          # periodic x and y, open z (C5 with PBC)
+    ((32, 128, 64), (0, 3, 0), ("f3_xfwd", "f3_y", "f3_z")),                    # open x, periodic y
+    ((128, 36, 32), (2, 0, 0), ("f3_xfwd", "y_fwd", "f3_z")),                   # periodic x, generic y (36 rows)
+    ((40, 48, 64), (0, 0, 0), ("x_fwd", "y_fwd", "f3_z")),                      # only z has a plan
+    ((64, 32, 20), (0, 2, 0), ("f3_xfwd", "f3_y", "last_3d")),                  # generic z between fast stages
+    ((256, 32, 32), (1, 0, 2), ("f3_xfwd", "f3_y", "last_3d"))])                # periodic z stays generic
+def test_fast3d_mixed_stages(mm, grid, pbc, kinds):
+    # every stage of a 3D box picks the register engine or the generic kernels on its own (open or periodic axis,
+    # extent with or without a plan); all combinations share one spectrum layout and must agree with the oracle
+    cfg = _rand_cfg(grid, (3e-9, 2e-9, 2.5e-9), pbc=pbc, nreg=3, anis=True, seed=35)
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    sim.profile(True)
+    _field_check(sim, ref, (MM_DEMAG, MM_ALL))
+    prof = sim.profile_read()
+    sim.profile(False)
+    assert all(k in prof for k in kinds), (kinds, sorted(prof))
+    Bf = sim.b_eff(MM_DEMAG)
+    sim.set_option(mm.MM_OPT_GENERIC_FFT, 1)
+    Bg = sim.b_eff(MM_DEMAG)
+    assert np.abs(Bf - Bg).max() <= 2e-5 * np.abs(Bg).max()
+
+
 def test_fast2d_one_region_and_steps(mm):
     # one region (the bench workload's shape): B_sat is a constant and the region gathers are skipped
     cfg = config_c4(512)
