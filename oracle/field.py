@@ -260,8 +260,9 @@ def zhang_li_torque_over_gamma(m, Msat_cell, alpha_cell, j, xi, cell, pbc, gamma
        tau_ZL = 1/(1+alpha^2) [ (1 + xi alpha) m x (m x (u.grad) m) + (xi - alpha) m x (u.grad) m ],
        u = mu_B mu0 / (2 e gamma_LL Bsat (1 + xi^2)) j      [T m].
     PAPER.md prints the two terms identically (garbled); the double cross product in the first term is the
-    reading of DESIGN.md #19. (u.grad) m by central differences; a missing neighbour at an open boundary is
-    replaced by the cell's own m (as for the exchange stencil, L196); periodic axes wrap."""
+    reading of DESIGN.md #19. (u.grad) m by central differences; a missing neighbour - beyond an open boundary, or
+    a vacuum cell (Msat = 0), which is how a shape inside the box ends (L53) - is replaced by the cell's own m
+    (as for the exchange stencil, L196); periodic axes wrap."""
     j = np.asarray(j, dtype=float)
     D = np.zeros_like(m)
     with np.errstate(divide="ignore", invalid="ignore"):
@@ -278,6 +279,15 @@ def zhang_li_torque_over_gamma(m, Msat_cell, alpha_cell, j, xi, cell, pbc, gamma
             sl_hi[ax] = slice(1, None); sl_lo[ax] = slice(None, -1)
             up[tuple(sl_lo)] = m[tuple(sl_hi)]        # neighbour at +1 (the last cell keeps its own m)
             dn[tuple(sl_hi)] = m[tuple(sl_lo)]        # neighbour at -1 (the first cell keeps its own m)
+        # the same shifts of Msat tell which neighbours are vacuum
+        if per:
+            ms_up, ms_dn = np.roll(Msat_cell, -1, axis=ax - 1), np.roll(Msat_cell, 1, axis=ax - 1)
+        else:
+            ms_up, ms_dn = Msat_cell.copy(), Msat_cell.copy()
+            ms_up[tuple(sl_lo[1:])] = Msat_cell[tuple(sl_hi[1:])]
+            ms_dn[tuple(sl_hi[1:])] = Msat_cell[tuple(sl_lo[1:])]
+        up = np.where(ms_up[None] > 0, up, m)
+        dn = np.where(ms_dn[None] > 0, dn, m)
         D += (pref * ja)[None] * (up - dn) / (2.0 * d)
     a = alpha_cell[None]
     mxD = cross(m, D)

@@ -463,6 +463,28 @@ def test_zhang_li_torque_advects_a_spiral():
     assert np.allclose(t2[:, 0, 0, 0], want0, rtol=1e-10, atol=1e-18)
 
 
+def test_zhang_li_next_to_vacuum_is_an_open_end():
+    # A shape inside the box ends where Msat = 0 (L53): for the current-driven gradient (u . grad) m a vacuum
+    # neighbour must count as a missing neighbour, exactly like the end of the box (L196). Pin: a chain whose right
+    # half is vacuum carries, cell by cell, the torque of the chain that simply ends there; and a vacuum cell in the
+    # middle of a uniform spiral does not act as a neighbour with m = 0 (which would give a gradient of m / 2 dx).
+    n, dx, Ms, alpha, j = 12, 4e-9, 8e5, 0.1, 2e12
+    k = 2 * np.pi / (20 * dx)
+    x = np.arange(n) * dx
+    m0 = np.zeros((3, 1, 1, n)); m0[0, 0, 0] = np.cos(k * x); m0[1, 0, 0] = np.sin(k * x)
+    regions = np.zeros((1, 1, n), dtype=np.uint8); regions[..., n // 2:] = 1
+    p2 = Params.uniform(2, Msat=[Ms, 0.0], Aex=0.0, alpha=alpha)
+    full = RefSim((n, 1, 1), (dx, dx, dx)); full.set_params(p2); full.set_regions(regions); full.set_terms(MM_ZEEMAN)
+    full.set_m(m0); full.set_zhang_li((j, 0, 0), xi=0.3)
+    half = RefSim((n // 2, 1, 1), (dx, dx, dx)); half.set_params(Params.uniform(1, Msat=Ms, Aex=0.0, alpha=alpha))
+    half.set_terms(MM_ZEEMAN); half.set_m(m0[..., :n // 2].copy()); half.set_zhang_li((j, 0, 0), xi=0.3)
+    tf, th = full.torque(full.m), half.torque(half.m)
+    assert np.abs(th).max() > 0 and np.array_equal(tf[..., :n // 2], th) and np.all(tf[..., n // 2:] == 0)
+    # the wrong rule (vacuum neighbour read as m = 0) would make the interface torque about 1 / (k dx) times larger
+    inner = np.abs(tf[:, 0, 0, 2]).max()
+    assert np.abs(tf[:, 0, 0, n // 2 - 1]).max() < 1.01 * inner
+
+
 # ------------------------------------------------------------------ pins added in round 2 ("What's weak" #1)
 def test_energy_conserved_without_damping_on_a_3d_box_with_unequal_cell_edges():
     # alpha = 0: the torque is gamma m x B_eff with B_eff = -dE/dM, so E is a constant of the motion - but only
