@@ -102,6 +102,16 @@ int mm_destroy(mm_sim* sim);
 /* Region index of every cell (L43): N bytes [z][y][x]. Default: all 0. */
 int mm_set_regions(mm_sim* sim, const uint8_t* regions);
 
+/* Geometry (L53, "B. Geometry", Fig. 2): the shape of the magnet as one byte per cell, [z][y][x], host or device
+ * pointer, copied during the call. Non-zero = inside the shape, 0 = outside: such a cell is vacuum whatever its
+ * region index says - no magnetisation (m = 0), no exchange coupling to it (a neighbour outside the shape is an
+ * open boundary, L196), no torque. The shape does not use up the caller's region indices, but it reserves index
+ * 255 of the look-up tables: with a geometry set, mm_set_params accepts at most 255 regions and a region map may
+ * not hold index 255 (MM_EINVAL otherwise). NULL removes the geometry. The magnetisation already stored is
+ * re-normalised (cells that left the shape become 0; cells that entered it keep 0 until mm_set_m gives them a
+ * direction), so mm_set_m usually follows. Errors: MM_EINVAL, MM_ENOMEM, MM_ECUDA. */
+int mm_set_geometry(mm_sim* sim, const uint8_t* inside);
+
 /* Material tables and applied field. Rebuilds the device look-up tables (1-D tables per region and
  * the lower-triangular inter-region exchange table, Fig. 1 L31) and invalidates the FSAL slope. */
 int mm_set_params(mm_sim* sim, const mm_params* params);

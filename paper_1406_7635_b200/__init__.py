@@ -60,6 +60,7 @@ _SIGNATURES = {
                                C.c_int, C.c_int, C.c_int, ALLOC_FN, FREE_FN, C.c_void_p, C.c_void_p]),
     "mm_destroy": (C.c_int, [C.c_void_p]),
     "mm_set_regions": (C.c_int, [C.c_void_p, C.c_void_p]),
+    "mm_set_geometry": (C.c_int, [C.c_void_p, C.c_void_p]),
     "mm_set_params": (C.c_int, [C.c_void_p, C.POINTER(mm_params)]),
     "mm_set_terms": (C.c_int, [C.c_void_p, C.c_uint]),
     "mm_set_option": (C.c_int, [C.c_void_p, C.c_int, C.c_int]),
@@ -161,7 +162,9 @@ def make_params(p):
 class Sim:
     """One simulation box on the current CUDA device; methods map 1:1 onto the mm_* calls."""
 
-    def __init__(self, grid, cell, pbc=(0, 0, 0), use_torch_allocator=True):
+    def __init__(self, grid, cell, pbc=(0, 0, 0), use_torch_allocator=True, guard_bytes=0):
+        """guard_bytes > 0 (debugging aid, with the torch allocator): every device buffer of the handle gets a guard
+        zone of that many bytes on either side, filled with 0xA5; check_guards() tells whether any kernel wrote there."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: the mm_b200 path has no CPU fallback")
@@ -173,7 +176,21 @@ class Sim:
         self._h = C.c_void_p()
         dev = torch.cuda.current_device()
         stream = torch.cuda.current_stream().cuda_stream     # 0 (the legacy default stream): the handle makes its own
-        if use_torch_allocator:
+        self._guards = {}
+        if use_torch_allocator and guard_bytes:
+            gb = (int(guard_bytes) + 255) // 256 * 256
+
+            def _alloc(nbytes, ctx):
+                try:
+                    buf = torch.full((int(nbytes) + 2 * gb,), 0xA5, dtype=torch.uint8, device="cuda")
+                except Exception:
+                    return None
+                self._guards[buf.data_ptr() + gb] = (buf, int(nbytes), gb)
+                return buf.data_ptr() + gb
+
+            def _free(ptr, ctx):
+                self._guards.pop(ptr, None)
+        elif use_torch_allocator:
             _new, _delete = torch.cuda.caching_allocator_alloc, torch.cuda.caching_allocator_delete
 
             def _alloc(nbytes, ctx):
@@ -195,6 +212,15 @@ class Sim:
             code = lib().mm_create(C.byref(self._h), nx, ny, nz, cell[0], cell[1], cell[2], pbc[0], pbc[1], pbc[2])
         if code != MM_OK:
             raise MMError(code, lib().mm_strerror(code).decode() + " (" + lib().mm_last_error(None).decode() + ")")
+
+    def check_guards(self):
+        """Number of device buffers whose guard zones were written to (needs guard_bytes > 0 at construction)."""
+        self._torch.cuda.synchronize()
+        bad = 0
+        for buf, n, gb in self._guards.values():
+            if not (bool((buf[:gb] == 0xA5).all()) and bool((buf[gb + n:] == 0xA5).all())):
+                bad += 1
+        return bad
 
     @property
     def stream(self):
@@ -219,6 +245,15 @@ class Sim:
         if isinstance(regions, np.ndarray):
             regions = np.ascontiguousarray(regions, dtype=np.uint8)
         _check(lib().mm_set_regions(self._h, _ptr(regions)), self._h)
+
+    def set_geometry(self, inside):
+        """Shape of the magnet: one byte per cell [z][y][x], non-zero = inside (None removes it)."""
+        if inside is None:
+            _check(lib().mm_set_geometry(self._h, None), self._h)
+            return
+        if isinstance(inside, np.ndarray):
+            inside = np.ascontiguousarray(inside, dtype=np.uint8)
+        _check(lib().mm_set_geometry(self._h, _ptr(inside)), self._h)
 
     def set_params(self, p):
         s, keep = make_params(p)

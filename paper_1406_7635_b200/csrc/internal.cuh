@@ -31,7 +31,9 @@ struct mm_sim {
   size_t cur_bytes = 0, peak_bytes = 0;
   // device memory
   float* field[R_COUNT] = {};
-  uint8_t* regions = nullptr;
+  uint8_t* regions = nullptr;      // effective region index of every cell (what the kernels read)
+  uint8_t* regions_user = nullptr; // with a geometry: the caller's region map (regions = inside ? regions_user : 255)
+  uint8_t* geom = nullptr;         // with a geometry: the shape, one byte per cell (mm_set_geometry)
   Luts* luts = nullptr;
   DevState* dstate = nullptr;
   float2* spec = nullptr;

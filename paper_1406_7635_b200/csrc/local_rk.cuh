@@ -487,6 +487,15 @@ __global__ void k_ctrl_end(DevState* st) {
   }
 }
 
+// effective region map of a box with a geometry (mm_set_geometry): cells outside the shape take the reserved
+// vacuum index (its look-up-table entries are zero: no B_sat, no exchange)
+#define MM_VACUUM_REGION (MM_MAX_REGIONS - 1)
+__global__ void k_apply_geometry(long long N, const uint8_t* __restrict__ user, const uint8_t* __restrict__ inside,
+                                 uint8_t* __restrict__ out) {
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x)
+    out[i] = inside[i] ? user[i] : (uint8_t)MM_VACUUM_REGION;
+}
+
 // largest region id of the map (validated against nregions without copying the map to the host)
 __global__ void k_max_region(long long N, const uint8_t* __restrict__ regions, unsigned* __restrict__ out) {
   unsigned best = 0;
@@ -691,6 +700,8 @@ __global__ void k_add_zl(Geometry g, const uint8_t* __restrict__ regions, const 
   const int y = (int)(t % g.Ny), z = (int)(t / g.Ny);
   float dx = 0.f, dy = 0.f, dz = 0.f;
   auto diff = [&](long long up, long long dn, float c) {
+    if (!(lut->Bsat[regions[up]] > 0.f)) up = i;       // a vacuum neighbour is a missing neighbour: own m (L196, L53)
+    if (!(lut->Bsat[regions[dn]] > 0.f)) dn = i;
     dx += c * (m[up] - m[dn]); dy += c * (m[N + up] - m[N + dn]); dz += c * (m[2 * N + up] - m[2 * N + dn]);
   };
   if (g.Nx > 1 && p.c[0] != 0.f) {

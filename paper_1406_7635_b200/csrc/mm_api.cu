@@ -229,7 +229,7 @@ void launch_local(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_
       if (th) MM_LOCAL4(U, true, 0, D); else if (fuse == 1) MM_LOCAL4(U, false, 1, D);                                   \
       else if (fuse == 2) MM_LOCAL4(U, false, 2, D); else MM_LOCAL4(U, false, 0, D);                                    \
     } while (0)
-    if (s->nregions == 1) { if (s->dmi_on) MM_LOCAL4_PICK(true, true); else MM_LOCAL4_PICK(true, false); }
+    if (s->nregions == 1 && !s->geom) { if (s->dmi_on) MM_LOCAL4_PICK(true, true); else MM_LOCAL4_PICK(true, false); }
     else { if (s->dmi_on) MM_LOCAL4_PICK(false, true); else MM_LOCAL4_PICK(false, false); }
 #undef MM_LOCAL4_PICK
 #undef MM_LOCAL4
@@ -538,6 +538,8 @@ static int max_region_on_device(mm_sim* s, const uint8_t* dev_regions, unsigned*
   return MM_OK;
 }
 
+static int apply_geometry(mm_sim* s);
+
 int mm_set_regions(mm_sim* s, const uint8_t* regions) {
   if (!s || !regions) return mm_fail(s, MM_EINVAL, "null argument");
   // validate the ids against the current table size before the handle's map is touched
@@ -551,15 +553,66 @@ int mm_set_regions(mm_sim* s, const uint8_t* regions) {
     }
     if ((int)top >= s->nregions) return mm_fail(s, MM_EINVAL, "region id >= nregions");
   }
-  int rc = copy_in(s, s->regions, regions, (size_t)s->g.N);
+  int rc = copy_in(s, s->geom ? s->regions_user : s->regions, regions, (size_t)s->g.N);
+  if (!rc && s->geom) rc = apply_geometry(s);
   s->have_k1 = false; s->graph_dirty = true;
   return rc;
+}
+
+// regions = inside the shape ? the caller's index : the reserved vacuum index
+static int apply_geometry(mm_sim* s) {
+  { Launch l(s, KK_OTHER); k_apply_geometry<<<s->nsm * 8, 256, 0, s->stream>>>(s->g.N, s->regions_user, s->geom, s->regions); }
+  CUDA_TRY(s, cudaGetLastError());
+  return MM_OK;
+}
+
+int mm_set_geometry(mm_sim* s, const uint8_t* inside) {
+  if (!s) return MM_EINVAL;
+  const size_t N = (size_t)s->g.N;
+  int rc;
+  if (!inside) {                                    // remove the shape: the caller's map becomes the effective one again
+    if (!s->geom) return MM_OK;
+    CUDA_TRY(s, cudaMemcpyAsync(s->regions, s->regions_user, N, cudaMemcpyDeviceToDevice, s->stream));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    mm_dev_free(s, s->geom); mm_dev_free(s, s->regions_user);
+    s->geom = s->regions_user = nullptr;
+  } else {
+    if (s->have_params && s->nregions > MM_MAX_REGIONS - 1)
+      return mm_fail(s, MM_EINVAL, "a geometry reserves region index 255: at most 255 regions");
+    if (!s->geom) {
+      unsigned top = 0;
+      if ((rc = max_region_on_device(s, s->regions, &top))) return rc;
+      if (top >= MM_MAX_REGIONS - 1) return mm_fail(s, MM_EINVAL, "a geometry reserves region index 255: the region map uses it");
+      s->geom = (uint8_t*)mm_dev_alloc(s, N);
+      s->regions_user = (uint8_t*)mm_dev_alloc(s, N);
+      if (!s->geom || !s->regions_user) {
+        mm_dev_free(s, s->geom); mm_dev_free(s, s->regions_user);
+        s->geom = s->regions_user = nullptr;
+        return mm_fail(s, MM_ENOMEM, "geometry");
+      }
+      CUDA_TRY(s, cudaMemcpyAsync(s->regions_user, s->regions, N, cudaMemcpyDeviceToDevice, s->stream));
+    }
+    if ((rc = copy_in(s, s->geom, inside, N))) return rc;
+    if ((rc = apply_geometry(s))) return rc;
+  }
+  // the kernels take their one-region shortcuts from the table size: a box with a shape has two kinds of cells
+  const int nreg_dev = s->geom ? MM_MAX_REGIONS : s->nregions;
+  CUDA_TRY(s, cudaMemcpyAsync(&s->luts->nregions, &nreg_dev, sizeof(int), cudaMemcpyHostToDevice, s->stream));
+  CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+  if (s->have_m) {                                  // cells outside the shape carry no magnetisation
+    if ((rc = pull_state(s))) return rc;
+    { Launch l(s, KK_OTHER); k_normalise<<<blocks_for(s->g.N, 256), 256, 0, s->stream>>>(s->g.N, s->hst.ptr[R_M], s->regions, s->luts); }
+    CUDA_TRY(s, cudaGetLastError());
+  }
+  s->have_k1 = false; s->graph_dirty = true;
+  return MM_OK;
 }
 
 int mm_set_params(mm_sim* s, const mm_params* p) {
   if (!s || !p) return mm_fail(s, MM_EINVAL, "null argument");
   const int n = p->nregions;
   if (n < 1 || n > MM_MAX_REGIONS) return mm_fail(s, MM_EINVAL, "nregions out of range");
+  if (s->geom && n > MM_MAX_REGIONS - 1) return mm_fail(s, MM_EINVAL, "a geometry reserves region index 255: at most 255 regions");
   if (s->dmi_n > 1 && s->dmi_n != n) return mm_fail(s, MM_EINVAL, "the DM table of mm_set_dmi has another number of regions");
   for (int r = 0; r < n; ++r) {
     if (!(p->Msat[r] >= 0) || !(p->Aex[r] >= 0) || !std::isfinite(p->Msat[r]) || !std::isfinite(p->Aex[r]) ||
@@ -569,7 +622,7 @@ int mm_set_params(mm_sim* s, const mm_params* p) {
   }
   {
     unsigned top = 0;
-    int rc = max_region_on_device(s, s->regions, &top);
+    int rc = max_region_on_device(s, s->geom ? s->regions_user : s->regions, &top);
     if (rc) return rc;
     if ((int)top >= n) return mm_fail(s, MM_EINVAL, "region map holds an id >= nregions");
   }
@@ -581,7 +634,7 @@ int mm_set_params(mm_sim* s, const mm_params* p) {
     double nn = std::sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
     for (int c = 0; c < 3; ++c) o[c] = nn > 0 ? v[c] / nn : 0.0;
   };
-  L->nregions = n;
+  L->nregions = s->geom ? MM_MAX_REGIONS : n;      // (entries beyond n stay zero: index 255 is the vacuum of a geometry)
   std::vector<double> q(n);
   for (int r = 0; r < n; ++r) {
     const double Ms = p->Msat[r], iMs = Ms > 0 ? 1.0 / Ms : 0.0;

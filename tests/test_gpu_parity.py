@@ -178,6 +178,29 @@ def test_fast3d_mixed_stages(mm, grid, pbc, kinds):
     assert np.abs(Bf - Bg).max() <= 2e-5 * np.abs(Bg).max()
 
 
+@pytest.mark.parametrize("grid,pbc", [((384, 320, 1), (0, 0, 0)), ((1000, 600, 1), (0, 0, 0)), ((40, 64, 32), (0, 0, 0)),
+                                      ((64, 64, 32), (2, 2, 0)), ((70, 45, 20), (0, 0, 0))])
+def test_kernels_stay_inside_their_buffers_and_are_reproducible(mm, grid, pbc):
+    # compute-sanitizer is closed on the GPU pool, so the two things it would check are tested directly: every
+    # device buffer of the handle sits between guard zones that must still hold their fill pattern after field
+    # evaluations and steps on every kernel path (out-of-bounds writes), and repeated evaluations of the same state
+    # must give the same bits (a shared-memory race in the exchange / TMA staging would not)
+    cfg = _rand_cfg(grid, (3e-9, 2e-9, 2.5e-9), pbc=pbc, nreg=3, anis=True, seed=41)
+    sim = mm.from_config(cfg, guard_bytes=1 << 16)
+    first = sim.b_eff(MM_ALL).copy()
+    for _ in range(5):
+        assert np.array_equal(sim.b_eff(MM_ALL), first)
+    sim.set_solver(fix_dt=2e-14)
+    sim.steps(3)
+    m1 = sim.get_m().copy()
+    assert sim.check_guards() == 0
+    sim2 = mm.from_config(cfg, guard_bytes=1 << 16)
+    sim2.set_solver(fix_dt=2e-14)
+    sim2.steps(3)
+    assert np.array_equal(sim2.get_m(), m1)
+    assert sim2.check_guards() == 0
+
+
 def test_fast2d_one_region_and_steps(mm):
     # one region (the bench workload's shape): B_sat is a constant and the region gathers are skipped
     cfg = config_c4(512)
@@ -859,6 +882,67 @@ def test_zhang_li_torque_and_advection(mm):
     sim.run(t)
     m = sim.get_m()
     assert np.abs(m[0, 0, 0] - np.cos(k * x - w * t)).max() < 2e-5 and np.abs(m[2]).max() < 1e-5
+
+
+def test_zhang_li_next_to_vacuum_cells(mm):
+    # a current through a box with vacuum regions (Msat = 0): a vacuum neighbour is a missing neighbour for the
+    # gradient of Eq. 26, as in the oracle (pinned there against the chain that ends at the interface)
+    cfg = _rand_cfg((24, 12, 4), (4e-9, 3e-9, 2e-9), pbc=(0, 2, 0), nreg=3, anis=True, seed=13)
+    cfg["params"].Msat[1] = 0.0
+    sim = mm.from_config(cfg)
+    ref = _ref_from(cfg, "fft")
+    j, xi = (3e12, -1e12, 2e12), 0.3
+    sim.set_zhang_li(j, xi); ref.set_zhang_li(j, xi)
+    tq = sim.torque().astype(np.float64)
+    tr = ref.torque(ref.m) / ref.p.gamma_LL
+    assert np.abs(tq - tr).max() <= FIELD_TOL * np.abs(tr).max()
+    assert np.all(tq[:, cfg["regions"] == 1] == 0)
+
+
+# --------------------------------------------------------------------------- geometry
+@pytest.mark.parametrize("grid", [(256, 256, 1), (48, 40, 1), (40, 64, 32), (20, 14, 6)])
+def test_geometry_mask_disk_in_a_box(mm, grid):
+    # mm_set_geometry (L53, Fig. 2): a disk (cylinder) inside the box, three material regions inside it. The oracle
+    # models the same magnet with one more region of Msat = 0 outside the shape; fields, energy and a short
+    # trajectory must agree, m stays 0 outside, and removing the shape restores the full box. Covers the fast 2D,
+    # generic and 3D register kernels (B_sat gather, stencil next to vacuum).
+    nx, ny, nz = grid
+    cfg = _rand_cfg(grid, (4e-9, 4e-9, 3e-9), nreg=3, anis=True, seed=51)
+    yy, xx = np.meshgrid(np.arange(ny) - (ny - 1) / 2, np.arange(nx) - (nx - 1) / 2, indexing="ij")
+    inside2d = (xx / (0.45 * nx)) ** 2 + (yy / (0.45 * ny)) ** 2 <= 1.0
+    inside = np.broadcast_to(inside2d, (nz, ny, nx)).astype(np.uint8).copy()
+    sim = mm.from_config(cfg)
+    sim.set_geometry(inside)
+    sim.set_m(cfg["m0"])
+    # the oracle's description of the same magnet: region 3 = vacuum
+    p = cfg["params"]
+    pr = Params.uniform(4, Msat=list(p.Msat) + [0.0], Aex=list(p.Aex) + [0.0], alpha=list(p.alpha) + [0.0], B_ext=p.B_ext)
+    for name in ("Ku1", "Ku2", "Kc1", "Kc2", "Kc3"):
+        setattr(pr, name, np.append(getattr(p, name), 0.0))
+    for name in ("anisU", "anisC1", "anisC2"):
+        setattr(pr, name, np.vstack([getattr(p, name), [[0.0, 0.0, 1.0] if name != "anisC2" else [1.0, 0.0, 0.0]]]))
+    S = np.ones(10); S[:6] = p.exch_scale
+    pr.exch_scale = S
+    cfg_ref = dict(cfg, regions=np.where(inside > 0, cfg["regions"], 3).astype(np.uint8), params=pr)
+    ref = _ref_from(cfg_ref, "fft")
+    _field_check(sim, ref, (MM_DEMAG, MM_EXCH, MM_ALL))
+    m = sim.get_m()
+    assert np.all(m[:, inside == 0] == 0) and np.allclose(np.linalg.norm(m[:, inside > 0], axis=0), 1.0, atol=1e-6)
+    assert abs(sim.energy() - ref.energy()) <= 2e-5 * abs(ref.energy())
+    sim.set_solver(fix_dt=2e-14); ref.set_solver(fix_dt=2e-14)
+    sim.steps(10)
+    for _ in range(10):
+        ref.step()
+    assert np.abs(sim.get_m() - ref.m).max() < 5e-5
+    assert np.all(sim.get_m()[:, inside == 0] == 0)
+    # error paths and removal
+    with pytest.raises(mm.MMError):
+        bad = cfg["regions"].copy(); bad[0, 0, 0] = 255
+        sim.set_regions(bad)
+    sim.set_geometry(None)
+    sim.set_m(cfg["m0"])
+    full = _ref_from(cfg, "fft")
+    _field_check(sim, full, (MM_ALL,))
 
 
 # --------------------------------------------------------------------------- Dzyaloshinskii-Moriya exchange
