@@ -205,6 +205,7 @@ class Sim:
                 except Exception:      # interpreter shutdown: torch is already gone
                     pass
 
+        if use_torch_allocator:
             self._cb = (ALLOC_FN(_alloc), FREE_FN(_free))
             code = lib().mm_create_ex(C.byref(self._h), nx, ny, nz, cell[0], cell[1], cell[2], pbc[0], pbc[1], pbc[2],
                                       self._cb[0], self._cb[1], None, C.c_void_p(stream))
