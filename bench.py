@@ -176,6 +176,48 @@ def spawn_ranks(args):
     raise SystemExit(subprocess.call(cmd))
 
 
+def run_batch(args, mm, torch, replicas, rank, world, local_rank):
+    """B independent C4 boxes per GPU stepping concurrently: aggregate cell-updates/s and time per box and step."""
+    from synth import config_c4
+    n, B = args.size, args.batch
+    sims = []
+    for b in range(B):
+        cfg = config_c4(n, seed_offset=replicas.replica_seed(b, rank))
+        sim = mm.from_config(cfg)
+        sim.set_solver(fix_dt=cfg["fix_dt"])
+        sims.append(sim)
+    mm.batch_steps(sims, args.warmup)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    l0 = sum(s_.launch_count() for s_ in sims)
+    streams = [s_.stream for s_ in sims]
+    e0 = [torch.cuda.Event(enable_timing=True) for _ in sims]
+    e1 = [torch.cuda.Event(enable_timing=True) for _ in sims]
+    for a_, st in zip(e0, streams):
+        a_.record(st)
+    mm.batch_steps(sims, args.steps)
+    for b_, st in zip(e1, streams):
+        b_.record(st)
+    torch.cuda.synchronize()
+    ms = max(a_.elapsed_time(b_) for a_ in e0 for b_ in e1)          # first start to last end, on the device
+    launches = sum(s_.launch_count() for s_ in sims) - l0
+    clocks = sampler.stop() if sampler else None
+    cells = n * n * B
+    value, ms = replicas.aggregate_throughput(cells * args.steps, ms, device="cuda")
+    if rank == 0:
+        working = sum(s_.stats()["peak_device_bytes"] for s_ in sims)
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms / args.steps, "ms_per_box_step": ms / args.steps / B, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": "%d independent C4 films %dx%dx1 advancing together (mm_batch_steps), fix_dt 1e-13 s" % (B, n, n),
+                           "cells": cells, "batch": B, "parallelism": "replicas x%d" % world,
+                           "l2": "working set %.2f GB (all boxes)" % (working / 1e9), "evals_per_step": 6},
+                "clocks": clocks, "gpu_launches": launches,
+                "step_roofline": {"achieved": STEP_BYTES_PER_CELL * value / 1e9, "peak": measured_peak_gbs()[0], "unit": "GB/s",
+                                  "frac": STEP_BYTES_PER_CELL * value / 1e9 / measured_peak_gbs()[0]}}
+        print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -186,6 +228,9 @@ def main():
                     help="c4: size x size x 1 film (default, the metric's workload); c4regions: the same film cut into 64 "
                          "Voronoi regions with an inter-region exchange table; c5 / c5pbc: size^3 cube, open / "
                          "PBC(4,4,0); c3: 128 x 128 x 32 multi-region block, adaptive steps (--size is ignored)")
+    ap.add_argument("--batch", type=int, default=0,
+                    help="c4 only: this many independent boxes of --size advance together (mm_batch_steps, one stream "
+                         "per handle): the paper's batch use of small simulations (L426, L800-L803)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-size", type=int, default=1024, help="film edge of the timed oracle sample")
     ap.add_argument("--cpu-steps", type=int, default=8)
@@ -222,6 +267,11 @@ def main():
     from synth import config_c4
 
     n = args.size
+    if args.batch > 0:
+        run_batch(args, mm, torch, replicas, rank, world, local_rank)
+        if world > 1:
+            dist.destroy_process_group()
+        return
     if args.workload == "c4":
         cfg = config_c4(n, seed_offset=replicas.replica_seed(0, rank))     # one independent replica per rank
         cells, step_bytes = n * n, STEP_BYTES_PER_CELL
