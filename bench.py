@@ -399,7 +399,7 @@ def main():
                            "evals_per_step": 6},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
                 "step_roofline": step_roofline, "kernels": kernels,
-                "peak_device_bytes": sim.stats()["peak_device_bytes"]}
+                "peak_device_bytes": sim.stats()["peak_device_bytes"], "resident_device_bytes": sim.memory()[0]}
         line["cpu_baseline"] = None if (args.no_cpu_baseline or world > 1) else cpu_baseline(args)
         print(json.dumps(line), flush=True)
     if world > 1:

@@ -239,6 +239,9 @@ int mm_set_time(mm_sim* sim, double t);
 int mm_get_avg_m(mm_sim* sim, double avg[3]);
 /* Counters: accepted steps, rejected attempts, torque evaluations, peak device bytes owned. */
 int mm_get_stats(mm_sim* sim, long* steps, long* rejected, long* evals, size_t* peak_device_bytes);
+/* Device bytes the handle owns now and the most it ever owned (the fp64 scratch of the kernel set-up is freed
+ * before the vector fields are allocated). The paper's context: about 220 B/cell for 2D RK45 (L533). */
+int mm_get_memory(mm_sim* sim, size_t* resident_bytes, size_t* peak_bytes);
 /* The CUDA stream all work of this handle is enqueued on (a cudaStream_t). */
 int mm_get_stream(mm_sim* sim, void** cuda_stream);
 /* Padded FFT sizes chosen for this box (Px, Py, Pz). */

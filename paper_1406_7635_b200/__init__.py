@@ -90,6 +90,7 @@ _SIGNATURES = {
     "mm_get_avg_m": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
     "mm_get_stats": (C.c_int, [C.c_void_p, C.POINTER(C.c_long), C.POINTER(C.c_long), C.POINTER(C.c_long),
                                C.POINTER(C.c_size_t)]),
+    "mm_get_memory": (C.c_int, [C.c_void_p, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]),
     "mm_get_stream": (C.c_int, [C.c_void_p, C.POINTER(C.c_void_p)]),
     "mm_get_fft_size": (C.c_int, [C.c_void_p, C.POINTER(C.c_int)]),
     "mm_get_launch_count": (C.c_int, [C.c_void_p, C.POINTER(C.c_long)]),
@@ -364,6 +365,12 @@ class Sim:
         a, b, c, d = C.c_long(), C.c_long(), C.c_long(), C.c_size_t()
         _check(lib().mm_get_stats(self._h, C.byref(a), C.byref(b), C.byref(c), C.byref(d)), self._h)
         return dict(steps=a.value, rejected=b.value, evals=c.value, peak_device_bytes=d.value)
+
+    def memory(self):
+        """(resident, peak) device bytes owned by the handle."""
+        a, b = C.c_size_t(), C.c_size_t()
+        _check(lib().mm_get_memory(self._h, C.byref(a), C.byref(b)), self._h)
+        return a.value, b.value
 
     def fft_size(self):
         v = (C.c_int * 3)()

@@ -91,7 +91,7 @@ struct mm_sim {
 int mm_fail(mm_sim* s, int code, const std::string& msg);
 void* mm_dev_alloc(mm_sim* s, size_t bytes);
 void mm_dev_free(mm_sim* s, void* p);
-int mm_build_kernel_spectrum(mm_sim* s);   // setup.cu
+int mm_build_kernel_spectrum(mm_sim* s, int layouts);   // setup.cu: bit 0 generic K, bit 1 fast 2D layout Kt
 bool mm_fast2d_supported(int Nx, int Ny, int Nz, const int* pbc);   // fast2d.cu
 int mm_fast2d_length(int N);      // transform length of the fast path for N physical cells (power of two)
 int mm_fast2d_init(mm_sim* s);

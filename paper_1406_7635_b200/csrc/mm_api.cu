@@ -472,10 +472,6 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
   if ((rc = configure_launches(s))) { std::string m = s->err; return bail(rc, m.c_str()); }
   // device memory
   const size_t fbytes = sizeof(float) * 3 * (size_t)g.N;
-  for (int r = 0; r < R_COUNT; ++r) {
-    s->field[r] = (float*)mm_dev_alloc(s, fbytes);
-    if (!s->field[r]) return bail(MM_ENOMEM, "field arrays");
-  }
   s->regions = (uint8_t*)mm_dev_alloc(s, (size_t)g.N);
   s->luts = (Luts*)mm_dev_alloc(s, sizeof(Luts));
   s->dstate = (DevState*)mm_dev_alloc(s, sizeof(DevState));
@@ -488,11 +484,10 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
   s->red_ticket = reinterpret_cast<unsigned*>(s->red_part + 3 * 8 * s->nsm);
   if (cudaMemsetAsync(s->red_ticket, 0, sizeof(double), s->stream) != cudaSuccess) return bail(MM_ECUDA, "memset");
   if (cudaMemsetAsync(s->regions, 0, (size_t)g.N, s->stream) != cudaSuccess) return bail(MM_ECUDA, "memset");
-  for (int r = 0; r < R_COUNT; ++r) cudaMemsetAsync(s->field[r], 0, fbytes, s->stream);
   if ((rc = upload_twiddles(s, g.Px, &s->twx)) || (rc = upload_twiddles(s, g.Py, &s->twy)) ||
       (rc = upload_twiddles(s, g.Pz, &s->twz)))
     return bail(rc, "twiddles");
-  if ((rc = mm_build_kernel_spectrum(s))) { std::string m = s->err; return bail(rc, m.c_str()); }
+  if ((rc = mm_build_kernel_spectrum(s, 3))) { std::string m = s->err; return bail(rc, m.c_str()); }
   // convolution arguments
   ConvArgs& c = s->conv;
   c.g = g; c.px = s->px; c.py = s->py; c.pz = s->pz;
@@ -502,6 +497,20 @@ int mm_create_ex(mm_sim** out, int Nx, int Ny, int Nz, double dx, double dy, dou
   c.regions = s->regions; c.luts = s->luts; c.st = s->dstate;
   if (s->fast2d && (rc = mm_fast2d_init(s))) { std::string m = s->err; return bail(rc, m.c_str()); }
   if (s->fast3d && (rc = mm_fast3d_init(s))) { std::string m = s->err; return bail(rc, m.c_str()); }
+  // a box whose convolution runs entirely on a fast layout (Kt of the 2D path, the z-stage tiles of the 3D path)
+  // does not keep the generic layout of the kernel spectrum; MM_OPT_GENERIC_FFT builds it again when asked for
+  if (s->fast2d || (s->fast3d && s->f3.mode[2])) {
+    if (cudaStreamSynchronize(s->stream) != cudaSuccess) return bail(MM_ECUDA, "kernel set-up");
+    mm_dev_free(s, s->K);
+    s->K = nullptr; s->conv.K = nullptr;
+  }
+  // the twelve vector fields come last: the fp64 scratch of the kernel set-up is gone by now, so the peak of the
+  // handle's device memory is what it keeps, not set-up scratch on top of it (the paper's B/cell context, L533)
+  for (int r = 0; r < R_COUNT; ++r) {
+    s->field[r] = (float*)mm_dev_alloc(s, fbytes);
+    if (!s->field[r]) return bail(MM_ENOMEM, "field arrays");
+    if (cudaMemsetAsync(s->field[r], 0, fbytes, s->stream) != cudaSuccess) return bail(MM_ECUDA, "memset");
+  }
   // controller state
   DevState& h = s->hst;
   memset(&h, 0, sizeof(h));
@@ -786,7 +795,14 @@ int mm_step(mm_sim* s, mm_step_info* info) { return mm_step_rk45(s, info); }
 int mm_set_option(mm_sim* s, int option, int value) {
   if (!s) return MM_EINVAL;
   switch (option) {
-    case MM_OPT_GENERIC_FFT: s->force_generic = value != 0; s->have_k1 = false; s->graph_dirty = true; return MM_OK;
+    case MM_OPT_GENERIC_FFT:
+      if (value && !s->K) {                    // the generic layout was dropped after the set-up: build it again
+        int rc = mm_build_kernel_spectrum(s, 1);
+        if (rc) return rc;
+        s->conv.K = s->K;
+      }
+      s->force_generic = value != 0; s->have_k1 = false; s->graph_dirty = true;
+      return MM_OK;
     case MM_OPT_NO_TMA: s->f2_no_tma = value != 0; s->have_k1 = false; s->graph_dirty = true; return MM_OK;
     case MM_OPT_NO_GRAPH: s->no_graph = value != 0; return MM_OK;
     default: return mm_fail(s, MM_EINVAL, "unknown option");
@@ -1171,6 +1187,13 @@ int mm_get_stats(mm_sim* s, long* steps, long* rejected, long* evals, size_t* pe
   if (steps) *steps = (long)s->hst.steps;
   if (rejected) *rejected = (long)s->hst.rejected;
   if (evals) *evals = (long)s->hst.evals + s->extra_evals;
+  if (peak) *peak = s->peak_bytes;
+  return MM_OK;
+}
+
+int mm_get_memory(mm_sim* s, size_t* resident, size_t* peak) {
+  if (!s) return MM_EINVAL;
+  if (resident) *resident = s->cur_bytes;
   if (peak) *peak = s->peak_bytes;
   return MM_OK;
 }

@@ -4,7 +4,8 @@
 #include "demag_setup.cuh"
 
 // ---- demag kernel set-up (fp64 on the device)
-int mm_build_kernel_spectrum(mm_sim* s) {
+// layouts: bit 0 = the generic K[comp][kz][ky][kx], bit 1 = the fast 2D layout Kt (only if the box has that path)
+int mm_build_kernel_spectrum(mm_sim* s, int layouts) {
   const Geometry& g = s->g;
   setup::TensorGrid tg;
   tg.N[0] = g.Nx; tg.N[1] = g.Ny; tg.N[2] = g.Nz;
@@ -18,11 +19,14 @@ int mm_build_kernel_spectrum(mm_sim* s) {
   const long long nfull = (long long)g.Px * g.Py * g.Pz;
   const int ncomp = (g.Nz == 1 && s->rep[2] == 0) ? 4 : 6;
   const long long nk = (long long)g.Cx * g.Hy * g.Hz;
-  s->K = (float*)mm_dev_alloc(s, sizeof(float) * nk * ncomp);
-  if (!s->K) return mm_fail(s, MM_ENOMEM, "kernel spectrum");
+  const bool want_k = (layouts & 1) != 0, want_kt = (layouts & 2) != 0 && s->fast2d;
+  if (want_k) {
+    s->K = (float*)mm_dev_alloc(s, sizeof(float) * nk * ncomp);
+    if (!s->K) return mm_fail(s, MM_ENOMEM, "kernel spectrum");
+  }
   const int fNy = g.Py / 2;      // transform length along y of the fast path
   const long long nkt = (long long)g.Cx * (fNy + 1);
-  if (s->fast2d) {
+  if (want_kt) {
     s->Kt = (float*)mm_dev_alloc(s, sizeof(float) * nkt * 4);
     if (!s->Kt) return mm_fail(s, MM_ENOMEM, "kernel spectrum (fast layout)");
   }
@@ -56,10 +60,12 @@ int mm_build_kernel_spectrum(mm_sim* s) {
       }
       stride *= pl.P;
     }
-    setup::k_pack_spectrum<<<blocks_for(nk, 256), 256, 0, s->stream>>>(tg, src, s->K + (size_t)comp * nk, g.Cx, g.Hy, g.Hz,
-                                                                       scale, maxim);
-    s->launches++;
-    if (s->fast2d) {
+    if (want_k) {
+      setup::k_pack_spectrum<<<blocks_for(nk, 256), 256, 0, s->stream>>>(tg, src, s->K + (size_t)comp * nk, g.Cx, g.Hy, g.Hz,
+                                                                         scale, maxim);
+      s->launches++;
+    }
+    if (want_kt) {
       setup::k_pack_spectrum_2dfast<<<blocks_for(nkt, 256), 256, 0, s->stream>>>(tg, src, s->Kt + (size_t)comp * nkt, g.Cx,
                                                                                  fNy, scale);
       s->launches++;
