@@ -151,9 +151,11 @@ __device__ __forceinline__ void stg_f(float* p, float v) { asm volatile("st.glob
 }  // namespace f3
 
 // ---------------------------------------------------------------------------------- x stage
-// grid (row pairs / G, component); block G * P::T threads (t fastest); shared memory G * row_pitch float4
+// grid (row pairs / G, component); block G * P::T threads (t fastest); shared memory G * row_pitch float4.
+// (The forward kernel waits mostly on its row loads: three CTAs per SM at 80 registers beat two at 96, 0.276 -> 0.222 ms
+// at 256^3; the same bound makes the inverse kernel and the y stage slower.)
 template <class P, int G>
-__global__ void __launch_bounds__(P::T * G) k3_xfwd(Fast3DArgs a, int src_role) {
+__global__ void __launch_bounds__(P::T * G, 3) k3_xfwd(Fast3DArgs a, int src_role) {
   if (a.st->skip) return;
   constexpr int N = P::N, T = P::T, E = P::E;
   static_assert(P::RA == 16 && E == 16, "sixteen points per thread at stride N/16 on the sample side");
