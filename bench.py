@@ -231,6 +231,8 @@ def main():
     ap.add_argument("--batch", type=int, default=0,
                     help="c4 only: this many independent boxes of --size advance together (mm_batch_steps, one stream "
                          "per handle): the paper's batch use of small simulations (L426, L800-L803)")
+    ap.add_argument("--adaptive", action="store_true",
+                    help="c4: adaptive RK45 (MaxErr 1e-5) instead of the fixed step; attempts (accepted or not) count as steps")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-size", type=int, default=1024, help="film edge of the timed oracle sample")
     ap.add_argument("--cpu-steps", type=int, default=8)
@@ -294,6 +296,9 @@ def main():
         cells = n ** 3
         step_bytes = 6 * 140.0 + 372.0 if args.workload == "c5pbc" else 2472.0
         wname = "C5 cube %d^3, 2 nm, Kc1 -5e3, random m, %s, fix_dt 1e-13 s" % (n, "PBC (4,4,0)" if args.workload == "c5pbc" else "open")
+    if args.adaptive and args.workload in ("c4", "c4regions"):
+        cfg["fix_dt"] = 0.0
+        wname = wname.replace("fix_dt 1e-13 s", "adaptive RK45 (MaxErr 1e-5, attempts counted)")
     sim = mm.from_config(cfg)
     sim.set_solver(fix_dt=cfg["fix_dt"])
     P = sim.fft_size()[0]

@@ -68,10 +68,10 @@ template <int N>
 int x_attrs(mm_sim* s) {
   using F = PlanFor<N>;
   const int fb = (int)k2_fwd_smem<typename F::P, F::NTF>();
-  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd4<typename F::P, F::NTF, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fb));
-  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd4<typename F::P, F::NTF, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, fb));
-  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd4<typename F::P, F::NTF, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fb));
-  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd4<typename F::P, F::NTF, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, fb));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd4<typename F::P, F::NTF, false, false, K2Fwd<typename F::P, F::NTF>::STAGED>, cudaFuncAttributeMaxDynamicSharedMemorySize, fb));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd4<typename F::P, F::NTF, true, false, K2Fwd<typename F::P, F::NTF>::STAGED>, cudaFuncAttributeMaxDynamicSharedMemorySize, fb));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd4<typename F::P, F::NTF, false, true, K2Fwd<typename F::P, F::NTF>::STAGED>, cudaFuncAttributeMaxDynamicSharedMemorySize, fb));
+  CUDA_TRY(s, cudaFuncSetAttribute(k2_xfwd4<typename F::P, F::NTF, true, true, K2Fwd<typename F::P, F::NTF>::STAGED>, cudaFuncAttributeMaxDynamicSharedMemorySize, fb));
   CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv<typename F::P, F::NTI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    (int)k2_smem<typename F::P, F::NTI>()));
   CUDA_TRY(s, cudaFuncSetAttribute(k2_xinv_tma<typename F::P, F::NTI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -102,11 +102,11 @@ void launch_x(mm_sim* s, bool inverse, int role) {
     const dim3 gf((s->g.Ny + ROWS - 1) / ROWS, 3);
     const size_t b = k2_fwd_smem<typename F::P, F::NTF>();
     if (tma_on) {
-      if (ragged) k2_xfwd4<typename F::P, F::NTF, true, true><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd, s->f2_map_fwd_odd);
-      else k2_xfwd4<typename F::P, F::NTF, false, true><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd, s->f2_map_fwd_odd);
+      if (ragged) k2_xfwd4<typename F::P, F::NTF, true, true, K2Fwd<typename F::P, F::NTF>::STAGED><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd, s->f2_map_fwd_odd);
+      else k2_xfwd4<typename F::P, F::NTF, false, true, K2Fwd<typename F::P, F::NTF>::STAGED><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd, s->f2_map_fwd_odd);
     } else {
-      if (ragged) k2_xfwd4<typename F::P, F::NTF, true, false><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd, s->f2_map_fwd_odd);
-      else k2_xfwd4<typename F::P, F::NTF, false, false><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd, s->f2_map_fwd_odd);
+      if (ragged) k2_xfwd4<typename F::P, F::NTF, true, false, K2Fwd<typename F::P, F::NTF>::STAGED><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd, s->f2_map_fwd_odd);
+      else k2_xfwd4<typename F::P, F::NTF, false, false, K2Fwd<typename F::P, F::NTF>::STAGED><<<gf, F::NTF, b, s->stream>>>(s->f2, role, s->f2_map_fwd, s->f2_map_fwd_odd);
     }
   }
   else if (tma_on && xinv_direct<N>())

@@ -313,14 +313,17 @@ __device__ __forceinline__ void exchange(C2* v, void* xbuf, int t, int gid) {
 // exchange buffer (P::XB float4, or P::XB float2 with PLANES). tw: P::TW forward twiddles of this plan. t: thread index inside
 // the group. The first exchange starts with a group barrier, so xb may still be read by the group
 // until then; after the call xb is only safe to reuse after another group barrier.
-template <class P, int DIR, int NT, bool PLANES = false>
-__device__ __forceinline__ void fft(C2* v, void* xb, int t, int gid, const float2* __restrict__ tw) {
+// first pass (butterflies + twiddles: registers only) and the rest (from the first exchange on) as two calls, for
+// kernels that must do something between them (e.g. wait until the exchange buffer is free again)
+template <class P, int DIR>
+__device__ __forceinline__ void fft_head(C2* v, int t, const float2* __restrict__ tw) {
   pass_butterflies<P, P::RA, DIR>(v);
-  {
-    float2 w[(P::RA - 1) * (P::E / P::RA)];
-    load_twiddles<P, P::RA>(w, t, tw);
-    apply_twiddles<P, P::RA, DIR>(v, w);
-  }
+  float2 w[(P::RA - 1) * (P::E / P::RA)];
+  load_twiddles<P, P::RA>(w, t, tw);
+  apply_twiddles<P, P::RA, DIR>(v, w);
+}
+template <class P, int DIR, int NT, bool PLANES = false>
+__device__ __forceinline__ void fft_tail(C2* v, void* xb, int t, int gid, const float2* __restrict__ tw) {
   exchange<P, P::RA, P::RB, P::M1, NT, PLANES>(v, xb, t, gid);
   pass_butterflies<P, P::RB, DIR>(v);
   if constexpr (P::NPASS == 3) {
@@ -332,6 +335,11 @@ __device__ __forceinline__ void fft(C2* v, void* xb, int t, int gid, const float
     exchange<P, P::RB, P::RC, P::M2, NT, PLANES>(v, xb, t, gid);
     pass_butterflies<P, P::RC, DIR>(v);
   }
+}
+template <class P, int DIR, int NT, bool PLANES = false>
+__device__ __forceinline__ void fft(C2* v, void* xb, int t, int gid, const float2* __restrict__ tw) {
+  fft_head<P, DIR>(v, t, tw);
+  fft_tail<P, DIR, NT, PLANES>(v, xb, t, gid, tw);
 }
 
 }  // namespace rf
