@@ -410,6 +410,99 @@ __global__ void __launch_bounds__(NT, 512 / NT) k2_xinv_direct(Fast2DArgs a, int
   }
 }
 
+// ---------------------------------------------------------------------------------- K_C, persistent
+// The direct-read x inverse as ONE CTA of 512 threads per SM that never waits for its pieces: its NG = 512 / T FFT
+// groups work through the CTA's row pairs (items: component x row pair, blockIdx.x + k gridDim.x) in turn, over a
+// ring of NG + NG/2 landing / exchange buffers. While the groups transform NG items, the pieces of the next NG/2 are
+// landing; a group that is done with a buffer (after the last exchange of its transform) hands it to TMA for the
+// item NBUF steps ahead at once. Each buffer has its mbarrier; the groups synchronise among themselves with named
+// barriers only. 4096^2: 0.190 -> 0.168 ms.
+template <class P>
+struct K2InvP {
+  static constexpr int NT = 512, NG = NT / P::T, NBUF = NG + NG / 2;
+  using S = K2Inv<P, P::T>;                                  // layout of one landing area (G = 1)
+  static constexpr int BUF4 = S::LAND4 > P::XB ? S::LAND4 : P::XB;
+  static constexpr size_t SMEM = sizeof(float4) * (size_t)NBUF * BUF4 + 128;
+};
+
+template <class P>
+__global__ void __launch_bounds__(512, 1) k2_xinv_pers(Fast2DArgs a, int dst_role, const __grid_constant__ CUtensorMap map_even,
+                                                            const __grid_constant__ CUtensorMap map_odd) {
+  if (a.st->skip) return;
+  using PI = typename P::Reversed;
+  using K = K2InvP<P>;
+  using S = typename K::S;
+  constexpr int N = P::N, T = P::T, E = P::E, NT = K::NT, NG = K::NG, KB = S::KB, NBUF = K::NBUF;
+  static_assert(T >= 32 && NG <= 15, "one named barrier per group, whole warps");
+  extern __shared__ __align__(128) float4 smem4[];
+  __shared__ __align__(8) uint64_t full[NBUF];
+  float4* base = reinterpret_cast<float4*>((reinterpret_cast<uintptr_t>(smem4) + 127) & ~(uintptr_t)127);
+  const int tid = threadIdx.x, gid = tid / T, t = tid % T;
+  const int npairs = a.Ny == 0 ? 0 : a.nyp / 2, nitems = 3 * npairs;
+  const int first = blockIdx.x, stride = gridDim.x;
+  const int nq = first < nitems ? (nitems - first + stride - 1) / stride : 0;      // items of this CTA
+  auto issue = [&](int q) {                    // one thread: bring the pieces of the CTA's q-th item into buffer q % NBUF
+    const int item = first + q * stride, c = item / npairs, r0 = 2 * (item - c * npairs);
+    float4* land = base + (size_t)(q % NBUF) * K::BUF4;
+    uint64_t* bar = &full[q % NBUF];
+    tma::mbar_expect_tx(bar, (uint32_t)(S::LAND4 * sizeof(float4)));
+#pragma unroll 1
+    for (int b = 0; b < S::NBE; ++b) tma::load_3d(land + (size_t)b * KB, &map_even, 2 * r0, b * KB, c, bar);
+#pragma unroll 1
+    for (int b = 0; b < S::NBO; ++b) tma::load_3d(land + (size_t)(S::NBE + b) * KB, &map_odd, 2 * r0, b * KB, c, bar);
+  };
+  if (tid == 0) {
+#pragma unroll
+    for (int b = 0; b < NBUF; ++b) tma::mbar_init(&full[b], 1);
+    tma::fence_barrier_init();
+    tma::fence_proxy_async();
+    for (int q = 0; q < NBUF && q < nq; ++q) issue(q);
+  }
+  const float2 wt = __ldg(&a.twox[t]);      // w_2N^t; the other points follow from constants
+  __syncthreads();                          // the barriers are initialised
+#pragma unroll 1
+  for (int q = gid; q < nq; q += NG) {
+    const int item = first + q * stride, c = item / npairs, r0 = 2 * (item - c * npairs);
+    float4* land = base + (size_t)(q % NBUF) * K::BUF4;
+    const float4* Se = land;
+    const float4* So = land + (size_t)S::NBE * KB;
+    tma::mbar_wait(&full[q % NBUF], (q / NBUF) & 1);
+    rf::C2 v[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+      const int n = rf::slot_index<PI, PI::RA>(t, e);        // = t + (N/16) e: the mirror tests fold per e
+      float4 qe, qo;
+      if (e < E / 2) {                      // n < N/2: bins 2n, 2n + 1 < N
+        qe = Se[n]; qo = So[n];
+        v[e] = {make_float2(qe.x - qe.w, qo.x - qo.w), make_float2(qe.y + qe.z, qo.y + qo.z)};
+      } else {                              // bins above N: the conjugate partner 2N - b
+        qo = So[N - 1 - n];
+        qe = Se[N - n];
+        const bool self = e == E / 2 && t == 0;              // bin N itself (n = N/2)
+        v[e] = {make_float2(self ? qe.x - qe.w : qe.x + qe.w, qo.x + qo.w), make_float2(self ? qe.y + qe.z : qe.z - qe.y, qo.z - qo.y)};
+      }
+    }
+    rf::group_sync<T, NT>(gid);             // the group has its points: its landing area becomes its exchange buffer
+    rf::fft<PI, +1, NT>(v, land, t, gid, a.twx_r);
+    // the buffer is free once every thread of the group is past the last exchange: order the generic accesses before
+    // the asynchronous writes that follow, then hand the buffer to TMA for the item three steps ahead
+    tma::fence_proxy_async();
+    rf::group_sync<T, NT>(gid);
+    if (t == 0 && q + NBUF < nq) issue(q + NBUF);
+    float* __restrict__ dst = a.st->ptr[dst_role] + (size_t)c * a.ncell;
+    const size_t rowA = (size_t)r0 * a.nxp;                  // physical row pitch; n >= nxp is zero fill
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+      const int n = rf::slot_index<PI, PI::RLAST>(t, e);
+      const float2 u = rf::cmul_tw1<+1>(make_float2(v[e].re.y, v[e].im.y), rf::half_twiddle(wt, e));
+      if (n < a.nxp) {
+        k2_stg(dst + rowA + n, v[e].re.x + u.x);
+        k2_stg(dst + rowA + a.nxp + n, v[e].im.x + u.y);
+      }
+    }
+  }
+}
+
 // ---------------------------------------------------------------------------------- K_A
 // x forward transform of FOUR rows per FFT group. Two real rows a, b form one complex line z = a + i b; the two
 // lanes of the packed engine carry two such lines (rows r, r+1 and r+2, r+3), and the even-bin and odd-bin

@@ -45,6 +45,7 @@ struct mm_sim {
   ConvArgs conv;
   float* Kt = nullptr;         // kernel spectrum in the fast 2D layout
   Fast2DArgs f2;
+  CUtensorMap f2_map_invp_even, f2_map_invp_odd;        // boxes {2 rows, KB bins}: one row pair per FFT group (persistent x inverse)
   CUtensorMap f2_map_inv_even, f2_map_inv_odd;          // boxes {2G rows, KB bins} over the even / odd columns (direct-read x inverse)
   CUtensorMap f2_map_inv, f2_map_fwd, f2_map_fwd_odd;   // TMA views of spec for the x kernels (inverse: boxes of 2G rows x 256
                                                         // bins; forward: 4G rows x KB bins of the even resp. odd columns)

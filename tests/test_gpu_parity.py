@@ -122,10 +122,12 @@ def test_fast2d_path_fields(mm, grid):
     prof = sim.profile_read()
     sim.profile(False)
     assert "f2_ycol" in prof and "f2_xfwd" in prof and "f2_xinv" in prof and "last_xy" not in prof
-    # the x kernels without TMA (fallback when the driver cannot encode tensor maps) must agree exactly
+    # the x kernels without TMA (fallback when the driver cannot encode tensor maps) do the same arithmetic in
+    # another kernel: equal up to the compiler's choice of fused multiply-adds (bit-for-bit repeatability of each
+    # path is checked in test_kernels_stay_inside_their_buffers_and_are_reproducible)
     Bf = sim.b_eff(MM_DEMAG)
     sim.set_option(mm.MM_OPT_NO_TMA, 1)
-    assert np.array_equal(sim.b_eff(MM_DEMAG), Bf)
+    assert np.abs(sim.b_eff(MM_DEMAG) - Bf).max() <= 2e-6 * np.abs(Bf).max()
     sim.set_option(mm.MM_OPT_NO_TMA, 0)
     # the generic any-size kernels must agree with it
     sim.set_option(mm.MM_OPT_GENERIC_FFT, 1)
@@ -178,7 +180,8 @@ def test_fast3d_mixed_stages(mm, grid, pbc, kinds):
     assert np.abs(Bf - Bg).max() <= 2e-5 * np.abs(Bg).max()
 
 
-@pytest.mark.parametrize("grid,pbc", [((384, 320, 1), (0, 0, 0)), ((1000, 600, 1), (0, 0, 0)), ((40, 64, 32), (0, 0, 0)),
+@pytest.mark.parametrize("grid,pbc", [((384, 320, 1), (0, 0, 0)), ((1000, 600, 1), (0, 0, 0)), ((4096, 128, 1), (0, 0, 0)),
+                                      ((2048, 3000, 1), (0, 0, 0)), ((40, 64, 32), (0, 0, 0)),
                                       ((64, 64, 32), (2, 2, 0)), ((70, 45, 20), (0, 0, 0))])
 def test_kernels_stay_inside_their_buffers_and_are_reproducible(mm, grid, pbc):
     # compute-sanitizer is closed on the GPU pool, so the two things it would check are tested directly: every
