@@ -19,7 +19,7 @@ MM_OPT_NO_GRAPH = 3
 MM_RK45, MM_RK23, MM_RK12 = 0, 1, 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("MM_B200_LIB") or os.path.join(_HERE, "libmm_b200.so")
+LIB_PATH = os.environ.get("MM_B200_LIB") or os.path.join(_HERE, "libmm_b200.so")     # (the variable: another build of the same library)
 _lib_handle = None
 
 

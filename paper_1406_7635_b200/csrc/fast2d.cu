@@ -11,13 +11,7 @@ namespace {
 // the CTA size NT; a CTA holds G = NT / T FFT groups and therefore 2G rows in the x kernels
 template <int N> struct PlanFor;
 // (NTF: CTA size of the forward x kernel, four rows per FFT group; NTI: of the inverse one, two rows per group)
-#ifndef MM_X4096_NTF
-#define MM_X4096_NTF 256
-#endif
-#ifndef MM_X4096_NTI
-#define MM_X4096_NTI 256
-#endif
-template <> struct PlanFor<4096> { using P = rf::Plan<4096, 256, 16, 16, 16>; static constexpr int NT = 256, NTF = MM_X4096_NTF, NTI = MM_X4096_NTI; };
+template <> struct PlanFor<4096> { using P = rf::Plan<4096, 256, 16, 16, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
 template <> struct PlanFor<2048> { using P = rf::Plan<2048, 128, 16, 8, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
 template <> struct PlanFor<1024> { using P = rf::Plan<1024, 64, 16, 4, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };
 template <> struct PlanFor<512> { using P = rf::Plan<512, 32, 16, 2, 16>; static constexpr int NT = 256, NTF = 256, NTI = 256; };

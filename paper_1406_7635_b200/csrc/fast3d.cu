@@ -15,11 +15,9 @@ template <> struct Plan3<512> { using P = rf::Plan<512, 32, 16, 2, 16>; };
 
 // lines per CTA: 256 threads in the y stage, 3 x 128 in the fused z stage
 template <int N> constexpr int cy() { return 256 / Plan3<N>::P::T; }
-#ifndef MM_F3_ZTHREADS
-#define MM_F3_ZTHREADS 128
-#endif
-template <int N> constexpr int cz() { return MM_F3_ZTHREADS / Plan3<N>::P::T; }
-constexpr int kZMinBlocks = MM_F3_ZTHREADS == 128 ? 1 : 3;
+// (64 threads per component, i.e. 192-thread CTAs, three per SM, need 96 registers and spill: 1.04 -> 1.24 ms at 256^3)
+template <int N> constexpr int cz() { return 128 / Plan3<N>::P::T; }
+constexpr int kZMinBlocks = 1;
 template <int N> constexpr size_t smem_y() { return sizeof(float4) * (size_t)N * cy<N>(); }
 template <int N> constexpr size_t smem_z() { return K3Z<typename Plan3<N>::P, cz<N>()>::SMEM; }
 
