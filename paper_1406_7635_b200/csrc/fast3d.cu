@@ -15,9 +15,12 @@ template <> struct Plan3<512> { using P = rf::Plan<512, 32, 16, 2, 16>; };
 
 // lines per CTA: 256 threads in the y stage, 3 x 128 in the fused z stage
 template <int N> constexpr int cy() { return 256 / Plan3<N>::P::T; }
-// (64 threads per component, i.e. 192-thread CTAs, three per SM, need 96 registers and spill: 1.04 -> 1.24 ms at 256^3)
-template <int N> constexpr int cz() { return 128 / Plan3<N>::P::T; }
-constexpr int kZMinBlocks = 1;
+// Long lines: 128 threads per component, one CTA of 384 threads per SM. 64 threads per component (192-thread CTAs,
+// three per SM at 96 registers, with spills) lose at 256 points (1.04 -> 1.24 ms at 256^3) but win for short lines,
+// where a CTA is mostly latency (C3, Nz = 32: 0.048 -> 0.037 ms).
+template <int N> constexpr int zthreads() { return N <= 64 ? 64 : 128; }
+template <int N> constexpr int cz() { return zthreads<N>() / Plan3<N>::P::T; }
+template <int N> constexpr int zminb() { return N <= 64 ? 3 : 1; }
 template <int N> constexpr size_t smem_y() { return sizeof(float4) * (size_t)N * cy<N>(); }
 template <int N> constexpr size_t smem_z() { return K3Z<typename Plan3<N>::P, cz<N>()>::SMEM; }
 
@@ -33,7 +36,7 @@ int attrs_y(mm_sim* s) {
 template <int N>
 int attrs_z(mm_sim* s) {
   using P = typename Plan3<N>::P;
-  CUDA_TRY(s, cudaFuncSetAttribute(k3_z<P, cz<N>(), kZMinBlocks>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_z<N>()));
+  CUDA_TRY(s, cudaFuncSetAttribute(k3_z<P, cz<N>(), zminb<N>()>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_z<N>()));
   // the kernel spectrum in the tile order of the z stage
   constexpr int C = cz<N>();
   const Geometry& g = s->g;
@@ -66,7 +69,7 @@ void launch_z(mm_sim* s) {
   using P = typename Plan3<N>::P;
   constexpr int C = cz<N>();
   const dim3 grid((s->g.Cx + C - 1) / C, s->g.Py);
-  k3_z<P, C, kZMinBlocks><<<grid, 3 * P::T * C, smem_z<N>(), s->stream>>>(s->f3);
+  k3_z<P, C, zminb<N>()><<<grid, 3 * P::T * C, smem_z<N>(), s->stream>>>(s->f3);
 }
 
 template <int N> constexpr int gx() { return 256 / Plan3<N>::P::T; }
