@@ -15,12 +15,15 @@ template <> struct Plan3<512> { using P = rf::Plan<512, 32, 16, 2, 16>; };
 
 // lines per CTA: 256 threads in the y stage, 3 x 128 in the fused z stage
 template <int N> constexpr int cy() { return 256 / Plan3<N>::P::T; }
-// Long lines: 128 threads per component, one CTA of 384 threads per SM. 64 threads per component (192-thread CTAs,
-// three per SM at 96 registers, with spills) lose at 256 points (1.04 -> 1.24 ms at 256^3) but win for short lines,
-// where a CTA is mostly latency (C3, Nz = 32: 0.048 -> 0.037 ms).
-template <int N> constexpr int zthreads() { return N <= 64 ? 64 : 128; }
+// CTA shape of the fused z stage, measured per line length (threads per component, CTAs per SM):
+//   512 points: 128 threads (C = 4 lines), one CTA of 384 threads per SM (fewer lines per CTA would mean 16-byte pieces);
+//   128, 256 : 64 threads (C = 8 / 4), two CTAs of 192 threads at 167 registers - two independent CTAs overlap their
+//              phases where one of 384 threads cannot (128^3: 0.138 -> 0.109 ms, 256^3 with PBC: 0.300 -> 0.254 ms,
+//              256^3 open: unchanged);
+//   32, 64   : 64 threads, three CTAs at 96 registers (spills, but a short-line CTA is mostly latency: C3 0.048 -> 0.037 ms).
+template <int N> constexpr int zthreads() { return N >= 512 ? 128 : 64; }
 template <int N> constexpr int cz() { return zthreads<N>() / Plan3<N>::P::T; }
-template <int N> constexpr int zminb() { return N <= 64 ? 3 : 1; }
+template <int N> constexpr int zminb() { return N <= 64 ? 3 : (N >= 512 ? 1 : 2); }
 template <int N> constexpr size_t smem_y() { return sizeof(float4) * (size_t)N * cy<N>(); }
 template <int N> constexpr size_t smem_z() { return K3Z<typename Plan3<N>::P, cz<N>()>::SMEM; }
 
