@@ -14,7 +14,10 @@ template <> struct Plan3<256> { using P = rf::Plan<256, 16, 16, 16, 1>; };
 template <> struct Plan3<512> { using P = rf::Plan<512, 32, 16, 2, 16>; };
 
 // lines per CTA: 256 threads in the y stage, 3 x 128 in the fused z stage
-template <int N> constexpr int cy() { return 256 / Plan3<N>::P::T; }
+// lines per CTA. Several small CTAs per SM overlap their phases better than few large ones (measured at 256^3 and 128^3):
+// 128 threads in the y stage (0.254 -> 0.242 ms, 0.041 -> 0.034 ms), in the x inverse (0.161 -> 0.134 ms) and in the
+// periodic x forward kernel (0.123 -> 0.110 ms); the open x forward kernel keeps 256 (0.223 ms; 0.254 ms with 128).
+template <int N> constexpr int cy() { return 128 / Plan3<N>::P::T; }
 // CTA shape of the fused z stage, measured per line length (threads per component, CTAs per SM):
 //   512 points: 128 threads (C = 4 lines), one CTA of 384 threads per SM (fewer lines per CTA would mean 16-byte pieces);
 //   128, 256 : 64 threads (C = 8 / 4), two CTAs of 192 threads at 167 registers - two independent CTAs overlap their
@@ -75,12 +78,14 @@ void launch_z(mm_sim* s) {
   k3_z<P, C, zminb<N>()><<<grid, 3 * P::T * C, smem_z<N>(), s->stream>>>(s->f3);
 }
 
-template <int N> constexpr int gx() { return 256 / Plan3<N>::P::T; }
+template <int N> constexpr int gxf() { return 256 / Plan3<N>::P::T; }      // x forward, open axis
+template <int N> constexpr int gx() { return 128 / Plan3<N>::P::T; }       // x inverse, periodic x forward
 template <int N> constexpr size_t smem_x() { return sizeof(float4) * (size_t)f3::row_pitch<typename Plan3<N>::P>() * gx<N>(); }
+template <int N> constexpr size_t smem_xf() { return sizeof(float4) * (size_t)f3::row_pitch<typename Plan3<N>::P>() * gxf<N>(); }
 template <int N>
 int attrs_x(mm_sim* s) {
   using P = typename Plan3<N>::P;
-  CUDA_TRY(s, cudaFuncSetAttribute(k3_xfwd<P, gx<N>()>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_x<N>()));
+  CUDA_TRY(s, cudaFuncSetAttribute(k3_xfwd<P, gxf<N>()>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_xf<N>()));
   CUDA_TRY(s, cudaFuncSetAttribute(k3_xinv<P, gx<N>()>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_x<N>()));
   CUDA_TRY(s, cudaFuncSetAttribute(k3_xfwd_p<P, gx<N>()>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_x<N>()));
   CUDA_TRY(s, cudaFuncSetAttribute(k3_xinv_p<P, gx<N>()>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_x<N>()));
@@ -89,16 +94,16 @@ int attrs_x(mm_sim* s) {
 template <int N>
 void launch_x(mm_sim* s, bool inverse, int role) {
   using P = typename Plan3<N>::P;
-  constexpr int G = gx<N>();
   const bool periodic = s->f3.mode[0] == 2;
   const int nlines = s->g.Ny * s->g.Nz / (periodic ? 4 : 2);      // row pairs, or row quadruples on a periodic axis
-  const dim3 grid((nlines + G - 1) / G, 3);
+  constexpr int G = gx<N>(), GF = gxf<N>();
+  const dim3 grid((nlines + G - 1) / G, 3), gridf((nlines + GF - 1) / GF, 3);
   if (periodic) {
     if (inverse) k3_xinv_p<P, G><<<grid, P::T * G, smem_x<N>(), s->stream>>>(s->f3, role);
     else k3_xfwd_p<P, G><<<grid, P::T * G, smem_x<N>(), s->stream>>>(s->f3, role);
   } else {
     if (inverse) k3_xinv<P, G><<<grid, P::T * G, smem_x<N>(), s->stream>>>(s->f3, role);
-    else k3_xfwd<P, G><<<grid, P::T * G, smem_x<N>(), s->stream>>>(s->f3, role);
+    else k3_xfwd<P, GF><<<gridf, P::T * GF, smem_xf<N>(), s->stream>>>(s->f3, role);
   }
 }
 
