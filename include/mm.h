@@ -237,6 +237,23 @@ int mm_get_time(mm_sim* sim, double* t);
 int mm_set_time(mm_sim* sim, double t);
 /* Plain mean of m over all cells (fp64 accumulation), the paper's m.average() (L861). */
 int mm_get_avg_m(mm_sim* sim, double avg[3]);
+/* The same mean (m.average(), L861) for callers that cannot allocate device memory - code under CUDA-graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc. Needs no handle and calls no cudaMalloc, cudaFree
+ * or allocating library routine: the per-block partial sums live in one file-scope device array of 196 864 bytes
+ * that every GPU loading the library holds until the process exits.
+ *   m_dev      DEVICE pointer, 3 * ncells floats, [component][cell] as everywhere in this header (caller-owned, read)
+ *   ncells     1 .. MM_NOALLOC_MAX_CELLS; beyond -> MM_EINVAL (the scratch array holds one partial per 8192 cells)
+ *   avg_dev    DEVICE pointer, 3 doubles: the mean of each component, fp64 accumulation in an order fixed by ncells
+ *              alone (same field -> same bits on any device)
+ *   cuda_stream a cudaStream_t (NULL = the default stream); a 4-byte memset and one kernel are enqueued on it, the
+ *              call does not synchronise. The device owning the stream and both buffers must be current.
+ *   errbuf     optional host buffer of errlen bytes for the text of a failure (may be NULL)
+ * The scratch array is shared by EVERY call in the process and keeps the last call's contents (the library clears
+ * what must start at zero): calls that overlap on the GPU - different streams without ordering, concurrent graph
+ * branches - race on it; order them. The first call on each device looks the array's address up
+ * (cudaGetSymbolAddress): make it before starting a capture. */
+#define MM_NOALLOC_MAX_CELLS 67108864LL /* 2^26 cells = 8192 x 8192 (a 4096^2 film or a 256^3 cube is 2^24) */
+int mm_avg_m_noalloc(const float* m_dev, long long ncells, double* avg_dev, void* cuda_stream, char* errbuf, size_t errlen);
 /* Counters: accepted steps, rejected attempts, torque evaluations, peak device bytes owned. */
 int mm_get_stats(mm_sim* sim, long* steps, long* rejected, long* evals, size_t* peak_device_bytes);
 /* Device bytes the handle owns now and the most it ever owned (the fp64 scratch of the kernel set-up is freed

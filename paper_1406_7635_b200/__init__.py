@@ -88,6 +88,7 @@ _SIGNATURES = {
     "mm_get_time": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
     "mm_set_time": (C.c_int, [C.c_void_p, C.c_double]),
     "mm_get_avg_m": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
+    "mm_avg_m_noalloc": (C.c_int, [C.c_void_p, C.c_longlong, C.c_void_p, C.c_void_p, C.c_char_p, C.c_size_t]),
     "mm_get_stats": (C.c_int, [C.c_void_p, C.POINTER(C.c_long), C.POINTER(C.c_long), C.POINTER(C.c_long),
                                C.POINTER(C.c_size_t)]),
     "mm_get_memory": (C.c_int, [C.c_void_p, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]),
@@ -416,6 +417,18 @@ def batch_run(sims, duration):
 def batch_relax(sims):
     arr, cnt = _handles(sims)
     _check(lib().mm_batch_relax(arr, cnt))
+
+
+MM_NOALLOC_MAX_CELLS = 1 << 26
+
+
+def avg_m_noalloc(m_dev, avg_dev, stream=None):
+    """mm_avg_m_noalloc: mean of the device field `m_dev` (torch CUDA tensor, 3N floats) into `avg_dev` (torch CUDA
+    tensor, 3 doubles) on `stream` (a raw cudaStream_t or None); allocates nothing and does not synchronise."""
+    err = C.create_string_buffer(256)
+    code = lib().mm_avg_m_noalloc(_ptr(m_dev), m_dev.numel() // 3, _ptr(avg_dev), C.c_void_p(stream or 0), err, len(err))
+    if code != MM_OK:
+        raise MMError(code, lib().mm_strerror(code).decode() + " (" + err.value.decode() + ")")
 
 
 def from_config(cfg, **kw):
