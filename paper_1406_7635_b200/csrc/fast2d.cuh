@@ -138,7 +138,7 @@ constexpr size_t k2_y_smem() { return (size_t)(NT / P::T) * K2YShape<P>::GROUP_B
 // a register permutation through local memory).
 // Two CTAs share an SM: butterflies of one over the exchanges and loads of the other. (Forcing the phases apart - two
 // groups per CTA taking turns in their exchanges by named-barrier tokens, or a start offset between the CTAs of an
-// SM - was measured and is slower or neutral, profiles/r02_experiments.md.)
+// SM - was measured and is slower or neutral.)
 template <class P, int NT>
 struct K2Col {
   using PI = typename P::Reversed;
