@@ -239,6 +239,13 @@ void launch_local(mm_sim* s, int src_role, int dst_role, unsigned mask, int out_
                                                        out_torque);
 }
 
+// stage input / new state from m0 and the slopes (k_stage; four cells per thread where the components stay 16-byte aligned)
+void launch_stage(mm_sim* s, const StageCoef& sc, int dst_role) {
+  const long long N = s->g.N;
+  if (N % 4 == 0) k_stage4<<<blocks_for(N / 4, 256), 256, 0, s->stream>>>(N, s->dstate, sc, dst_role);
+  else k_stage<<<blocks_for(N, 256), 256, 0, s->stream>>>(N, s->dstate, sc, dst_role);
+}
+
 void enqueue_step(mm_sim* s) {
   const long long N = s->g.N;
   const int tq = s->precession ? 1 : 2;                       // torque with / without the precession term
@@ -252,10 +259,10 @@ void enqueue_step(mm_sim* s) {
     StageCoef sc;
     for (int j = 0; j < 6; ++j) sc.a[j] = 0.f;
     sc.n = 1; sc.a[0] = 1.f;
-    { Launch l(s, KK_STAGE); k_stage<<<blocks_for(N, 256), 256, 0, s->stream>>>(N, s->dstate, sc, R_Y); }
+    { Launch l(s, KK_STAGE); launch_stage(s, sc, R_Y); }
     launch_eval(s, R_Y, R_K1, mask, tq);
     sc.n = 2; sc.a[0] = 0.5f; sc.a[1] = 0.5f;
-    { Launch l(s, KK_STAGE); k_stage<<<blocks_for(N, 256), 256, 0, s->stream>>>(N, s->dstate, sc, R_MNEW); }
+    { Launch l(s, KK_STAGE); launch_stage(s, sc, R_MNEW); }
     ErrCoef ec;
     for (int j = 0; j < 7; ++j) ec.e[j] = 0.f;
     ec.e[0] = -0.5f; ec.e[1] = 0.5f;                          // 2nd-order minus Euler weights
@@ -286,7 +293,7 @@ void enqueue_step(mm_sim* s) {
     // last one reduces the error norm: ns + 1 fewer launches, no slope is read back right after it is written
     const StageCoef s1 = row(1);
     int cur = (ns == 2) ? R_MNEW : R_Y;
-    { Launch l(s, KK_STAGE); k_stage<<<blocks_for(N, 256), 256, 0, s->stream>>>(N, s->dstate, s1, cur); }
+    { Launch l(s, KK_STAGE); launch_stage(s, s1, cur); }
     for (int i = 1; i < ns; ++i) {
       if (i < ns - 1) {
         const StageCoef sn = row(i + 1);
@@ -301,7 +308,7 @@ void enqueue_step(mm_sim* s) {
     for (int i = 1; i < ns; ++i) {
       const StageCoef sc = row(i);
       const int yrole = (i == ns - 1) ? R_MNEW : R_Y;
-      { Launch l(s, KK_STAGE); k_stage<<<blocks_for(N, 256), 256, 0, s->stream>>>(N, s->dstate, sc, yrole); }
+      { Launch l(s, KK_STAGE); launch_stage(s, sc, yrole); }
       launch_eval(s, yrole, R_K0 + i, s->terms, tq);
     }
     { Launch l(s, KK_ERROR); k_error<<<s->nsm * 8, 256, 0, s->stream>>>(N, s->dstate, ec); }
